@@ -1,0 +1,164 @@
+/* ks.h — C ABI of libks: batched per-kernel latency prediction + serving-step composition,
+ * the data-parallel hot path of KernelSight-LM (arxiv 2606.28565), on one B200 (sm_100a).
+ *
+ * Citations are PAPER.md:<line> (the paper text) or DESIGN.md §3 Q<n> (a stated reading where the
+ * paper is silent).  Everything here runs in hand-written CUDA kernels; there is no CPU fallback:
+ * every call fails with KS_ECUDA if no sm_100 device/context can be used.
+ *
+ * Model (Eq. 2):   t = max(t_roof * eta, t0),
+ *                               t_roof = max(F_comp / P_peak * u, F_mem / BW_peak),
+ *   u = ceil(B/S) * S / B  with S = n_sm * ctas_per_sm CTA slots (Fig. 2; Q4),
+ *   eta = 1/e, e in (0,1] from a per-family MLP head over dimensionless features (Tier A,
+ *   PAPER.md:199-201) or from trilinear interpolation in a measured efficiency grid (Tier B,
+ *   PAPER.md:211), or e = 1 (KS_TIER_NONE).
+ * Step composition (Eq. 4):
+ *   t_gpu = body_scale * sum_k t_k ;  t_step = max(t_gpu + n c_disp, l) + max(0, c_ovl - t_gpu) + c_tail.
+ *
+ * Conventions
+ *  - Ownership: the library owns only what ks_load_* copies and its internal workspace.  Every
+ *    descriptor/offset/output buffer is caller-owned and only borrowed for the duration of the call.
+ *  - Memory space: each compute call takes a ks_mem_space saying where ALL its array arguments
+ *    (columns, offsets, outputs) live.  KS_MEM_DEVICE: device pointers on the ctx device, 16-byte
+ *    aligned; work is enqueued on the ctx stream and the call returns without synchronising.
+ *    KS_MEM_HOST: host pointers (pinned or pageable); the library copies inputs to its device
+ *    workspace, runs the same kernels, copies results back and synchronises the stream before
+ *    returning.  Host structs (ks_desc_batch, ks_hw_spec, ks_step_params, pointer arrays) are always
+ *    host memory and are read during the call only.
+ *  - Errors: every function returns a ks_status; nothing throws or aborts.  Arguments are validated
+ *    before anything is enqueued: on KS_EINVAL / KS_ESTATE / KS_EUNSUPPORTED nothing was written.
+ *    A CUDA failure returns KS_ECUDA and is sticky until ks_destroy.
+ *  - Determinism: no floating-point atomics; identical inputs give bit-identical outputs.
+ */
+#ifndef KS_H
+#define KS_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define KS_API __attribute__((visibility("default")))
+#else
+#define KS_API
+#endif
+
+typedef struct ks_ctx ks_ctx;   /* opaque; owns device copies of heads and grids + workspace */
+
+typedef enum { KS_OK = 0, KS_EINVAL = 1, KS_ENOMEM = 2, KS_ECUDA = 3, KS_ESTATE = 4, KS_EUNSUPPORTED = 5 } ks_status;
+typedef enum { KS_FAM_GEMM = 0, KS_FAM_GROUPED_GEMM = 1, KS_FAM_ATTN = 2, KS_FAM_ELEMWISE = 3, KS_FAM_COUNT = 4 } ks_family;
+typedef enum { KS_TIER_NONE = 0, KS_TIER_A = 1, KS_TIER_B = 2 } ks_tier;
+typedef enum { KS_COL_I32 = 0, KS_COL_F32 = 1 } ks_col_dtype;   /* F32 columns must hold exact integers < 2^24 */
+typedef enum { KS_MEM_DEVICE = 0, KS_MEM_HOST = 1 } ks_mem_space;
+
+#define KS_MAX_COLS 10      /* grouped GEMM: N, K, m_0..m_7 */
+#define KS_MAX_BATCHES 8    /* family buckets per call */
+#define KS_N_EXPERTS 8
+#define KS_MAX_GRID_NODES 32768   /* a Tier-B grid is staged whole in shared memory (128 KiB fp32) */
+
+/* Hardware-spec vector (peak compute, peak bandwidth, SM count, cache sizes; Table 5
+ * PAPER.md:473-487).  tile_*, ctas_per_sm, ew_elems_per_cta parameterise the CTA count B (Q1, Q4);
+ * t0 is the launch floor of Eq. 2.  All integer fields must be >= 1. */
+typedef struct {
+  float peak_flops;        /* FLOP/s for the descriptor dtype */
+  float peak_bw;           /* bytes/s */
+  int32_t n_sm, ctas_per_sm, tile_m, tile_n, ew_elems_per_cta;
+  float l2_bytes;          /* L2 capacity in bytes */
+  float t0;                /* launch floor, seconds (>= 0) */
+} ks_hw_spec;
+
+/* One family bucket of kernel-instance descriptors in SoA form.
+ * Column meaning by family (all values non-negative integers):
+ *   KS_FAM_GEMM          cols = {M, N, K}
+ *   KS_FAM_GROUPED_GEMM  cols = {N, K, m_0, ..., m_7}   tokens per expert, shared N, K
+ *   KS_FAM_ATTN          cols = {batch, q_len, kv_len}  causal, kv_len >= q_len (smaller kv is raised to q);
+ *                        attn_hq / attn_hkv / attn_head_dim are per-bucket constants
+ *   KS_FAM_ELEMWISE      cols = {n_elements, subop}     subop: 0 RMSNorm, 1 SiLU*Mul, 2 RoPE,
+ *                        3 KV-cache write, 4 embedding, 5 residual add (out-of-range is clamped)
+ * Each column has n elements of col_dtype; pointers live in the call's ks_mem_space. */
+typedef struct {
+  int32_t family;          /* ks_family */
+  int32_t n;               /* rows; 0 is a legal no-op */
+  int32_t col_dtype;       /* ks_col_dtype */
+  int32_t dtype_bytes;     /* s: bytes per tensor element of the modelled kernel (1, 2 or 4) */
+  int32_t n_cols;          /* columns supplied; must equal the family's count */
+  int32_t attn_hq, attn_hkv, attn_head_dim;
+  const void *cols[KS_MAX_COLS];
+} ks_desc_batch;
+
+/* Host-overlap constants of Eq. 4; body_scale multiplies sum t (Q7). */
+typedef struct { float c_disp, floor_l, c_ovl, c_tail, body_scale; } ks_step_params;
+
+/* Create a context on `device`.  `cuda_stream` is a borrowed cudaStream_t (NULL = legacy default
+ * stream) on which all work of this context is enqueued.  KS_ECUDA if the device is not sm_100. */
+KS_API ks_status ks_create(ks_ctx **out, int device, void *cuda_stream);
+
+/* Load (or replace) the Tier-A efficiency head of `family`: MLP n_in -> h1 -> h2 -> 1 with GELU
+ * hidden activations and a sigmoid output giving the efficiency e (sizes and
+ * activations BASELINE.json; Q3, Q6).  All arrays are HOST fp32 and are copied: W1[n_in][h1],
+ * b1[h1], W2[h1][h2], b2[h2], w3[h2].  Weights are rounded to bf16 (RNE) for the tensor-core
+ * contraction; biases keep >= 16 significant bits.  The feature vector is fixed by the library
+ * (Q2): n_in must be 8, 12 or 32.  Supported hidden sizes: h1 == h2 in {64, 128, 256};
+ * anything else returns KS_EUNSUPPORTED. */
+KS_API ks_status ks_load_heads(ks_ctx *ctx, ks_family family, int n_in, int h1, int h2, const float *W1,
+                        const float *b1, const float *W2, const float *b2, const float *w3, float b3);
+
+/* Load (or replace) the Tier-B measured-efficiency grid of `family` (Q5).
+ * values: HOST fp32 [dims[0]][dims[1]][dims[2]], last index fastest, copied; each dims[a] >= 1 and
+ * the product <= KS_MAX_GRID_NODES.  Axis a spans [lo_log2[a], hi_log2[a]] in log2 units with
+ * dims[a] uniformly spaced nodes; queries are clamped to the span.  Axis values per family:
+ * GEMM (M, N, K); GROUPED (sum m_e, N, K); ATTN (batch, q_len, kv_len); ELEMWISE (n, 2^subop, 1). */
+KS_API ks_status ks_load_grid(ks_ctx *ctx, ks_family family, const int32_t dims[3], const float lo_log2[3],
+                       const float hi_log2[3], const float *values);
+
+/* Predict the latency of every (spec, descriptor) pair (steps S1-S5 of DESIGN.md §1).
+ *   batches[n_batches]   family buckets (<= KS_MAX_BATCHES)
+ *   specs[n_specs]       hardware-spec vectors (host)
+ *   tier                 KS_TIER_NONE (e = 1), KS_TIER_A (heads), KS_TIER_B (grids, clamped)
+ *   latency[b]           out, fp32 [n_specs][batches[b].n] seconds
+ *   tiles[b], waves[b]   optional out (array pointer or entry may be NULL), int32 [n_specs][n]:
+ *                        CTA count B and wave count W = ceil(B/S)
+ *   t_roof[b]            optional out, fp32 [n_specs][n]
+ * KS_ESTATE if the tier needs a head/grid that was not loaded for a bucket's family. */
+KS_API ks_status ks_predict_kernels(ks_ctx *ctx, const ks_desc_batch *batches, int n_batches,
+                             const ks_hw_spec *specs, int n_specs, ks_tier tier, ks_mem_space space,
+                             float *const *latency, int32_t *const *tiles, int32_t *const *waves,
+                             float *const *t_roof);
+
+/* Compose per-kernel latencies into per-step and per-configuration latencies (S6-S7).
+ *   latency[b]      fp32 [n_specs][batch_n[b]] as written by ks_predict_kernels
+ *   step_off[b]     int32 CSR [n_steps+1]: rows [step_off[b][s], step_off[b][s+1]) of bucket b
+ *                   belong to step s (non-decreasing; step_off[b][n_steps] <= batch_n[b])
+ *   cfg_off         int32 CSR [n_cfg+1] over steps (may be NULL iff n_cfg == 0)
+ *   step_latency    out fp32 [n_specs][n_steps]   (Eq. 4)
+ *   cfg_latency     out fp32 [n_specs][n_cfg]     (sum of step latencies, accumulated in fp64) */
+KS_API ks_status ks_compose_steps(ks_ctx *ctx, const float *const *latency, const int32_t *const *step_off,
+                           const int32_t *batch_n, int n_batches, int n_steps, int n_specs,
+                           const ks_step_params *params, const int32_t *cfg_off, int n_cfg,
+                           ks_mem_space space, float *step_latency, float *cfg_latency);
+
+/* Convenience: ks_predict_kernels followed by ks_compose_steps in one call (one pass of the whole
+ * hot path).  latency may be NULL (or hold NULL entries): per-kernel latencies then stay in the
+ * library workspace and only the step/config results are returned.  With KS_MEM_HOST this is the
+ * end-to-end call: descriptors and offsets go host->device, results device->host, then sync. */
+KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const int32_t *const *step_off,
+                       int n_batches, const ks_hw_spec *specs, int n_specs, ks_tier tier, int n_steps,
+                       const ks_step_params *params, const int32_t *cfg_off, int n_cfg,
+                       ks_mem_space space, float *const *latency, float *step_latency, float *cfg_latency);
+
+/* Counters: number of kernel launches this context has enqueued so far (for gpu_launches). */
+KS_API ks_status ks_get_launch_count(ks_ctx *ctx, int64_t *out);
+
+/* Tier-A activation mode: 0 = fp32 tanh-form GELU (default, most accurate),
+ * 1 = packed bf16x2 tanh-form GELU (faster; see DESIGN.md §5 for measured error). */
+KS_API ks_status ks_set_gelu_mode(ks_ctx *ctx, int mode);
+
+/* Free everything the context owns.  NULL is a no-op returning KS_OK. */
+KS_API ks_status ks_destroy(ks_ctx *ctx);
+
+KS_API const char *ks_status_string(ks_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,226 @@
+"""Thin ctypes binding over libks (include/ks.h).  Argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; this module converts numpy
+arrays / torch tensors into pointers and structs.  PyTorch is used for device memory and streams
+only.  There is no CPU fallback: if libks.so is missing or no sm_100 device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libks.so")
+
+KS_OK, KS_EINVAL, KS_ENOMEM, KS_ECUDA, KS_ESTATE, KS_EUNSUPPORTED = range(6)
+KS_FAM_GEMM, KS_FAM_GROUPED_GEMM, KS_FAM_ATTN, KS_FAM_ELEMWISE = range(4)
+KS_TIER_NONE, KS_TIER_A, KS_TIER_B = range(3)
+KS_COL_I32, KS_COL_F32 = 0, 1
+KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
+KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
+EXPORTS = ["ks_create", "ks_load_heads", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
+           "ks_run_steps", "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
+
+
+class KsError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)}")
+
+
+class ks_hw_spec(C.Structure):
+    _fields_ = [("peak_flops", C.c_float), ("peak_bw", C.c_float), ("n_sm", C.c_int32),
+                ("ctas_per_sm", C.c_int32), ("tile_m", C.c_int32), ("tile_n", C.c_int32),
+                ("ew_elems_per_cta", C.c_int32), ("l2_bytes", C.c_float), ("t0", C.c_float)]
+
+
+class ks_desc_batch(C.Structure):
+    _fields_ = [("family", C.c_int32), ("n", C.c_int32), ("col_dtype", C.c_int32), ("dtype_bytes", C.c_int32),
+                ("n_cols", C.c_int32), ("attn_hq", C.c_int32), ("attn_hkv", C.c_int32),
+                ("attn_head_dim", C.c_int32), ("cols", C.c_void_p * KS_MAX_COLS)]
+
+
+class ks_step_params(C.Structure):
+    _fields_ = [("c_disp", C.c_float), ("floor_l", C.c_float), ("c_ovl", C.c_float), ("c_tail", C.c_float),
+                ("body_scale", C.c_float)]
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen libks.so (built in-tree by ``python -m paper_2606_28565_b200.build``). Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: build the CUDA library first "
+                           "(python -m paper_2606_28565_b200.build). There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, fp = C.c_void_p, C.c_int, C.POINTER(C.c_float)
+    L.ks_create.argtypes = [C.POINTER(vp), i32, vp]
+    L.ks_load_heads.argtypes = [vp, i32, i32, i32, i32, fp, fp, fp, fp, fp, C.c_float]
+    L.ks_load_grid.argtypes = [vp, i32, C.POINTER(C.c_int32), fp, fp, fp]
+    L.ks_predict_kernels.argtypes = [vp, C.POINTER(ks_desc_batch), i32, C.POINTER(ks_hw_spec), i32, i32, i32,
+                                     C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    L.ks_compose_steps.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int32), i32, i32, i32,
+                                   C.POINTER(ks_step_params), vp, i32, i32, vp, vp]
+    L.ks_run_steps.argtypes = [vp, C.POINTER(ks_desc_batch), C.POINTER(vp), i32, C.POINTER(ks_hw_spec), i32, i32,
+                               i32, C.POINTER(ks_step_params), vp, i32, i32, C.POINTER(vp), vp, vp]
+    L.ks_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.ks_set_gelu_mode.argtypes = [vp, i32]
+    L.ks_destroy.argtypes = [vp]
+    L.ks_status_string.argtypes = [i32]
+    L.ks_status_string.restype = C.c_char_p
+    for name in EXPORTS[:-1]:
+        getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def status_string(s: int) -> str:
+    return load().ks_status_string(int(s)).decode()
+
+
+def _check(st: int, where: str):
+    if st != KS_OK:
+        raise KsError(st, where)
+
+
+def _ptr(a) -> Optional[int]:
+    """Address of a numpy array or torch tensor (None -> NULL)."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return int(a.data_ptr())
+
+
+def _is_host(a) -> bool:
+    return isinstance(a, np.ndarray) or (hasattr(a, "is_cuda") and not a.is_cuda)
+
+
+def _ptr_array(items: Sequence) -> "C.Array":
+    arr = (C.c_void_p * max(len(items), 1))()
+    for i, it in enumerate(items):
+        arr[i] = _ptr(it)
+    return arr
+
+
+def make_spec(s: dict) -> ks_hw_spec:
+    return ks_hw_spec(float(s["peak_flops"]), float(s["peak_bw"]), int(s["n_sm"]), int(s["ctas_per_sm"]),
+                      int(s["tile_m"]), int(s["tile_n"]), int(s["ew_elems_per_cta"]), float(s["l2_bytes"]),
+                      float(s["t0"]))
+
+
+def make_batch(bucket) -> ks_desc_batch:
+    """bucket: any object with family, cols (numpy arrays or torch tensors), dtype_bytes, hq, hkv, head_dim."""
+    cols = list(bucket.cols)
+    n = int(cols[0].shape[0]) if cols else 0
+    dt = str(cols[0].dtype) if cols else "int32"
+    if "float32" in dt:
+        cd = KS_COL_F32
+    elif "int32" in dt:
+        cd = KS_COL_I32
+    else:
+        raise TypeError(f"descriptor columns must be int32 or float32, got {dt}")
+    arr = (C.c_void_p * KS_MAX_COLS)()
+    for i, c in enumerate(cols):
+        if hasattr(c, "is_contiguous") and not c.is_contiguous():
+            raise ValueError("descriptor columns must be contiguous")
+        arr[i] = _ptr(c)
+    return ks_desc_batch(int(bucket.family), n, cd, int(bucket.dtype_bytes), len(cols), int(bucket.hq),
+                         int(bucket.hkv), int(bucket.head_dim), arr)
+
+
+def make_step_params(p: dict) -> ks_step_params:
+    return ks_step_params(float(p["c_disp"]), float(p["floor_l"]), float(p["c_ovl"]), float(p["c_tail"]),
+                          float(p["body_scale"]))
+
+
+class Context:
+    """Owns one ks_ctx.  Method names mirror the C entry points."""
+
+    def __init__(self, device: int = 0, stream: Optional[int] = None):
+        self._h = C.c_void_p()
+        self._lib = load()
+        _check(self._lib.ks_create(C.byref(self._h), int(device), C.c_void_p(stream or 0)), "ks_create")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.ks_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- loading
+    def load_heads(self, family: int, head) -> None:
+        f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+        W1, b1, W2, b2, w3 = f32(head.W1), f32(head.b1), f32(head.W2), f32(head.b2), f32(head.w3)
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        _check(self._lib.ks_load_heads(self._h, int(family), int(head.n_in), int(head.h1), int(head.h2), fp(W1),
+                                       fp(b1), fp(W2), fp(b2), fp(w3), float(head.b3)), "ks_load_heads")
+
+    def load_grid(self, family: int, grid) -> None:
+        dims = np.ascontiguousarray(grid.dims, dtype=np.int32)
+        lo = np.ascontiguousarray(grid.lo_log2, dtype=np.float32)
+        hi = np.ascontiguousarray(grid.hi_log2, dtype=np.float32)
+        vals = np.ascontiguousarray(grid.values, dtype=np.float32)
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        _check(self._lib.ks_load_grid(self._h, int(family), dims.ctypes.data_as(C.POINTER(C.c_int32)), fp(lo),
+                                      fp(hi), fp(vals)), "ks_load_grid")
+
+    def set_gelu_mode(self, mode: int) -> None:
+        _check(self._lib.ks_set_gelu_mode(self._h, int(mode)), "ks_set_gelu_mode")
+
+    def launch_count(self) -> int:
+        out = C.c_int64()
+        _check(self._lib.ks_get_launch_count(self._h, C.byref(out)), "ks_get_launch_count")
+        return out.value
+
+    # ---- compute
+    def predict_kernels(self, buckets: Sequence, specs: Sequence[dict], tier: int, latency: Sequence,
+                        tiles: Optional[Sequence] = None, waves: Optional[Sequence] = None,
+                        t_roof: Optional[Sequence] = None, space: Optional[int] = None) -> None:
+        nb = len(buckets)
+        batches = (ks_desc_batch * max(nb, 1))(*[make_batch(b) for b in buckets])
+        sp = (ks_hw_spec * max(len(specs), 1))(*[make_spec(s) for s in specs])
+        if space is None:
+            space = KS_MEM_HOST if (nb and _is_host(latency[0])) else KS_MEM_DEVICE
+        opt = lambda x: _ptr_array(x) if x is not None else None
+        _check(self._lib.ks_predict_kernels(self._h, batches, nb, sp, len(specs), int(tier), int(space),
+                                            _ptr_array(latency), opt(tiles), opt(waves), opt(t_roof)),
+               "ks_predict_kernels")
+
+    def compose_steps(self, latency: Sequence, step_off: Sequence, batch_n: Sequence[int], n_steps: int,
+                      n_specs: int, params: dict, cfg_off, n_cfg: int, step_latency, cfg_latency,
+                      space: Optional[int] = None) -> None:
+        nb = len(latency)
+        bn = (C.c_int32 * max(nb, 1))(*[int(x) for x in batch_n])
+        p = make_step_params(params)
+        if space is None:
+            space = KS_MEM_HOST if _is_host(step_latency) else KS_MEM_DEVICE
+        _check(self._lib.ks_compose_steps(self._h, _ptr_array(latency), _ptr_array(step_off), bn, nb, int(n_steps),
+                                          int(n_specs), C.byref(p), _ptr(cfg_off), int(n_cfg), int(space),
+                                          _ptr(step_latency), _ptr(cfg_latency)), "ks_compose_steps")
+
+    def run_steps(self, buckets: Sequence, step_off: Sequence, specs: Sequence[dict], tier: int, n_steps: int,
+                  params: dict, cfg_off, n_cfg: int, step_latency, cfg_latency, latency: Optional[Sequence] = None,
+                  space: Optional[int] = None) -> None:
+        nb = len(buckets)
+        batches = (ks_desc_batch * max(nb, 1))(*[make_batch(b) for b in buckets])
+        sp = (ks_hw_spec * max(len(specs), 1))(*[make_spec(s) for s in specs])
+        p = make_step_params(params)
+        if space is None:
+            space = KS_MEM_HOST if _is_host(step_latency) else KS_MEM_DEVICE
+        _check(self._lib.ks_run_steps(self._h, batches, _ptr_array(step_off), nb, sp, len(specs), int(tier),
+                                      int(n_steps), C.byref(p), _ptr(cfg_off), int(n_cfg), int(space),
+                                      _ptr_array(latency) if latency is not None else None, _ptr(step_latency),
+                                      _ptr(cfg_latency)), "ks_run_steps")

@@ -1,0 +1,666 @@
+// ks_api.cu — the C ABI of libks (include/ks.h): context, head/grid loading (host-side operand
+// image construction), argument validation, host<->device staging, kernel dispatch.
+// No arithmetic of the method runs on the host; there is no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "ks_internal.h"
+
+namespace {
+
+struct HeadState {
+  bool loaded = false;
+  int n_in = 0, h = 0;
+  void* w1_img = nullptr;
+  void* w2_img = nullptr;
+  float* w3 = nullptr;
+  float b3 = 0.0f;
+};
+
+struct GridState {
+  bool loaded = false;
+  KsGridDev dev;
+  float* values = nullptr;
+};
+
+}  // namespace
+
+struct ks_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int num_sms = 0;
+  bool sticky = false;
+  int gelu_mode = 0;
+  int64_t launches = 0;
+  HeadState heads[KS_FAM_COUNT];
+  GridState grids[KS_FAM_COUNT];
+  // grow-only device workspace with a bump pointer (host-space staging, internal latencies)
+  char* ws = nullptr;
+  size_t ws_cap = 0, ws_used = 0;
+};
+
+namespace {
+
+const int kFamCols[KS_FAM_COUNT] = {3, 10, 3, 2};
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+ks_status cuda_fail(ks_ctx* c) {
+  if (c) c->sticky = true;
+  return KS_ECUDA;
+}
+
+#define KS_CUDA(ctx, call)                       \
+  do {                                           \
+    if ((call) != cudaSuccess) return cuda_fail(ctx); \
+  } while (0)
+
+ks_status ws_reserve(ks_ctx* c, size_t bytes) {
+  c->ws_used = 0;
+  if (bytes <= c->ws_cap) return KS_OK;
+  if (c->ws) {
+    KS_CUDA(c, cudaStreamSynchronize(c->stream));
+    KS_CUDA(c, cudaFree(c->ws));
+    c->ws = nullptr;
+    c->ws_cap = 0;
+  }
+  const size_t cap = align_up(bytes + bytes / 8, 1 << 20);
+  if (cudaMalloc(reinterpret_cast<void**>(&c->ws), cap) != cudaSuccess) {
+    cudaGetLastError();
+    c->ws = nullptr;
+    return KS_ENOMEM;
+  }
+  c->ws_cap = cap;
+  return KS_OK;
+}
+
+void* ws_take(ks_ctx* c, size_t bytes) {
+  void* p = c->ws + c->ws_used;
+  c->ws_used += align_up(bytes, 256);
+  return p;
+}
+
+// fp32 -> bf16 bits, round to nearest even (NaN kept quiet)
+uint16_t f32_to_bf16_bits(float f) {
+  uint32_t u;
+  memcpy(&u, &f, 4);
+  if ((u & 0x7f800000u) == 0x7f800000u && (u & 0x007fffffu)) return (uint16_t)((u >> 16) | 0x40u);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+float bf16_bits_to_f32(uint16_t b) {
+  uint32_t u = (uint32_t)b << 16;
+  float f;
+  memcpy(&f, &u, 4);
+  return f;
+}
+
+KsFastDiv make_fastdiv(uint32_t d) {
+  KsFastDiv f;
+  f.d = d;
+  f.pad = 0;
+  if (d <= 1) { f.mul = 0; f.shr = 0; f.d = 1; return f; }
+  uint32_t l = 0;
+  while ((1ull << l) < d) ++l;                       // ceil(log2 d)
+  const uint32_t p = 31 + l;
+  f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
+  f.shr = p - 32;
+  return f;
+}
+
+bool spec_ok(const ks_hw_spec& s) {
+  if (!(s.peak_flops > 0.0f) || !(s.peak_bw > 0.0f) || !isfinite(s.peak_flops) || !isfinite(s.peak_bw)) return false;
+  if (s.n_sm < 1 || s.ctas_per_sm < 1 || s.tile_m < 1 || s.tile_n < 1 || s.ew_elems_per_cta < 1) return false;
+  if ((long long)s.n_sm * s.ctas_per_sm > 0x7fffffffll) return false;
+  if (!(s.l2_bytes >= 0.0f) || !(s.t0 >= 0.0f) || !isfinite(s.t0)) return false;
+  return true;
+}
+
+KsSpecDev make_spec_dev(const ks_hw_spec& s) {
+  KsSpecDev d;
+  const uint32_t slots = (uint32_t)s.n_sm * (uint32_t)s.ctas_per_sm;
+  d.inv_peak_flops = (float)(1.0 / (double)s.peak_flops);
+  d.inv_peak_bw = (float)(1.0 / (double)s.peak_bw);
+  d.t0 = s.t0;
+  d.inv_t0 = s.t0 > 0.0f ? (float)(1.0 / (double)s.t0) : INFINITY;
+  d.l2_bytes = s.l2_bytes;
+  d.lg_ridge = (float)log2((double)s.peak_flops / (double)s.peak_bw);
+  d.inv_slots = (float)(1.0 / (double)slots);
+  d.slots_f = (float)slots;
+  d.tile_m = make_fastdiv((uint32_t)s.tile_m);
+  d.tile_n = make_fastdiv((uint32_t)s.tile_n);
+  d.ew = make_fastdiv((uint32_t)s.ew_elems_per_cta);
+  d.slots = make_fastdiv(slots);
+  return d;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// validation shared by predict / run_steps.  `device_ptrs`: enforce 16-byte alignment.
+ks_status validate_batches(const ks_ctx* c, const ks_desc_batch* batches, int n_batches, const ks_hw_spec* specs,
+                           int n_specs, int tier, bool device_ptrs) {
+  if (!c) return KS_EINVAL;
+  if (n_batches < 0 || n_batches > KS_MAX_BATCHES || n_specs < 0) return KS_EINVAL;
+  if (n_batches > 0 && !batches) return KS_EINVAL;
+  if (n_specs > 0 && !specs) return KS_EINVAL;
+  if (tier != KS_TIER_NONE && tier != KS_TIER_A && tier != KS_TIER_B) return KS_EINVAL;
+  for (int s = 0; s < n_specs; ++s)
+    if (!spec_ok(specs[s])) return KS_EINVAL;
+  for (int b = 0; b < n_batches; ++b) {
+    const ks_desc_batch& k = batches[b];
+    if (k.family < 0 || k.family >= KS_FAM_COUNT || k.n < 0) return KS_EINVAL;
+    if (k.col_dtype != KS_COL_I32 && k.col_dtype != KS_COL_F32) return KS_EINVAL;
+    if (k.dtype_bytes != 1 && k.dtype_bytes != 2 && k.dtype_bytes != 4) return KS_EINVAL;
+    if (k.n_cols != kFamCols[k.family]) return KS_EINVAL;
+    if (k.family == KS_FAM_ATTN && (k.attn_hq < 1 || k.attn_hkv < 1 || k.attn_head_dim < 1)) return KS_EINVAL;
+    if (k.n > 0)
+      for (int col = 0; col < k.n_cols; ++col) {
+        if (!k.cols[col]) return KS_EINVAL;
+        if (device_ptrs && !aligned16(k.cols[col])) return KS_EINVAL;
+      }
+    if (tier == KS_TIER_A && !c->heads[k.family].loaded) return KS_ESTATE;
+    if (tier == KS_TIER_B && !c->grids[k.family].loaded) return KS_ESTATE;
+  }
+  return KS_OK;
+}
+
+struct DevOut {
+  float* lat = nullptr;
+  int32_t* tiles = nullptr;
+  int32_t* waves = nullptr;
+  float* troof = nullptr;
+};
+
+KsBucketDev make_bucket_dev(const ks_desc_batch& k, const void* const* cols, const DevOut& o, long long spec0) {
+  KsBucketDev d;
+  memset(&d, 0, sizeof(d));
+  for (int c = 0; c < k.n_cols; ++c) d.cols[c] = cols[c];
+  const long long off = spec0 * (long long)k.n;
+  d.lat = o.lat ? o.lat + off : nullptr;
+  d.tiles = o.tiles ? o.tiles + off : nullptr;
+  d.waves = o.waves ? o.waves + off : nullptr;
+  d.troof = o.troof ? o.troof + off : nullptr;
+  d.family = k.family;
+  d.n = k.n;
+  d.col_f32 = k.col_dtype == KS_COL_F32 ? 1 : 0;
+  d.s = k.dtype_bytes;
+  d.hq = k.attn_hq;
+  d.hkv = k.attn_hkv;
+  d.hd = k.attn_head_dim;
+  d.n_cols = k.n_cols;
+  return d;
+}
+
+// Enqueue S1-S5 for device-resident columns/outputs.  Arguments are already validated.
+ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* const (*cols)[KS_MAX_COLS], int n_batches,
+                         const ks_hw_spec* specs, int n_specs, int tier, const DevOut* outs) {
+  for (int s0 = 0; s0 < n_specs; s0 += KS_MAX_SPECS_PER_LAUNCH) {
+    const int ns = n_specs - s0 < KS_MAX_SPECS_PER_LAUNCH ? n_specs - s0 : KS_MAX_SPECS_PER_LAUNCH;
+    if (tier != KS_TIER_A) {
+      for (int b = 0; b < n_batches; ++b) {
+        if (batches[b].n == 0) continue;
+        KsStreamParams p;
+        memset(&p, 0, sizeof(p));
+        p.bk = make_bucket_dev(batches[b], cols[b], outs[b], s0);
+        if (tier == KS_TIER_B) p.grid = c->grids[batches[b].family].dev;
+        p.n_specs = ns;
+        p.tier = tier;
+        p.spec_stride = batches[b].n;
+        for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
+        KS_CUDA(c, ks_launch_stream(p, c->num_sms, c->stream));
+        c->launches += 1;
+      }
+    } else {
+      // group buckets by head dimensions; one persistent launch per group of <= 4 buckets
+      bool done[KS_MAX_BATCHES] = {false};
+      for (int b = 0; b < n_batches; ++b) {
+        if (done[b] || batches[b].n == 0) { done[b] = true; continue; }
+        const HeadState& h0 = c->heads[batches[b].family];
+        KsMlpParams p;
+        memset(&p, 0, sizeof(p));
+        int nb = 0, tiles = 0;
+        for (int q = b; q < n_batches && nb < KS_MLP_MAX_BUCKETS; ++q) {
+          if (done[q] || batches[q].n == 0) continue;
+          const HeadState& hq = c->heads[batches[q].family];
+          if (hq.n_in != h0.n_in || hq.h != h0.h) continue;
+          p.bk[nb] = make_bucket_dev(batches[q], cols[q], outs[q], s0);
+          p.head[nb].w1_img = hq.w1_img;
+          p.head[nb].w2_img = hq.w2_img;
+          p.head[nb].w3 = hq.w3;
+          p.head[nb].b3 = hq.b3;
+          p.tile_begin[nb] = tiles;
+          tiles += (batches[q].n + 127) / 128;
+          done[q] = true;
+          ++nb;
+        }
+        p.tile_begin[nb] = tiles;
+        p.n_buckets = nb;
+        p.n_specs = ns;
+        p.gelu_mode = c->gelu_mode;
+        for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
+        KS_CUDA(c, ks_launch_mlp(p, h0.n_in, h0.h, c->num_sms, c->stream));
+        c->launches += 1;
+      }
+    }
+  }
+  return KS_OK;
+}
+
+}  // namespace
+
+// =================================================================== extern "C" entry points
+extern "C" {
+
+const char* ks_status_string(ks_status s) {
+  switch (s) {
+    case KS_OK: return "KS_OK";
+    case KS_EINVAL: return "KS_EINVAL";
+    case KS_ENOMEM: return "KS_ENOMEM";
+    case KS_ECUDA: return "KS_ECUDA";
+    case KS_ESTATE: return "KS_ESTATE";
+    case KS_EUNSUPPORTED: return "KS_EUNSUPPORTED";
+  }
+  return "KS_?";
+}
+
+ks_status ks_create(ks_ctx** out, int device, void* cuda_stream) {
+  if (!out) return KS_EINVAL;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) { cudaGetLastError(); return KS_ECUDA; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return KS_ECUDA; }
+  if (prop.major != 10) return KS_ECUDA;            // kernels are built for sm_100a only; no fallback
+  if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return KS_ECUDA; }
+  ks_ctx* c = new (std::nothrow) ks_ctx();
+  if (!c) return KS_ENOMEM;
+  c->device = device;
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->num_sms = prop.multiProcessorCount;
+  *out = c;
+  return KS_OK;
+}
+
+ks_status ks_destroy(ks_ctx* c) {
+  if (!c) return KS_OK;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  for (int f = 0; f < KS_FAM_COUNT; ++f) {
+    cudaFree(c->heads[f].w1_img);
+    cudaFree(c->heads[f].w2_img);
+    cudaFree(c->heads[f].w3);
+    cudaFree(c->grids[f].values);
+  }
+  cudaFree(c->ws);
+  cudaGetLastError();
+  delete c;
+  return KS_OK;
+}
+
+ks_status ks_get_launch_count(ks_ctx* c, int64_t* out) {
+  if (!c || !out) return KS_EINVAL;
+  *out = c->launches;
+  return KS_OK;
+}
+
+ks_status ks_set_gelu_mode(ks_ctx* c, int mode) {
+  if (!c || (mode != 0 && mode != 1)) return KS_EINVAL;
+  c->gelu_mode = mode;
+  return KS_OK;
+}
+
+ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, const float* W1, const float* b1,
+                        const float* W2, const float* b2, const float* w3, float b3) {
+  if (!c || family < 0 || family >= KS_FAM_COUNT || !W1 || !b1 || !W2 || !b2 || !w3) return KS_EINVAL;
+  if (n_in <= 0 || h1 <= 0 || h2 <= 0) return KS_EINVAL;
+  if (c->sticky) return KS_ECUDA;
+  if ((n_in != 8 && n_in != 12 && n_in != 32) || h1 != h2 || (h1 != 64 && h1 != 128 && h1 != 256)) return KS_EUNSUPPORTED;
+  const int H = h1, K1 = ks_mlp_k1(n_in);
+  const int n_real = n_in == 32 ? 22 : n_in;          // features 22..31 are identically zero (Q2)
+  const int bias_row = n_real;
+  // UMMA operand images, K-major no-swizzle: element (n, k) at ((k/8) * H + n) * 8 + k % 8
+  std::vector<uint16_t> i1((size_t)K1 * H, 0), i2((size_t)(H + 16) * H, 0);
+  auto at = [H](int n, int k) { return ((size_t)(k / 8) * H + n) * 8 + (k % 8); };
+  for (int j = 0; j < H; ++j) {
+    for (int k = 0; k < n_real; ++k) i1[at(j, k)] = f32_to_bf16_bits(W1[(size_t)k * H + j]);
+    const uint16_t hi1 = f32_to_bf16_bits(b1[j]);
+    i1[at(j, bias_row)] = hi1;
+    i1[at(j, bias_row + 1)] = f32_to_bf16_bits(b1[j] - bf16_bits_to_f32(hi1));
+    for (int k = 0; k < H; ++k) i2[at(j, k)] = f32_to_bf16_bits(W2[(size_t)k * H + j]);
+    const uint16_t hi2 = f32_to_bf16_bits(b2[j]);
+    i2[at(j, H)] = hi2;
+    i2[at(j, H + 1)] = f32_to_bf16_bits(b2[j] - bf16_bits_to_f32(hi2));
+  }
+  // layer 3 runs in fp32 on the CUDA cores; its weights are still bf16-rounded like the others
+  std::vector<float> w3r(H);
+  for (int j = 0; j < H; ++j) w3r[j] = bf16_bits_to_f32(f32_to_bf16_bits(w3[j]));
+
+  KS_CUDA(c, cudaSetDevice(c->device));
+  KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read the old head
+  HeadState& hs = c->heads[family];
+  cudaFree(hs.w1_img); cudaFree(hs.w2_img); cudaFree(hs.w3);
+  hs = HeadState();
+  void *d1 = nullptr, *d2 = nullptr, *d3 = nullptr;
+  if (cudaMalloc(&d1, i1.size() * 2) != cudaSuccess || cudaMalloc(&d2, i2.size() * 2) != cudaSuccess ||
+      cudaMalloc(&d3, (size_t)H * 4) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(d1); cudaFree(d2); cudaFree(d3);
+    return KS_ENOMEM;
+  }
+  KS_CUDA(c, cudaMemcpy(d1, i1.data(), i1.size() * 2, cudaMemcpyHostToDevice));
+  KS_CUDA(c, cudaMemcpy(d2, i2.data(), i2.size() * 2, cudaMemcpyHostToDevice));
+  KS_CUDA(c, cudaMemcpy(d3, w3r.data(), (size_t)H * 4, cudaMemcpyHostToDevice));
+  hs.loaded = true;
+  hs.n_in = n_in;
+  hs.h = H;
+  hs.w1_img = d1;
+  hs.w2_img = d2;
+  hs.w3 = static_cast<float*>(d3);
+  hs.b3 = b3;
+  return KS_OK;
+}
+
+ks_status ks_load_grid(ks_ctx* c, ks_family family, const int32_t dims[3], const float lo_log2[3],
+                       const float hi_log2[3], const float* values) {
+  if (!c || family < 0 || family >= KS_FAM_COUNT || !dims || !lo_log2 || !hi_log2 || !values) return KS_EINVAL;
+  long long nodes = 1;
+  for (int a = 0; a < 3; ++a) {
+    if (dims[a] < 1 || dims[a] > KS_MAX_GRID_NODES) return KS_EINVAL;
+    if (dims[a] > 1 && !(hi_log2[a] > lo_log2[a])) return KS_EINVAL;
+    nodes *= dims[a];
+  }
+  if (nodes > KS_MAX_GRID_NODES) return KS_EINVAL;
+  if (c->sticky) return KS_ECUDA;
+  KS_CUDA(c, cudaSetDevice(c->device));
+  KS_CUDA(c, cudaStreamSynchronize(c->stream));
+  GridState& g = c->grids[family];
+  cudaFree(g.values);
+  g = GridState();
+  const size_t padded = ((size_t)nodes + 3) & ~(size_t)3;    // bulk copies move multiples of 16 bytes
+  float* d = nullptr;
+  if (cudaMalloc(reinterpret_cast<void**>(&d), padded * 4) != cudaSuccess) { cudaGetLastError(); return KS_ENOMEM; }
+  KS_CUDA(c, cudaMemset(d, 0, padded * 4));
+  KS_CUDA(c, cudaMemcpy(d, values, (size_t)nodes * 4, cudaMemcpyHostToDevice));
+  memset(&g.dev, 0, sizeof(g.dev));
+  g.dev.values = d;
+  g.dev.n_nodes = (int32_t)nodes;
+  const int32_t strides[3] = {dims[1] * dims[2], dims[2], 1};
+  for (int a = 0; a < 3; ++a) {
+    g.dev.dims[a] = dims[a];
+    g.dev.stride[a] = dims[a] > 1 ? strides[a] : 0;
+    g.dev.lo[a] = lo_log2[a];
+    g.dev.scale[a] = dims[a] > 1 ? (float)((double)(dims[a] - 1) / ((double)hi_log2[a] - (double)lo_log2[a])) : 0.0f;
+  }
+  g.values = d;
+  g.loaded = true;
+  return KS_OK;
+}
+
+}  // extern "C"
+
+// =================================================================== compute entry points
+namespace {
+
+bool params_ok(const ks_step_params* p) {
+  return p && isfinite(p->c_disp) && isfinite(p->floor_l) && isfinite(p->c_ovl) && isfinite(p->c_tail) &&
+         isfinite(p->body_scale);
+}
+
+bool csr_ok(const int32_t* off, int n, long long limit) {       // host-resident CSR only
+  if (off[0] < 0) return false;
+  for (int i = 0; i < n; ++i)
+    if (off[i + 1] < off[i]) return false;
+  return limit < 0 || off[n] <= limit;
+}
+
+ks_status compose_device(ks_ctx* c, const float* const* lat, const int32_t* const* step_off, const int32_t* batch_n,
+                         int n_batches, int n_steps, int n_specs, const ks_step_params* params,
+                         const int32_t* cfg_off, int n_cfg, float* step_lat, float* cfg_lat) {
+  if (n_steps == 0 || n_specs == 0) {
+    if (n_cfg > 0 && n_specs > 0) KS_CUDA(c, cudaMemsetAsync(cfg_lat, 0, (size_t)n_cfg * n_specs * 4, c->stream));
+    return KS_OK;
+  }
+  KsComposeParams p;
+  memset(&p, 0, sizeof(p));
+  for (int b = 0; b < n_batches; ++b) {
+    p.lat[b] = lat[b];
+    p.step_off[b] = step_off[b];
+    p.spec_stride[b] = batch_n[b];
+  }
+  p.n_batches = n_batches;
+  p.n_steps = n_steps;
+  p.n_specs = n_specs;
+  p.n_cfg = n_cfg;
+  p.sp = *params;
+  p.cfg_off = cfg_off;
+  p.step_lat = step_lat;
+  p.cfg_lat = cfg_lat;
+  int launches = 0;
+  KS_CUDA(c, ks_launch_compose(p, c->num_sms, c->stream, &launches));
+  c->launches += launches;
+  return KS_OK;
+}
+
+ks_status validate_compose(const ks_ctx* c, const float* const* lat, const int32_t* const* step_off,
+                           const int32_t* batch_n, int n_batches, int n_steps, int n_specs,
+                           const ks_step_params* params, const int32_t* cfg_off, int n_cfg, ks_mem_space space,
+                           const float* step_lat, const float* cfg_lat, bool lat_optional) {
+  if (!c) return KS_EINVAL;
+  if (space != KS_MEM_DEVICE && space != KS_MEM_HOST) return KS_EINVAL;
+  if (n_batches < 0 || n_batches > KS_MAX_BATCHES || n_steps < 0 || n_specs < 0 || n_cfg < 0) return KS_EINVAL;
+  if (!params_ok(params)) return KS_EINVAL;
+  if (n_batches > 0 && (!step_off || !batch_n || (!lat && !lat_optional))) return KS_EINVAL;
+  for (int b = 0; b < n_batches; ++b) {
+    if (batch_n[b] < 0 || !step_off[b]) return KS_EINVAL;
+    if (!lat_optional && !lat[b] && batch_n[b] > 0) return KS_EINVAL;
+    if (space == KS_MEM_HOST && !csr_ok(step_off[b], n_steps, batch_n[b])) return KS_EINVAL;
+  }
+  if (n_cfg > 0 && (!cfg_off || !cfg_lat)) return KS_EINVAL;
+  if (n_cfg > 0 && space == KS_MEM_HOST && !csr_ok(cfg_off, n_cfg, n_steps)) return KS_EINVAL;
+  if ((long long)n_steps * n_specs > 0 && !step_lat) return KS_EINVAL;
+  return KS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+ks_status ks_predict_kernels(ks_ctx* c, const ks_desc_batch* batches, int n_batches, const ks_hw_spec* specs,
+                             int n_specs, ks_tier tier, ks_mem_space space, float* const* latency,
+                             int32_t* const* tiles, int32_t* const* waves, float* const* t_roof) {
+  if (space != KS_MEM_DEVICE && space != KS_MEM_HOST) return KS_EINVAL;
+  const bool dev = space == KS_MEM_DEVICE;
+  ks_status st = validate_batches(c, batches, n_batches, specs, n_specs, tier, dev);
+  if (st != KS_OK) return st;
+  if (n_batches > 0 && !latency) return KS_EINVAL;
+  for (int b = 0; b < n_batches; ++b) {
+    if (batches[b].n == 0 || n_specs == 0) continue;
+    if (!latency[b]) return KS_EINVAL;
+    if (dev && (!aligned16(latency[b]) || (tiles && tiles[b] && !aligned16(tiles[b])) ||
+                (waves && waves[b] && !aligned16(waves[b])) || (t_roof && t_roof[b] && !aligned16(t_roof[b]))))
+      return KS_EINVAL;
+  }
+  if (c->sticky) return KS_ECUDA;
+  if (n_batches == 0 || n_specs == 0) return KS_OK;
+  KS_CUDA(c, cudaSetDevice(c->device));
+
+  const void* cols[KS_MAX_BATCHES][KS_MAX_COLS] = {};
+  DevOut outs[KS_MAX_BATCHES];
+  if (dev) {
+    for (int b = 0; b < n_batches; ++b) {
+      for (int k = 0; k < batches[b].n_cols; ++k) cols[b][k] = batches[b].cols[k];
+      outs[b].lat = latency[b];
+      outs[b].tiles = tiles ? tiles[b] : nullptr;
+      outs[b].waves = waves ? waves[b] : nullptr;
+      outs[b].troof = t_roof ? t_roof[b] : nullptr;
+    }
+    return predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+  }
+  // host space: stage through the workspace
+  size_t need = 0;
+  for (int b = 0; b < n_batches; ++b) {
+    const size_t n = batches[b].n, o = align_up(n * (size_t)n_specs * 4, 256);
+    need += batches[b].n_cols * align_up(n * 4, 256) + o;
+    if (tiles && tiles[b]) need += o;
+    if (waves && waves[b]) need += o;
+    if (t_roof && t_roof[b]) need += o;
+  }
+  st = ws_reserve(c, need);
+  if (st != KS_OK) return st;
+  for (int b = 0; b < n_batches; ++b) {
+    const size_t n = batches[b].n, ob = n * (size_t)n_specs * 4;
+    for (int k = 0; k < batches[b].n_cols; ++k) {
+      void* d = ws_take(c, n * 4);
+      if (n) KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+      cols[b][k] = d;
+    }
+    outs[b].lat = static_cast<float*>(ws_take(c, ob));
+    if (tiles && tiles[b]) outs[b].tiles = static_cast<int32_t*>(ws_take(c, ob));
+    if (waves && waves[b]) outs[b].waves = static_cast<int32_t*>(ws_take(c, ob));
+    if (t_roof && t_roof[b]) outs[b].troof = static_cast<float*>(ws_take(c, ob));
+  }
+  st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+  if (st != KS_OK) return st;
+  for (int b = 0; b < n_batches; ++b) {
+    const size_t ob = (size_t)batches[b].n * n_specs * 4;
+    if (!ob) continue;
+    KS_CUDA(c, cudaMemcpyAsync(latency[b], outs[b].lat, ob, cudaMemcpyDeviceToHost, c->stream));
+    if (outs[b].tiles) KS_CUDA(c, cudaMemcpyAsync(tiles[b], outs[b].tiles, ob, cudaMemcpyDeviceToHost, c->stream));
+    if (outs[b].waves) KS_CUDA(c, cudaMemcpyAsync(waves[b], outs[b].waves, ob, cudaMemcpyDeviceToHost, c->stream));
+    if (outs[b].troof) KS_CUDA(c, cudaMemcpyAsync(t_roof[b], outs[b].troof, ob, cudaMemcpyDeviceToHost, c->stream));
+  }
+  KS_CUDA(c, cudaStreamSynchronize(c->stream));
+  return KS_OK;
+}
+
+ks_status ks_compose_steps(ks_ctx* c, const float* const* latency, const int32_t* const* step_off,
+                           const int32_t* batch_n, int n_batches, int n_steps, int n_specs,
+                           const ks_step_params* params, const int32_t* cfg_off, int n_cfg, ks_mem_space space,
+                           float* step_latency, float* cfg_latency) {
+  ks_status st = validate_compose(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg,
+                                  space, step_latency, cfg_latency, false);
+  if (st != KS_OK) return st;
+  if (c->sticky) return KS_ECUDA;
+  KS_CUDA(c, cudaSetDevice(c->device));
+  if (space == KS_MEM_DEVICE)
+    return compose_device(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg,
+                          step_latency, cfg_latency);
+  size_t need = align_up((size_t)(n_cfg + 1) * 4, 256) + align_up((size_t)n_steps * n_specs * 4, 256) +
+                align_up((size_t)n_cfg * n_specs * 4 + 4, 256);
+  for (int b = 0; b < n_batches; ++b)
+    need += align_up((size_t)batch_n[b] * n_specs * 4, 256) + align_up((size_t)(n_steps + 1) * 4, 256);
+  st = ws_reserve(c, need);
+  if (st != KS_OK) return st;
+  const float* dlat[KS_MAX_BATCHES];
+  const int32_t* doff[KS_MAX_BATCHES];
+  for (int b = 0; b < n_batches; ++b) {
+    const size_t lb = (size_t)batch_n[b] * n_specs * 4, ob = (size_t)(n_steps + 1) * 4;
+    float* dl = static_cast<float*>(ws_take(c, lb));
+    int32_t* dofs = static_cast<int32_t*>(ws_take(c, ob));
+    if (lb) KS_CUDA(c, cudaMemcpyAsync(dl, latency[b], lb, cudaMemcpyHostToDevice, c->stream));
+    KS_CUDA(c, cudaMemcpyAsync(dofs, step_off[b], ob, cudaMemcpyHostToDevice, c->stream));
+    dlat[b] = dl;
+    doff[b] = dofs;
+  }
+  int32_t* dcfg = static_cast<int32_t*>(ws_take(c, (size_t)(n_cfg + 1) * 4));
+  float* dstep = static_cast<float*>(ws_take(c, (size_t)n_steps * n_specs * 4));
+  float* dtot = static_cast<float*>(ws_take(c, (size_t)n_cfg * n_specs * 4 + 4));
+  if (n_cfg > 0) KS_CUDA(c, cudaMemcpyAsync(dcfg, cfg_off, (size_t)(n_cfg + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+  st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot);
+  if (st != KS_OK) return st;
+  if ((size_t)n_steps * n_specs)
+    KS_CUDA(c, cudaMemcpyAsync(step_latency, dstep, (size_t)n_steps * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
+  if ((size_t)n_cfg * n_specs)
+    KS_CUDA(c, cudaMemcpyAsync(cfg_latency, dtot, (size_t)n_cfg * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
+  KS_CUDA(c, cudaStreamSynchronize(c->stream));
+  return KS_OK;
+}
+
+ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* const* step_off, int n_batches,
+                       const ks_hw_spec* specs, int n_specs, ks_tier tier, int n_steps, const ks_step_params* params,
+                       const int32_t* cfg_off, int n_cfg, ks_mem_space space, float* const* latency,
+                       float* step_latency, float* cfg_latency) {
+  if (space != KS_MEM_DEVICE && space != KS_MEM_HOST) return KS_EINVAL;
+  const bool dev = space == KS_MEM_DEVICE;
+  ks_status st = validate_batches(c, batches, n_batches, specs, n_specs, tier, dev);
+  if (st != KS_OK) return st;
+  int32_t batch_n[KS_MAX_BATCHES] = {0};
+  for (int b = 0; b < n_batches; ++b) batch_n[b] = batches[b].n;
+  st = validate_compose(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg, space,
+                        step_latency, cfg_latency, true);
+  if (st != KS_OK) return st;
+  if (dev && latency)
+    for (int b = 0; b < n_batches; ++b)
+      if (latency[b] && !aligned16(latency[b])) return KS_EINVAL;
+  if (c->sticky) return KS_ECUDA;
+  KS_CUDA(c, cudaSetDevice(c->device));
+
+  size_t need = 0;
+  for (int b = 0; b < n_batches; ++b) {
+    const size_t n = batches[b].n;
+    const bool user_lat = dev && latency && latency[b];
+    if (!user_lat) need += align_up(n * (size_t)n_specs * 4, 256);
+    if (!dev) need += batches[b].n_cols * align_up(n * 4, 256) + align_up((size_t)(n_steps + 1) * 4, 256);
+  }
+  if (!dev)
+    need += align_up((size_t)(n_cfg + 1) * 4, 256) + align_up((size_t)n_steps * n_specs * 4, 256) +
+            align_up((size_t)n_cfg * n_specs * 4 + 4, 256);
+  st = ws_reserve(c, need);
+  if (st != KS_OK) return st;
+
+  const void* cols[KS_MAX_BATCHES][KS_MAX_COLS] = {};
+  DevOut outs[KS_MAX_BATCHES];
+  const float* dlat[KS_MAX_BATCHES];
+  const int32_t* doff[KS_MAX_BATCHES];
+  for (int b = 0; b < n_batches; ++b) {
+    const size_t n = batches[b].n;
+    for (int k = 0; k < batches[b].n_cols; ++k) {
+      if (dev) { cols[b][k] = batches[b].cols[k]; continue; }
+      void* d = ws_take(c, n * 4);
+      if (n) KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+      cols[b][k] = d;
+    }
+    outs[b].lat = (dev && latency && latency[b]) ? latency[b] : static_cast<float*>(ws_take(c, n * (size_t)n_specs * 4));
+    dlat[b] = outs[b].lat;
+    if (dev) { doff[b] = step_off[b]; continue; }
+    int32_t* dofs = static_cast<int32_t*>(ws_take(c, (size_t)(n_steps + 1) * 4));
+    KS_CUDA(c, cudaMemcpyAsync(dofs, step_off[b], (size_t)(n_steps + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    doff[b] = dofs;
+  }
+  const int32_t* dcfg = cfg_off;
+  float *dstep = step_latency, *dtot = cfg_latency;
+  if (!dev) {
+    int32_t* t = static_cast<int32_t*>(ws_take(c, (size_t)(n_cfg + 1) * 4));
+    if (n_cfg > 0) KS_CUDA(c, cudaMemcpyAsync(t, cfg_off, (size_t)(n_cfg + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    dcfg = t;
+    dstep = static_cast<float*>(ws_take(c, (size_t)n_steps * n_specs * 4));
+    dtot = static_cast<float*>(ws_take(c, (size_t)n_cfg * n_specs * 4 + 4));
+  }
+  if (n_specs > 0 && n_batches > 0) {
+    st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+    if (st != KS_OK) return st;
+  }
+  st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot);
+  if (st != KS_OK) return st;
+  if (!dev) {
+    for (int b = 0; b < n_batches; ++b) {
+      const size_t ob = (size_t)batches[b].n * n_specs * 4;
+      if (latency && latency[b] && ob)
+        KS_CUDA(c, cudaMemcpyAsync(latency[b], outs[b].lat, ob, cudaMemcpyDeviceToHost, c->stream));
+    }
+    if ((size_t)n_steps * n_specs)
+      KS_CUDA(c, cudaMemcpyAsync(step_latency, dstep, (size_t)n_steps * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
+    if ((size_t)n_cfg * n_specs)
+      KS_CUDA(c, cudaMemcpyAsync(cfg_latency, dtot, (size_t)n_cfg * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
+    KS_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return KS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,54 @@
+// ks_internal.h — launcher interfaces between the C-ABI layer (ks_api.cu) and the kernels.
+#pragma once
+#include "ks_common.cuh"
+
+struct KsSpecTable {
+  KsSpecDev s[KS_MAX_SPECS_PER_LAUNCH];
+};
+
+// ---- streaming kernels (Tier NONE / Tier B): ks_stream.cu
+struct KsStreamParams {
+  KsBucketDev bk;
+  KsGridDev grid;          // Tier B only
+  int32_t n_specs;
+  int32_t tier;
+  int64_t spec_stride;     // elements between consecutive specs in the outputs (= bucket n)
+  KsSpecTable specs;
+};
+cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st);
+
+// ---- Tier-A MLP head kernel: ks_mlp.cu
+#define KS_MLP_MAX_BUCKETS 4
+struct KsHeadDev {
+  const void* w1_img;      // bf16 UMMA image [K1/8][H][8]  (rows n_in, n_in+1 hold b1 hi/lo)
+  const void* w2_img;      // bf16 UMMA image [(H+16)/8][H][8] (K rows H, H+1 hold b2 hi/lo)
+  const float* w3;         // fp32 [H]
+  float b3;
+  int32_t pad;
+};
+struct KsMlpParams {
+  KsBucketDev bk[KS_MLP_MAX_BUCKETS];
+  KsHeadDev head[KS_MLP_MAX_BUCKETS];
+  int32_t tile_begin[KS_MLP_MAX_BUCKETS + 1];   // prefix of 128-row tiles per bucket
+  int32_t n_buckets, n_specs, gelu_mode, pad;
+  KsSpecTable specs;
+};
+// n_in in {8,12,32}; h in {64,128,256}; all buckets of one launch share (n_in, h)
+cudaError_t ks_launch_mlp(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st);
+// sizes of the device weight images for a head
+size_t ks_mlp_w1_img_bytes(int n_in, int h);
+size_t ks_mlp_w2_img_bytes(int h);
+int ks_mlp_k1(int n_in);   // padded K of layer 1 (16 or 32)
+
+// ---- step composition: ks_compose.cu
+struct KsComposeParams {
+  const float* lat[KS_MAX_BATCHES];
+  const int32_t* step_off[KS_MAX_BATCHES];
+  int64_t spec_stride[KS_MAX_BATCHES];
+  int32_t n_batches, n_steps, n_specs, n_cfg;
+  ks_step_params sp;
+  const int32_t* cfg_off;
+  float* step_lat;   // [n_specs][n_steps]
+  float* cfg_lat;    // [n_specs][n_cfg]
+};
+cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_t st, int* launches);

@@ -1,0 +1,214 @@
+// ks_stream.cu — the HBM-bound streaming kernels: descriptor decode + roofline + wave quantization
+// (+ Tier-B trilinear interpolation from a shared-memory-resident grid) + launch floor.
+// S1, S2, S4b, S5 of DESIGN.md §1.  PAPER.md:191 Eq. 2, :88 Fig. 2, :211 Tier B.
+//
+// Layout: SoA int32/fp32 columns; each thread owns 4 consecutive rows and moves them with 16-byte
+// vector loads/stores (streaming cache hints: every byte is touched once).  Per-spec constants sit
+// in the kernel-parameter constant bank.  Tier B stages the whole grid (<= 128 KiB) into shared
+// memory once per persistent CTA with a 1-D TMA bulk copy.
+#include "ks_internal.h"
+#include "ks_ptx.cuh"
+
+namespace {
+
+template <int FAM> struct NCols { static constexpr int v = 3; };
+template <> struct NCols<KS_FAM_GROUPED_GEMM> { static constexpr int v = 10; };
+template <> struct NCols<KS_FAM_ELEMWISE> { static constexpr int v = 2; };
+
+template <int NC, bool F32>
+KS_DEV void load_rows4(const KsBucketDev& bk, int row0, int n, int (&v)[4][NC]) {
+  if (row0 + 4 <= n) {
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+      if (F32) {
+        const float4 f = __ldcs(reinterpret_cast<const float4*>(static_cast<const float*>(bk.cols[c]) + row0));
+        v[0][c] = __float2int_rn(f.x); v[1][c] = __float2int_rn(f.y);
+        v[2][c] = __float2int_rn(f.z); v[3][c] = __float2int_rn(f.w);
+      } else {
+        const int4 q = __ldcs(reinterpret_cast<const int4*>(static_cast<const int*>(bk.cols[c]) + row0));
+        v[0][c] = q.x; v[1][c] = q.y; v[2][c] = q.z; v[3][c] = q.w;
+      }
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int c = 0; c < NC; ++c) v[j][c] = (row0 + j < n) ? ks_load_col(bk.cols[c], row0 + j, F32) : 0;
+  }
+}
+
+template <typename T>
+KS_DEV void store4(T* base, long long off, int row0, int n, bool vec, T a, T b, T c, T d) {
+  T* ptr = base + off + row0;
+  if (vec && row0 + 4 <= n) {
+    if (sizeof(T) == 4) {
+      float4 q;
+      q.x = *reinterpret_cast<float*>(&a); q.y = *reinterpret_cast<float*>(&b);
+      q.z = *reinterpret_cast<float*>(&c); q.w = *reinterpret_cast<float*>(&d);
+      __stcs(reinterpret_cast<float4*>(ptr), q);
+    }
+  } else {
+    if (row0 + 0 < n) ptr[0] = a;
+    if (row0 + 1 < n) ptr[1] = b;
+    if (row0 + 2 < n) ptr[2] = c;
+    if (row0 + 3 < n) ptr[3] = d;
+  }
+}
+
+// Tier-B axis values (Q5): GEMM (M,N,K); GROUPED (sum m,N,K); ATTN (B,q,max(kv,q));
+// ELEMWISE (n, 2^subop, 1) -> log2 coordinates.
+template <int FAM>
+KS_DEV void grid_log2_axes(const int* v, float (&lg)[3], bool (&pos)[3]) {
+  float a[3];
+  if (FAM == KS_FAM_GEMM) {
+    a[0] = (float)v[0]; a[1] = (float)v[1]; a[2] = (float)v[2];
+  } else if (FAM == KS_FAM_GROUPED_GEMM) {
+    float sum = 0.0f;
+#pragma unroll
+    for (int e = 0; e < KS_N_EXPERTS; ++e) sum += (float)ks_nonneg(v[2 + e]);
+    a[0] = sum; a[1] = (float)v[0]; a[2] = (float)v[1];
+  } else if (FAM == KS_FAM_ATTN) {
+    a[0] = (float)v[0]; a[1] = (float)v[1]; a[2] = (float)(v[2] < v[1] ? v[1] : v[2]);
+  } else {
+    a[0] = (float)v[0]; a[1] = 1.0f; a[2] = 1.0f;
+  }
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { pos[k] = a[k] > 0.0f; lg[k] = pos[k] ? ks_log2_pos(a[k]) : 0.0f; }
+  if (FAM == KS_FAM_ELEMWISE) lg[1] = (float)ks_ew_op(v[1]);
+}
+
+// trilinear interpolation of the stored efficiency; grid values in shared memory
+template <int FAM>
+KS_DEV float trilinear(const int* v, const KsGridDev& g, const float* __restrict__ sg) {
+  float lg[3];
+  bool pos[3];
+  grid_log2_axes<FAM>(v, lg, pos);
+  int base = 0;
+  float f[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const float top = (float)(g.dims[a] - 1);
+    float c = pos[a] ? (lg[a] - g.lo[a]) * g.scale[a] : 0.0f;
+    c = fminf(fmaxf(c, 0.0f), top);                 // clamp to the measured span (fmaxf drops NaN)
+    int i = (int)c;
+    const int imax = g.dims[a] >= 2 ? g.dims[a] - 2 : 0;
+    i = i > imax ? imax : i;
+    f[a] = c - (float)i;
+    base += i * g.stride[a];
+  }
+  const int s0 = g.stride[0], s1 = g.stride[1], s2 = g.stride[2];
+  const float v000 = sg[base], v001 = sg[base + s2];
+  const float v010 = sg[base + s1], v011 = sg[base + s1 + s2];
+  const float v100 = sg[base + s0], v101 = sg[base + s0 + s2];
+  const float v110 = sg[base + s0 + s1], v111 = sg[base + s0 + s1 + s2];
+  const float c00 = fmaf(f[2], v001 - v000, v000), c01 = fmaf(f[2], v011 - v010, v010);
+  const float c10 = fmaf(f[2], v101 - v100, v100), c11 = fmaf(f[2], v111 - v110, v110);
+  const float c0 = fmaf(f[1], c01 - c00, c00), c1 = fmaf(f[1], c11 - c10, c10);
+  return fmaf(f[0], c1 - c0, c0);
+}
+
+template <int FAM, int TIER, bool F32>
+__global__ void __launch_bounds__(TIER == KS_TIER_B ? (FAM == KS_FAM_GROUPED_GEMM ? 512 : 1024) : 256)
+ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
+  constexpr int NC = NCols<FAM>::v;
+  extern __shared__ __align__(128) float sgrid[];
+  __shared__ __align__(8) uint64_t grid_bar;
+
+  if (TIER == KS_TIER_B) {
+    // stage the grid once per CTA: 1-D TMA bulk copies signalled on an mbarrier
+    const uint32_t bytes = (uint32_t)(((p.grid.n_nodes + 3) & ~3) * 4);
+    if (threadIdx.x == 0) {
+      ks_mbar_init(&grid_bar, 1);
+      ks_fence_mbar_init();
+      ks_mbar_expect_tx(&grid_bar, bytes);
+      for (uint32_t off = 0; off < bytes; off += 32768u) {
+        const uint32_t len = bytes - off < 32768u ? bytes - off : 32768u;
+        ks_bulk_g2s(reinterpret_cast<char*>(sgrid) + off, reinterpret_cast<const char*>(p.grid.values) + off, len,
+                    &grid_bar);
+      }
+    }
+    __syncthreads();
+    ks_mbar_wait(&grid_bar, 0);
+  }
+
+  const int n = p.bk.n;
+  const int n4 = (n + 3) >> 2;
+  const int stride = gridDim.x * blockDim.x;
+  for (int g = blockIdx.x * blockDim.x + threadIdx.x; g < n4; g += stride) {
+    const int row0 = g << 2;
+    int v[4][NC];
+    load_rows4<NC, F32>(p.bk, row0, n, v);
+
+    float e[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) e[j] = 1.0f;
+    if (TIER == KS_TIER_B) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) e[j] = fmaxf(trilinear<FAM>(v[j], p.grid, sgrid), 0.0009765625f);
+    }
+
+    for (int s = 0; s < p.n_specs; ++s) {
+      const KsSpecDev& sp = p.specs.s[s];
+      const long long off = (long long)s * p.spec_stride;
+      const bool vec = ((off & 3ll) == 0);
+      float t[4], tr[4];
+      int tiles[4], waves[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const KsWork w = ks_decode<FAM>(v[j], p.bk, sp);
+        const KsRoof r = ks_roofline(w, sp);
+        tiles[j] = (int)w.B;
+        waves[j] = (int)r.W;
+        tr[j] = r.t_roof;
+        // Eq. 2: t = max(t_roof * eta, t0), eta = 1/e; the floor is applied after eta
+        t[j] = fmaxf(TIER == KS_TIER_NONE ? r.t_roof : __fdiv_rn(r.t_roof, e[j]), sp.t0);
+      }
+      store4<float>(p.bk.lat, off, row0, n, vec, t[0], t[1], t[2], t[3]);
+      if (p.bk.tiles) store4<int>(p.bk.tiles, off, row0, n, vec, tiles[0], tiles[1], tiles[2], tiles[3]);
+      if (p.bk.waves) store4<int>(p.bk.waves, off, row0, n, vec, waves[0], waves[1], waves[2], waves[3]);
+      if (p.bk.troof) store4<float>(p.bk.troof, off, row0, n, vec, tr[0], tr[1], tr[2], tr[3]);
+    }
+  }
+}
+
+template <int FAM, int TIER>
+cudaError_t launch_ft(const KsStreamParams& p, int num_sms, cudaStream_t st) {
+  const int n4 = (p.bk.n + 3) >> 2;
+  if (n4 == 0) return cudaSuccess;
+  const bool f32 = p.bk.col_f32 != 0;
+  if (TIER == KS_TIER_B) {
+    const int threads = FAM == KS_FAM_GROUPED_GEMM ? 512 : 1024;   // 10 columns x 4 rows need > 64 registers
+    const size_t smem = (size_t)((p.grid.n_nodes + 3) & ~3) * 4;
+    int blocks = (n4 + threads - 1) / threads;
+    if (blocks > num_sms) blocks = num_sms;          // persistent: one CTA per SM, grid staged once
+    auto kern = f32 ? ks_stream_kernel<FAM, TIER, true> : ks_stream_kernel<FAM, TIER, false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<blocks, threads, smem, st>>>(p);
+  } else {
+    const int threads = 256;
+    int blocks = (n4 + threads - 1) / threads;
+    const int cap = num_sms * 8 * 4;                 // up to 4 waves of 8 resident CTAs per SM
+    if (blocks > cap) blocks = cap - (cap % num_sms);
+    auto kern = f32 ? ks_stream_kernel<FAM, TIER, true> : ks_stream_kernel<FAM, TIER, false>;
+    kern<<<blocks, threads, 0, st>>>(p);
+  }
+  return cudaGetLastError();
+}
+
+template <int TIER>
+cudaError_t launch_t(const KsStreamParams& p, int num_sms, cudaStream_t st) {
+  switch (p.bk.family) {
+    case KS_FAM_GEMM: return launch_ft<KS_FAM_GEMM, TIER>(p, num_sms, st);
+    case KS_FAM_GROUPED_GEMM: return launch_ft<KS_FAM_GROUPED_GEMM, TIER>(p, num_sms, st);
+    case KS_FAM_ATTN: return launch_ft<KS_FAM_ATTN, TIER>(p, num_sms, st);
+    case KS_FAM_ELEMWISE: return launch_ft<KS_FAM_ELEMWISE, TIER>(p, num_sms, st);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace
+
+cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st) {
+  return p.tier == KS_TIER_B ? launch_t<KS_TIER_B>(p, num_sms, st) : launch_t<KS_TIER_NONE>(p, num_sms, st);
+}

@@ -1,0 +1,286 @@
+"""-m gpu: parity of the CUDA path (through the C ABI) against the CPU oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json's: bit-exact integers (tiles, waves,
+counts), <= 1e-5 relative for the fp32 roofline / interpolation / sum paths, <= 1e-2 relative on
+latency for the bf16 tensor-core MLP path.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2606_28565_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_F32 = 1e-5
+TOL_MLP = 1e-2
+
+
+@pytest.fixture(scope="module")
+def ks():
+    import torch
+    from paper_2606_28565_b200 import binding as B
+    from paper_2606_28565_b200 import build as ksbuild
+    from paper_2606_28565_b200 import driver as D
+    ksbuild.build()
+    assert torch.cuda.is_available()
+    return B, D
+
+
+def rel_err(got, want):
+    want = np.asarray(want, np.float64)
+    return np.abs(np.asarray(got, np.float64) - want) / np.maximum(np.abs(want), 1e-300)
+
+
+def oracle_all(w, tier=None, rows=None):
+    tier = w.tier if tier is None else tier
+    heads = {f: O.Head(h) for f, h in w.heads.items()} if tier == W.TIER_A else {}
+    grids = {f: O.Grid(g) for f, g in w.grids.items()} if tier == W.TIER_B else {}
+    out = []
+    for i, b in enumerate(w.buckets):
+        r = None if rows is None else rows[i]
+        out.append(O.predict_bucket(b, w.specs, tier, head=heads.get(b.family), grid=grids.get(b.family), rows=r))
+    return out
+
+
+def check_bucket(g, o, tol, rows=None, what=""):
+    sel = (lambda a: a) if rows is None else (lambda a: a[:, rows])
+    assert np.array_equal(sel(g["tiles"]), o["tiles"]), f"{what}: tiles not bit-exact"
+    assert np.array_equal(sel(g["waves"]), o["waves"]), f"{what}: waves not bit-exact"
+    e_tr = rel_err(sel(g["troof"]), o["troof"])
+    e_tr[o["troof"] == 0] = np.abs(sel(g["troof"]))[o["troof"] == 0]
+    assert e_tr.max(initial=0) <= TOL_F32, f"{what}: t_roof rel err {e_tr.max()}"
+    e = rel_err(sel(g["lat"]), o["lat"])
+    assert e.max(initial=0) <= tol, f"{what}: latency rel err {e.max()}"
+    return float(e.max(initial=0))
+
+
+def run_and_check(ks, w, tol, tier=None, gelu_mode=0):
+    B, D = ks
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        ctx.set_gelu_mode(gelu_mode)
+        g = D.predict(ctx, w, tier=tier)
+    finally:
+        ctx.close()
+    o = oracle_all(w, tier)
+    return [check_bucket(gi, oi, tol, what=f"{w.name}/bucket{i}") for i, (gi, oi) in enumerate(zip(g, o))]
+
+
+# ------------------------------------------------------------------ Tier NONE (S1, S2, S5)
+@pytest.mark.parametrize("make", [lambda: W.config1(), lambda: W.config2(n=30011),
+                                  lambda: W.config4(n_steps=60), lambda: W.config5(n_rows=20003, n_specs=3)])
+def test_tier_none_parity(ks, make):
+    w = make()
+    run_and_check(ks, w, TOL_F32, tier=W.TIER_NONE)
+
+
+def test_degenerate_rows_and_clamps(ks):
+    spec = [W.spec_gb200(tile_m=96, tile_n=160, ctas_per_sm=2, ew_elems_per_cta=1000)]
+    i32 = lambda *a: [np.asarray(x, np.int32) for x in a]
+    buckets = [
+        W.Bucket(W.FAM_GEMM, i32([0, 5, 1, 2 ** 20, 7], [8, 0, 1, 4096, 9], [8, 8, 0, 64, 3])),
+        W.Bucket(W.FAM_GROUPED, i32([256] * 3, [64] * 3, *[[0, 1, 5000]] * 1, *[[0, 0, 17]] * 7)),
+        W.Bucket(W.FAM_ATTN, i32([1, 3, 0, 2], [1, 700, 5, 64], [1, 100, 9, 64]), hq=32, hkv=8, head_dim=128),  # kv<q raised
+        W.Bucket(W.FAM_ELEMWISE, i32([0, 1, 999, 1000, 1001, 5], [0, 1, 2, 3, 9, -4])),                       # subop clamped
+    ]
+    w = W.Workload("edge", buckets, spec, W.TIER_NONE)
+    run_and_check(ks, w, TOL_F32)
+
+
+@pytest.mark.parametrize("n", [1, 3, 4, 127, 128, 129, 1027])
+def test_ragged_tails_and_misaligned_spec_stride(ks, n):
+    w = W.config2(n=10 * n)      # buckets of 5n, 3n, 2n rows; n_specs = 3 makes spec rows start unaligned
+    w.specs = [W.spec_gb200(), W.spec_gb200(n_sm=80, peak_bw=2e12), W.spec_gb200(tile_m=64, t0=1e-9)]
+    run_and_check(ks, w, TOL_F32, tier=W.TIER_NONE)
+    run_and_check(ks, w, TOL_MLP, tier=W.TIER_A)
+
+
+# ------------------------------------------------------------------ Tier B (S4b)
+def test_tier_b_parity(ks):
+    errs = run_and_check(ks, W.config3(n=60001), TOL_F32)
+    print("tier B max rel err", errs)
+
+
+def test_tier_b_nodes_exact_and_flat_axes(ks):
+    B, D = ks
+    rng = np.random.default_rng(11)
+    # queries exactly on grid nodes (integer log2 coordinates) must return the node value
+    vals = rng.uniform(0.2, 0.95, (8, 8, 8)).astype(np.float32)
+    grid = W.Grid(np.array([8, 8, 8], np.int32), np.zeros(3, np.float32), np.full(3, 7, np.float32), vals)
+    idx = rng.integers(0, 8, (500, 3))
+    cols = [np.left_shift(1, idx[:, a]).astype(np.int32) for a in range(3)]
+    spec = W.spec_gb200(t0=0.0)
+    w = W.Workload("nodes", [W.Bucket(W.FAM_GEMM, cols)], [spec], W.TIER_B, grids={W.FAM_GEMM: grid})
+    ctx = B.Context(0)
+    D.load_models(ctx, w)
+    g = D.predict(ctx, w)[0]
+    e = g["troof"][0].astype(np.float64) / g["lat"][0].astype(np.float64)
+    assert np.allclose(e, vals[idx[:, 0], idx[:, 1], idx[:, 2]], rtol=3e-7)
+    # elementwise family: sub-op axis nodes + one flat axis
+    ev = rng.uniform(0.2, 0.95, (32, 6, 1)).astype(np.float32)
+    ge = W.Grid(np.array([32, 6, 1], np.int32), np.array([12, 0, 0], np.float32), np.array([25, 5, 0], np.float32), ev)
+    ne, sub = W._elem_rows(rng, 5000)
+    w2 = W.Workload("ew", [W.Bucket(W.FAM_ELEMWISE, W._i32(ne, sub))], [W.spec_gb200()], W.TIER_B,
+                    grids={W.FAM_ELEMWISE: ge})
+    D.load_models(ctx, w2)
+    g2 = D.predict(ctx, w2)
+    ctx.close()
+    check_bucket(g2[0], oracle_all(w2)[0], TOL_F32, what="elementwise grid")
+
+
+# ------------------------------------------------------------------ Tier A (S3, S4a)
+@pytest.mark.parametrize("make", [lambda: W.config1(), lambda: W.config2(n=40013),
+                                  lambda: W.config5(n_rows=12001, n_specs=3, n_layers=4),
+                                  lambda: W.config4(n_steps=40, tier=W.TIER_A, n_layers=4)])
+def test_tier_a_parity(ks, make):
+    w = make()
+    errs = run_and_check(ks, w, TOL_MLP)
+    print(w.name, "tier A max rel err per bucket", errs)
+    assert max(errs) < TOL_MLP
+
+
+@pytest.mark.parametrize("n_in,h", [(8, 64), (8, 128), (12, 64), (12, 256), (32, 64), (32, 128), (8, 256)])
+def test_tier_a_all_head_shapes_with_wide_weights(ks, n_in, h):
+    # wider weights (std 0.25) push pre-activations to |x| ~ 2-3 where the tanh-form GELU differs most
+    w = W.config2(n=6007, n_in=n_in, h=h)
+    rng = np.random.Generator(np.random.PCG64(100 + n_in + h))
+    w.heads = {f: W.make_head(rng, n_in, h, bias_std=0.2, w_std=0.25 if h < 256 else 0.15) for f in w.heads}
+    errs = run_and_check(ks, w, TOL_MLP)
+    print(n_in, h, "wide-weight max rel err", errs)
+
+
+def test_tier_a_packed_gelu_mode_within_tolerance(ks):
+    w = W.config2(n=40013)
+    errs = run_and_check(ks, w, TOL_MLP, gelu_mode=1)
+    print("gelu_mode=1 max rel err", errs)
+
+
+def test_zero_weight_head_is_exact_closed_form(ks):
+    B, D = ks
+    w = W.config1()
+    w.heads = {W.FAM_GEMM: W.make_head(np.random.default_rng(0), 8, 64, bias_std=0.0, w_std=0.0)}
+    ctx = B.Context(0)
+    D.load_models(ctx, w)
+    g = D.predict(ctx, w)[0]
+    ctx.close()
+    want = np.maximum(2.0 * g["troof"][0], np.float32(2e-6))     # e = 0.5 exactly -> eta = 2
+    assert np.array_equal(g["lat"][0], want.astype(np.float32))
+
+
+# ------------------------------------------------------------------ S6 / S7
+@pytest.mark.parametrize("params", [W.STEP_PARAMS_CFG4, W.STEP_PARAMS_HOSTBOUND,
+                                    dict(c_disp=1e-6, floor_l=0.0, c_ovl=0.0, c_tail=1e-5, body_scale=1.25)])
+def test_compose_parity(ks, params):
+    B, D = ks
+    w = W.config4(n_steps=700, n_cfg=9, step_params=params)
+    ctx = B.Context(0)
+    db = D.to_device(w)
+    g = D.predict(ctx, w, dbuckets=db)
+    step, tot = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+    ctx.close()
+    o = oracle_all(w)
+    # same per-kernel inputs on both sides: feed the oracle's composer the GPU's fp32 latencies
+    so, to = O.compose([x["lat"][0] for x in g], [b.step_off for b in w.buckets], w.n_steps, params, w.cfg_off)
+    assert rel_err(step[0], so).max() <= TOL_F32
+    assert rel_err(tot[0], to).max() <= TOL_F32
+    # and end to end against the pure-oracle pipeline
+    so2, to2 = O.compose([x["lat"][0] for x in o], [b.step_off for b in w.buckets], w.n_steps, params, w.cfg_off)
+    assert rel_err(step[0], so2).max() <= TOL_F32 and rel_err(tot[0], to2).max() <= TOL_F32
+
+
+def test_compose_ones_empty_segments_and_multi_spec(ks):
+    import torch
+    B, D = ks
+    rng = np.random.default_rng(3)
+    n_steps, ns = 257, 3
+    ns_rows = [1000, 37]
+    offs = [np.concatenate([[0], np.sort(rng.integers(0, n + 1, n_steps - 1)), [n]]).astype(np.int32) for n in ns_rows]
+    lat = [rng.uniform(1e-6, 1e-3, (ns, n)).astype(np.float32) for n in ns_rows]
+    cfg = np.array([0, 0, 100, 257], np.int32)                        # first config empty
+    ctx = B.Context(0)
+    dl = [torch.from_numpy(x).cuda() for x in lat]
+    do = [torch.from_numpy(x).cuda() for x in offs]
+    step = torch.empty((ns, n_steps), dtype=torch.float32, device="cuda")
+    tot = torch.empty((ns, 3), dtype=torch.float32, device="cuda")
+    ctx.compose_steps(dl, do, ns_rows, n_steps, ns, W.STEP_PARAMS_HOSTBOUND, torch.from_numpy(cfg).cuda(), 3, step, tot)
+    torch.cuda.synchronize()
+    for s in range(ns):
+        so, to = O.compose([x[s] for x in lat], offs, n_steps, W.STEP_PARAMS_HOSTBOUND, cfg)
+        assert rel_err(step[s].cpu().numpy(), so).max() <= TOL_F32
+        assert np.allclose(tot[s].cpu().numpy(), to, rtol=TOL_F32, atol=0)
+    ones = [torch.ones((1, n), dtype=torch.float32, device="cuda") for n in ns_rows]
+    step1 = torch.empty((1, n_steps), dtype=torch.float32, device="cuda")
+    tot1 = torch.empty((1, 3), dtype=torch.float32, device="cuda")
+    ctx.compose_steps(ones, do, ns_rows, n_steps, 1, W.STEP_PARAMS_ZERO, torch.from_numpy(cfg).cuda(), 3, step1, tot1)
+    torch.cuda.synchronize()
+    ctx.close()
+    assert np.array_equal(step1[0].cpu().numpy(), (np.diff(offs[0]) + np.diff(offs[1])).astype(np.float32))
+    assert np.array_equal(tot1[0].cpu().numpy(), np.array([0, offs[0][100] + offs[1][100],
+                                                           1037 - offs[0][100] - offs[1][100]], np.float32))
+
+
+# ------------------------------------------------------------------ ABI behaviour on the device
+def test_host_space_equals_device_space_and_run_steps(ks):
+    import torch
+    B, D = ks
+    w = W.config2(n=20011)
+    ctx = B.Context(0)
+    D.load_models(ctx, w)
+    db = D.to_device(w)
+    g = D.predict(ctx, w, dbuckets=db)
+    step_d, tot_d = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+    n_cfg = w.cfg_off.shape[0] - 1
+    # host space through ks_predict_kernels
+    lat_h = [np.empty((1, b.n), np.float32) for b in w.buckets]
+    tiles_h = [np.empty((1, b.n), np.int32) for b in w.buckets]
+    ctx.predict_kernels(w.buckets, w.specs, w.tier, lat_h, tiles=tiles_h)
+    for i in range(len(w.buckets)):
+        assert np.array_equal(lat_h[i], g[i]["lat"]) and np.array_equal(tiles_h[i], g[i]["tiles"])
+    # host space through the fused ks_run_steps
+    step_h, tot_h = np.empty((1, w.n_steps), np.float32), np.empty((1, n_cfg), np.float32)
+    lat_h2 = [np.empty((1, b.n), np.float32) for b in w.buckets]
+    ctx.run_steps(w.buckets, [b.step_off for b in w.buckets], w.specs, w.tier, w.n_steps, w.step_params,
+                  w.cfg_off, n_cfg, step_h, tot_h, latency=lat_h2)
+    assert np.array_equal(step_h, step_d) and np.array_equal(tot_h, tot_d)
+    assert all(np.array_equal(a, b["lat"]) for a, b in zip(lat_h2, g))
+    # device space run_steps without returning per-kernel latencies; determinism (bit-identical rerun)
+    cfg = torch.from_numpy(w.cfg_off).cuda()
+    s1 = torch.empty((1, w.n_steps), dtype=torch.float32, device="cuda")
+    t1 = torch.empty((1, n_cfg), dtype=torch.float32, device="cuda")
+    for _ in range(2):
+        ctx.run_steps(db, [b.step_off for b in db], w.specs, w.tier, w.n_steps, w.step_params, cfg, n_cfg, s1, t1)
+        torch.cuda.synchronize()
+        assert np.array_equal(s1.cpu().numpy(), step_d) and np.array_equal(t1.cpu().numpy(), tot_d)
+    assert ctx.launch_count() > 0
+    ctx.close()
+
+
+def test_status_codes_on_device(ks):
+    import torch
+    B, D = ks
+    w = W.config2(n=1000)
+    ctx = B.Context(0)
+    db = D.to_device(w)
+    lat = [torch.empty((1, b.n), dtype=torch.float32, device="cuda") for b in db]
+    with pytest.raises(B.KsError) as e:
+        ctx.predict_kernels(db, w.specs, W.TIER_A, lat)              # heads not loaded
+    assert e.value.status == B.KS_ESTATE
+    with pytest.raises(B.KsError) as e:
+        ctx.predict_kernels(db, w.specs, W.TIER_B, lat)              # grids not loaded
+    assert e.value.status == B.KS_ESTATE
+    bad = W.make_head(np.random.default_rng(0), 12, 96)
+    with pytest.raises(B.KsError) as e:
+        ctx.load_heads(W.FAM_GEMM, bad)
+    assert e.value.status == B.KS_EUNSUPPORTED
+    sentinel = torch.full((1, db[0].n + 1), -1.0, dtype=torch.float32, device="cuda")
+    with pytest.raises(B.KsError) as e:                              # misaligned device output
+        ctx.predict_kernels(db[:1], w.specs, W.TIER_NONE, [sentinel[0, 1:]])
+    assert e.value.status == B.KS_EINVAL and bool((sentinel == -1.0).all())   # nothing was written
+    badspec = [W.spec_gb200(n_sm=0)]
+    with pytest.raises(B.KsError) as e:
+        ctx.predict_kernels(db, badspec, W.TIER_NONE, lat)
+    assert e.value.status == B.KS_EINVAL
+    empty = W.Workload("empty", [W.Bucket(W.FAM_GEMM, W._i32([], [], []))], w.specs, W.TIER_NONE)
+    ctx.predict_kernels(D.to_device(empty), w.specs, W.TIER_NONE, [torch.empty((1, 0), device="cuda")])   # n = 0 no-op
+    ctx.close()
