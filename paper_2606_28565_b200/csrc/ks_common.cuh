@@ -127,7 +127,7 @@ KS_DEV KsRoof ks_roofline(const KsWork& w, const KsSpecDev& sp) {
   KsRoof r;
   if (w.B == 0u) { r.W = 0u; r.u = 1.0f; r.t_comp = 0.0f; r.t_mem = 0.0f; r.t_roof = 0.0f; return r; }
   r.W = ks_ceil_div(w.B, sp.slots);
-  r.u = __fdiv_rn((float)r.W * sp.slots_f, (float)w.B);
+  r.u = __fdividef((float)r.W * sp.slots_f, (float)w.B);
   r.t_comp = w.F * sp.inv_peak_flops;
   r.t_mem = w.Y * sp.inv_peak_bw;
   r.t_roof = fmaxf(r.t_comp * r.u, r.t_mem);

@@ -1,15 +1,17 @@
 // ks_compose.cu — S6/S7: segmented reduction of kernel latencies into per-step GPU bodies
 // (PAPER.md:231), the host-overlap step formula (Eq. 4) and per-configuration totals.
 //
-// One warp per (spec, step): for every family bucket the warp streams its CSR segment with
-// coalesced loads (4 independent accumulators per lane), then a fixed-order shuffle tree combines
-// the lanes — no atomics, so results are bit-reproducible.  Config totals: one CTA per
+// One warp per (spec, step): one parallel load fetches every bucket's CSR bounds, then the first
+// 128 elements of every bucket are loaded before the first add (one memory round trip per step),
+// longer segments stream the rest; a fixed-order shuffle tree combines the lanes — no atomics, so results are bit-reproducible.  Config totals: one CTA per
 // (spec, config), fp64 accumulation, fixed-order block reduction.
 #include "ks_internal.h"
 
 namespace {
 
 constexpr int kWarpsPerBlock = 8;
+
+constexpr int kRounds = 4;   // predicated first-round loads per bucket issued before any add
 
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
@@ -20,23 +22,50 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
   const int spec = (int)(warp / p.n_steps);
   const int step = (int)(warp - (long long)spec * p.n_steps);
 
-  float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+  // all CSR offsets of this step in ONE parallel load: lane 2b -> begin, lane 2b+1 -> end of bucket b
+  int off = 0;
+  if (lane < 2 * p.n_batches) off = __ldg(p.step_off[lane >> 1] + step + (lane & 1));
+
+  // first kRounds x 32 elements of every bucket: issue every load before the first add so one
+  // memory round trip covers the whole step for typical segment lengths (<= 128 per bucket)
+  float x[KS_MAX_BATCHES][kRounds];
   int count = 0;
-  for (int b = 0; b < p.n_batches; ++b) {
-    const int beg = __ldg(p.step_off[b] + step);
-    const int end = __ldg(p.step_off[b] + step + 1);
-    count += end - beg;
+#pragma unroll
+  for (int b = 0; b < KS_MAX_BATCHES; ++b) {
+    const int beg = __shfl_sync(0xffffffffu, off, 2 * b);
+    const int end = __shfl_sync(0xffffffffu, off, 2 * b + 1);
+    const bool on = b < p.n_batches;
+    count += on ? end - beg : 0;
     const float* __restrict__ lat = p.lat[b] + (long long)spec * p.spec_stride[b];
-    int k = beg + lane;
-    for (; k + 96 < end; k += 128) {
-      a0 += __ldcs(lat + k);
-      a1 += __ldcs(lat + k + 32);
-      a2 += __ldcs(lat + k + 64);
-      a3 += __ldcs(lat + k + 96);
+#pragma unroll
+    for (int r = 0; r < kRounds; ++r) {
+      const int k = beg + lane + 32 * r;
+      x[b][r] = (on && k < end) ? __ldcs(lat + k) : 0.0f;
     }
-    for (; k < end; k += 32) a0 += __ldcs(lat + k);
   }
-  float acc = (a0 + a1) + (a2 + a3);
+  float a[kRounds];
+#pragma unroll
+  for (int r = 0; r < kRounds; ++r) a[r] = 0.0f;
+#pragma unroll
+  for (int b = 0; b < KS_MAX_BATCHES; ++b)
+#pragma unroll
+    for (int r = 0; r < kRounds; ++r) a[r] += x[b][r];
+  // long segments: stream the remainder
+  for (int b = 0; b < p.n_batches; ++b) {
+    const int beg = __shfl_sync(0xffffffffu, off, 2 * b);
+    const int end = __shfl_sync(0xffffffffu, off, 2 * b + 1);
+    if (end - beg <= 32 * kRounds) continue;
+    const float* __restrict__ lat = p.lat[b] + (long long)spec * p.spec_stride[b];
+    int k = beg + lane + 32 * kRounds;
+    for (; k + 96 < end; k += 128) {
+      a[0] += __ldcs(lat + k);
+      a[1] += __ldcs(lat + k + 32);
+      a[2] += __ldcs(lat + k + 64);
+      a[3] += __ldcs(lat + k + 96);
+    }
+    for (; k < end; k += 32) a[0] += __ldcs(lat + k);
+  }
+  float acc = (a[0] + a[1]) + (a[2] + a[3]);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if (lane == 0) {

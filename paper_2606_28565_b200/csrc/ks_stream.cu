@@ -107,7 +107,7 @@ KS_DEV float trilinear(const int* v, const KsGridDev& g, const float* __restrict
   return fmaf(f[0], c1 - c0, c0);
 }
 
-template <int FAM, int TIER, bool F32>
+template <int FAM, int TIER, bool F32, bool ONE>
 __global__ void __launch_bounds__(TIER == KS_TIER_B ? (FAM == KS_FAM_GROUPED_GEMM ? 512 : 1024) : 256)
 ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
   constexpr int NC = NCols<FAM>::v;
@@ -147,8 +147,10 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
       for (int j = 0; j < 4; ++j) e[j] = fmaxf(trilinear<FAM>(v[j], p.grid, sgrid), 0.0009765625f);
     }
 
-    for (int s = 0; s < p.n_specs; ++s) {
-      const KsSpecDev& sp = p.specs.s[s];
+    // ONE: a single spec -> its constants are read straight from the constant bank (no index math)
+    const int n_specs = ONE ? 1 : p.n_specs;
+    for (int s = 0; s < n_specs; ++s) {
+      const KsSpecDev& sp = p.specs.s[ONE ? 0 : s];
       const long long off = (long long)s * p.spec_stride;
       const bool vec = ((off & 3ll) == 0);
       float t[4], tr[4];
@@ -161,7 +163,7 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
         waves[j] = (int)r.W;
         tr[j] = r.t_roof;
         // Eq. 2: t = max(t_roof * eta, t0), eta = 1/e; the floor is applied after eta
-        t[j] = fmaxf(TIER == KS_TIER_NONE ? r.t_roof : __fdiv_rn(r.t_roof, e[j]), sp.t0);
+        t[j] = fmaxf(TIER == KS_TIER_NONE ? r.t_roof : __fdividef(r.t_roof, e[j]), sp.t0);
       }
       store4<float>(p.bk.lat, off, row0, n, vec, t[0], t[1], t[2], t[3]);
       if (p.bk.tiles) store4<int>(p.bk.tiles, off, row0, n, vec, tiles[0], tiles[1], tiles[2], tiles[3]);
@@ -181,7 +183,9 @@ cudaError_t launch_ft(const KsStreamParams& p, int num_sms, cudaStream_t st) {
     const size_t smem = (size_t)((p.grid.n_nodes + 3) & ~3) * 4;
     int blocks = (n4 + threads - 1) / threads;
     if (blocks > num_sms) blocks = num_sms;          // persistent: one CTA per SM, grid staged once
-    auto kern = f32 ? ks_stream_kernel<FAM, TIER, true> : ks_stream_kernel<FAM, TIER, false>;
+    const bool one = p.n_specs == 1;
+    auto kern = f32 ? (one ? ks_stream_kernel<FAM, TIER, true, true> : ks_stream_kernel<FAM, TIER, true, false>)
+                    : (one ? ks_stream_kernel<FAM, TIER, false, true> : ks_stream_kernel<FAM, TIER, false, false>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<blocks, threads, smem, st>>>(p);
@@ -190,7 +194,9 @@ cudaError_t launch_ft(const KsStreamParams& p, int num_sms, cudaStream_t st) {
     int blocks = (n4 + threads - 1) / threads;
     const int cap = num_sms * 8 * 4;                 // up to 4 waves of 8 resident CTAs per SM
     if (blocks > cap) blocks = cap - (cap % num_sms);
-    auto kern = f32 ? ks_stream_kernel<FAM, TIER, true> : ks_stream_kernel<FAM, TIER, false>;
+    const bool one = p.n_specs == 1;
+    auto kern = f32 ? (one ? ks_stream_kernel<FAM, TIER, true, true> : ks_stream_kernel<FAM, TIER, true, false>)
+                    : (one ? ks_stream_kernel<FAM, TIER, false, true> : ks_stream_kernel<FAM, TIER, false, false>);
     kern<<<blocks, threads, 0, st>>>(p);
   }
   return cudaGetLastError();
