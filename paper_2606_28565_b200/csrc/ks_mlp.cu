@@ -36,9 +36,17 @@ template <int NIN, int H>
 struct Cfg {
   static constexpr int K1 = NIN == 32 ? 32 : 16;
   static constexpr int BIAS_ROW = NIN == 32 ? 22 : NIN;   // features >= 22 are identically zero (Q2)
-  static constexpr int NSLOTS = H == 256 ? 1 : 2;
-  static constexpr int THREADS = NSLOTS * 256;
-  static constexpr int TMEM_COLS = NSLOTS * 2 * H;
+  // A slot = one 128-row tile in flight.  H <= 128: one warpgroup per slot (a thread owns a whole
+  // row), D2 reuses D1's TMEM columns, four slots per CTA hide each other's MMA / barrier waits.
+  // H == 256: the W2 image alone is 136 KiB, so only one A2 buffer fits: one slot, two warpgroups
+  // splitting the columns, D1 and D2 separate so MMA2 starts under layer 1's activation work.
+  static constexpr int G = H == 256 ? 2 : 1;              // warpgroups per slot
+  static constexpr bool ALIAS = H != 256;                 // D2 aliases D1
+  static constexpr int NSLOTS = H == 256 ? 1 : 4;
+  static constexpr int SLOT_THREADS = G * 128;
+  static constexpr int THREADS = NSLOTS * SLOT_THREADS;
+  static constexpr int TMEM_PER_SLOT = ALIAS ? H : 2 * H;
+  static constexpr int TMEM_COLS = NSLOTS * TMEM_PER_SLOT;   // 256 (H = 64) or 512
   static constexpr int W1_BYTES = K1 * H * 2;
   static constexpr int W2_BYTES = (H + 16) * H * 2;
   static constexpr int A2_BYTES = (H / 8) * kChunkBytes;
@@ -51,8 +59,8 @@ struct Cfg {
   static constexpr int OFF_ZP = OFF_W3 + H * 4;
   static constexpr int OFF_BAR = OFF_ZP + NSLOTS * kRows * 4;
   static constexpr int SMEM_BYTES = OFF_BAR + 128;
-  static constexpr int HALF = H / 2;          // columns per warpgroup
-  static constexpr int NCHUNK = HALF / 32;    // 32-column chunks per warpgroup
+  static constexpr int WGCOLS = H / G;        // columns per warpgroup
+  static constexpr int NCHUNK = WGCOLS / 32;  // 32-column chunks per warpgroup
 };
 
 // tanh-form GELU, fp32: 0.5 x (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3)))
@@ -79,8 +87,8 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
   using C = Cfg<NIN, H>;
   constexpr int NC = NCols<FAM>::v;
   const int tid = threadIdx.x;
-  const int slot = tid >> 8;
-  const int st = tid & 255;
+  const int slot = tid / C::SLOT_THREADS;
+  const int st = tid - slot * C::SLOT_THREADS;
   const int wg = st >> 7;
   const int r = st & 127;
   const KsBucketDev& bk = p.bk[b];
@@ -96,8 +104,8 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
   const uint32_t w1_addr = ks_smem_u32(smem + C::OFF_W1);
   const uint32_t w2_addr = ks_smem_u32(smem + C::OFF_W2);
   const uint32_t ones_addr = ks_smem_u32(smem + C::OFF_ONES);
-  const uint32_t d1 = tmem_base + (uint32_t)(slot * 2 * H);
-  const uint32_t d2 = d1 + (uint32_t)H;
+  const uint32_t d1 = tmem_base + (uint32_t)(slot * C::TMEM_PER_SLOT);
+  const uint32_t d2 = C::ALIAS ? d1 : d1 + (uint32_t)H;
   const uint32_t lane_off = (uint32_t)((r >> 5) * 32) << 16;     // this warp's TMEM lane quarter
   constexpr uint32_t idesc = ks_umma_idesc_bf16(128, H);
   constexpr uint32_t B_LBO = H * 16;                              // K-chunk stride of a weight image
@@ -105,14 +113,29 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
   const float b3 = p.head[b].b3;
   const int gelu_mode = p.gelu_mode;
   const int tile0 = p.tile_begin[b];
+  const bool f32cols = bk.col_f32 != 0;
+
+  // descriptor columns of the first tile; every later tile is prefetched one iteration ahead
+  int vn[NC];
+  {
+    const int row = (t_lo + slot - tile0) * kRows + r;
+    const bool ok = wg == 0 && t_lo + slot < t_hi && row < bk.n;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) vn[c] = ok ? ks_load_col(bk.cols[c], row, f32cols) : 0;
+  }
 
   for (int t = t_lo + slot; t < t_hi; t += C::NSLOTS) {
     const int row = (t - tile0) * kRows + r;
     const bool valid = row < bk.n;
     int v[NC];
-    if (wg == 0) {
 #pragma unroll
-      for (int c = 0; c < NC; ++c) v[c] = valid ? ks_load_col(bk.cols[c], row, bk.col_f32 != 0) : 0;
+    for (int c = 0; c < NC; ++c) v[c] = vn[c];
+    {
+      const int tn = t + C::NSLOTS;
+      const int rown = (tn - tile0) * kRows + r;
+      const bool ok = wg == 0 && tn < t_hi && rown < bk.n;
+#pragma unroll
+      for (int c = 0; c < NC; ++c) vn[c] = ok ? ks_load_col(bk.cols[c], rown, f32cols) : 0;
     }
     for (int s = 0; s < p.n_specs; ++s) {
       const KsSpecDev& sp = p.specs.s[s];
@@ -146,7 +169,7 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
         ks_fence_proxy_async();
       }
       ks_tc_fence_before();
-      ks_bar_sync(bar_id, 256);
+      ks_bar_sync(bar_id, C::SLOT_THREADS);
       // ---- MMA1: D1 = A1 . W1   (one thread issues for the slot)
       if (st == 0) {
         ks_tc_fence_after();
@@ -162,10 +185,10 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
       ph1 ^= 1u;
       ks_tc_fence_after();
 
-      // ---- epi1: GELU(D1) -> A2, chunk by chunk; MMA2 K ranges are issued as they complete
+      // ---- epi1: GELU(D1) -> A2, chunk by chunk
 #pragma unroll 1
       for (int c = 0; c < C::NCHUNK; ++c) {
-        const int col0 = wg * C::HALF + c * 32;
+        const int col0 = wg * C::WGCOLS + c * 32;
         uint32_t acc[32];
         ks_tmem_ld32(d1 + lane_off + (uint32_t)col0, acc);
         ks_tmem_ld_wait();
@@ -185,27 +208,50 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
           q.x = pk[4 * j + 0]; q.y = pk[4 * j + 1]; q.z = pk[4 * j + 2]; q.w = pk[4 * j + 3];
           *reinterpret_cast<uint4*>(A2 + (col0 / 8 + j) * kChunkBytes + r * 16) = q;
         }
+        if (!C::ALIAS) {
+          // D2 is separate: issue the K range of MMA2 that both warpgroups just finished, so
+          // layer 2 runs on the tensor core under the rest of layer 1's activation work
+          ks_fence_proxy_async();
+          ks_tc_fence_before();
+          ks_bar_sync(bar_id, C::SLOT_THREADS);
+          if (st == 0) {
+            ks_tc_fence_after();
+#pragma unroll
+            for (int g = 0; g < C::G; ++g) {
+#pragma unroll
+              for (int kk = 0; kk < 2; ++kk) {
+                const int k16 = (g * C::WGCOLS + c * 32) / 16 + kk;
+                const uint64_t ad = ks_umma_desc(a2_addr + k16 * 2 * kChunkBytes, kChunkBytes, 128);
+                const uint64_t bd = ks_umma_desc(w2_addr + k16 * 2 * B_LBO, B_LBO, 128);
+                ks_umma_bf16(d2, ad, bd, idesc, (c > 0 || g > 0 || kk > 0) ? 1u : 0u);
+              }
+            }
+            if (c == C::NCHUNK - 1) {            // bias step: ones-block x {b2_hi, b2_lo, 0...}
+              const uint64_t ad = ks_umma_desc(ones_addr, kChunkBytes, 128);
+              const uint64_t bd = ks_umma_desc(w2_addr + (H / 8) * B_LBO, B_LBO, 128);
+              ks_umma_bf16(d2, ad, bd, idesc, 1u);
+              ks_umma_commit(mbar2);
+            }
+          }
+        }
+      }
+      if (C::ALIAS) {
+        // D2 overwrites D1: every warp of the slot has drained its D1 reads (tcgen05.wait::ld above)
         ks_fence_proxy_async();
         ks_tc_fence_before();
-        ks_bar_sync(bar_id, 256);
+        ks_bar_sync(bar_id, C::SLOT_THREADS);
         if (st == 0) {
           ks_tc_fence_after();
 #pragma unroll
-          for (int g = 0; g < 2; ++g) {          // the K range each warpgroup just finished
-#pragma unroll
-            for (int kk = 0; kk < 2; ++kk) {
-              const int k16 = (g * C::HALF + c * 32) / 16 + kk;
-              const uint64_t ad = ks_umma_desc(a2_addr + k16 * 2 * kChunkBytes, kChunkBytes, 128);
-              const uint64_t bd = ks_umma_desc(w2_addr + k16 * 2 * B_LBO, B_LBO, 128);
-              ks_umma_bf16(d2, ad, bd, idesc, (c > 0 || g > 0 || kk > 0) ? 1u : 0u);
-            }
+          for (int k16 = 0; k16 < H / 16; ++k16) {
+            const uint64_t ad = ks_umma_desc(a2_addr + k16 * 2 * kChunkBytes, kChunkBytes, 128);
+            const uint64_t bd = ks_umma_desc(w2_addr + k16 * 2 * B_LBO, B_LBO, 128);
+            ks_umma_bf16(d2, ad, bd, idesc, k16 > 0 ? 1u : 0u);
           }
-          if (c == C::NCHUNK - 1) {              // bias step: ones-block x {b2_hi, b2_lo, 0...}
-            const uint64_t ad = ks_umma_desc(ones_addr, kChunkBytes, 128);
-            const uint64_t bd = ks_umma_desc(w2_addr + (H / 8) * B_LBO, B_LBO, 128);
-            ks_umma_bf16(d2, ad, bd, idesc, 1u);
-            ks_umma_commit(mbar2);
-          }
+          const uint64_t ad = ks_umma_desc(ones_addr, kChunkBytes, 128);
+          const uint64_t bd = ks_umma_desc(w2_addr + (H / 8) * B_LBO, B_LBO, 128);
+          ks_umma_bf16(d2, ad, bd, idesc, 1u);
+          ks_umma_commit(mbar2);
         }
       }
       ks_mbar_wait(mbar2, ph2);
@@ -216,7 +262,7 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
       float zp = 0.0f;
 #pragma unroll 1
       for (int c = 0; c < C::NCHUNK; ++c) {
-        const int col0 = wg * C::HALF + c * 32;
+        const int col0 = wg * C::WGCOLS + c * 32;
         uint32_t acc[32];
         ks_tmem_ld32(d2 + lane_off + (uint32_t)col0, acc);
         ks_tmem_ld_wait();
@@ -242,11 +288,14 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
           }
         }
       }
-      if (wg == 1) zpart[r] = zp;
-      ks_tc_fence_before();
-      ks_bar_sync(bar_id, 256);
+      if (C::G == 2) {
+        if (wg == 1) zpart[r] = zp;
+        ks_tc_fence_before();
+        ks_bar_sync(bar_id, C::SLOT_THREADS);
+        if (wg == 0) zp += zpart[r];
+      }
       if (wg == 0 && valid) {
-        const float z = zp + zpart[r] + b3;
+        const float z = zp + b3;
         // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
         const float eta = fminf(1.0f + __expf(-z), 1024.0f);
         bk.lat[(long long)s * bk.n + row] = fmaxf(t_roof * eta, sp.t0);
@@ -271,10 +320,9 @@ ks_mlp_kernel(const __grid_constant__ KsMlpParams p) {
     ks_fence_mbar_init();
   }
   if (tid < 32) { ks_tmem_alloc(tmem_slot, C::TMEM_COLS); ks_tmem_relinquish(); }
-  if (tid < 256) {   // constant ones-block: K chunk 0 = {1, 1, 0, ...} per row, K chunk 1 = 0
-    uint4 q = make_uint4(0u, 0u, 0u, 0u);
-    if (tid < 128) q.x = 0x3F803F80u;
-    *reinterpret_cast<uint4*>(smem + C::OFF_ONES + tid * 16) = q;
+  if (tid < 128) {   // constant ones-block: K chunk 0 = {1, 1, 0, ...} per row, K chunk 1 = 0
+    *reinterpret_cast<uint4*>(smem + C::OFF_ONES + tid * 16) = make_uint4(0x3F803F80u, 0u, 0u, 0u);
+    *reinterpret_cast<uint4*>(smem + C::OFF_ONES + kChunkBytes + tid * 16) = make_uint4(0u, 0u, 0u, 0u);
   }
   ks_fence_proxy_async();
   ks_tc_fence_before();
