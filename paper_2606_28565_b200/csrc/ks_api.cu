@@ -332,14 +332,16 @@ ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, c
     const uint16_t hi1 = f32_to_bf16_bits(b1[j]);
     i1[at(j, bias_row)] = hi1;
     i1[at(j, bias_row + 1)] = f32_to_bf16_bits(b1[j] - bf16_bits_to_f32(hi1));
-    for (int k = 0; k < H; ++k) i2[at(j, k)] = f32_to_bf16_bits(W2[(size_t)k * H + j]);
+    // the kernels produce 2 GELU(.) as hidden activation; the factor 1/2 lives in the next layer's
+    // weights (a power-of-two scaling of a bf16 value is exact)
+    for (int k = 0; k < H; ++k) i2[at(j, k)] = f32_to_bf16_bits(0.5f * bf16_bits_to_f32(f32_to_bf16_bits(W2[(size_t)k * H + j])));
     const uint16_t hi2 = f32_to_bf16_bits(b2[j]);
     i2[at(j, H)] = hi2;
     i2[at(j, H + 1)] = f32_to_bf16_bits(b2[j] - bf16_bits_to_f32(hi2));
   }
   // layer 3 runs in fp32 on the CUDA cores; its weights are still bf16-rounded like the others
   std::vector<float> w3r(H);
-  for (int j = 0; j < H; ++j) w3r[j] = bf16_bits_to_f32(f32_to_bf16_bits(w3[j]));
+  for (int j = 0; j < H; ++j) w3r[j] = 0.5f * bf16_bits_to_f32(f32_to_bf16_bits(w3[j]));
 
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read the old head

@@ -35,6 +35,7 @@ struct KsMlpParams {
 };
 // n_in in {8,12,32}; h in {64,128,256}; all buckets of one launch share (n_in, h)
 cudaError_t ks_launch_mlp(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st);
+cudaError_t ks_launch_mlp_ws(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st);   // h <= 128
 // sizes of the device weight images for a head
 size_t ks_mlp_w1_img_bytes(int n_in, int h);
 size_t ks_mlp_w2_img_bytes(int h);

@@ -20,17 +20,11 @@
 // Operand layout (both A and B): K-major, no swizzle: [K/8][rows][8] bf16, i.e. each 8-row x 16-byte
 // core matrix is 128 contiguous bytes; SBO = 128 B, LBO = rows * 16 B.  A thread owns one row, so a
 // warp's 16-byte stores to one K chunk cover 512 contiguous bytes (bank-conflict free).
-#include "ks_internal.h"
-#include "ks_ptx.cuh"
+#include "ks_mlp_common.cuh"
 
 namespace {
 
-template <int FAM> struct NCols { static constexpr int v = 3; };
-template <> struct NCols<KS_FAM_GROUPED_GEMM> { static constexpr int v = 10; };
-template <> struct NCols<KS_FAM_ELEMWISE> { static constexpr int v = 2; };
-
-constexpr int kRows = 128;                 // rows per tile = TMEM lanes
-constexpr int kChunkBytes = kRows * 16;    // one K chunk (8 bf16) of a 128-row operand
+using namespace ksmlp;
 
 template <int NIN, int H>
 struct Cfg {
@@ -62,24 +56,6 @@ struct Cfg {
   static constexpr int WGCOLS = H / G;        // columns per warpgroup
   static constexpr int NCHUNK = WGCOLS / 32;  // 32-column chunks per warpgroup
 };
-
-// tanh-form GELU, fp32: 0.5 x (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3)))
-KS_PTX float gelu_f32(float x) {
-  const float x2 = x * x;
-  const float p = fmaf(x2, 0.0356774081f, 0.7978845608f);
-  const float t = ks_tanh_approx(x * p);
-  const float hx = 0.5f * x;
-  return fmaf(hx, t, hx);
-}
-// packed bf16x2 variant (two activations per instruction)
-KS_PTX uint32_t gelu_bf16x2(float a, float b) {
-  const uint32_t x = ks_pack_bf16x2(a, b);
-  const uint32_t x2 = ks_mul_bf16x2(x, x);
-  const uint32_t p = ks_fma_bf16x2(x2, 0x3D123D12u /*0.0356*/, 0x3F4C3F4Cu /*0.7969*/);
-  const uint32_t t = ks_tanh_bf16x2(ks_mul_bf16x2(x, p));
-  const uint32_t hx = ks_mul_bf16x2(x, 0x3F003F00u /*0.5*/);
-  return ks_fma_bf16x2(hx, t, hx);
-}
 
 template <int NIN, int H, int FAM>
 KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, const int t_hi, unsigned char* smem,
@@ -121,7 +97,7 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
     const int row = (t_lo + slot - tile0) * kRows + r;
     const bool ok = wg == 0 && t_lo + slot < t_hi && row < bk.n;
 #pragma unroll
-    for (int c = 0; c < NC; ++c) vn[c] = ok ? ks_load_col(bk.cols[c], row, f32cols) : 0;
+    for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], row) : 0;
   }
 
   for (int t = t_lo + slot; t < t_hi; t += C::NSLOTS) {
@@ -129,13 +105,13 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
     const bool valid = row < bk.n;
     int v[NC];
 #pragma unroll
-    for (int c = 0; c < NC; ++c) v[c] = vn[c];
+    for (int c = 0; c < NC; ++c) v[c] = col_value(vn[c], f32cols);
     {
       const int tn = t + C::NSLOTS;
       const int rown = (tn - tile0) * kRows + r;
       const bool ok = wg == 0 && tn < t_hi && rown < bk.n;
 #pragma unroll
-      for (int c = 0; c < NC; ++c) vn[c] = ok ? ks_load_col(bk.cols[c], rown, f32cols) : 0;
+      for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], rown) : 0;
     }
     for (int s = 0; s < p.n_specs; ++s) {
       const KsSpecDev& sp = p.specs.s[s];
@@ -196,11 +172,11 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
         if (gelu_mode == 0) {
 #pragma unroll
           for (int j = 0; j < 16; ++j)
-            pk[j] = ks_pack_bf16x2(gelu_f32(__uint_as_float(acc[2 * j])), gelu_f32(__uint_as_float(acc[2 * j + 1])));
+            pk[j] = ks_pack_bf16x2(gelu2_f32(__uint_as_float(acc[2 * j])), gelu2_f32(__uint_as_float(acc[2 * j + 1])));
         } else {
 #pragma unroll
           for (int j = 0; j < 16; ++j)
-            pk[j] = gelu_bf16x2(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1]));
+            pk[j] = gelu2_bf16x2(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1]));
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -270,17 +246,17 @@ KS_DEV void process_bucket(const KsMlpParams& p, const int b, const int t_lo, co
 #pragma unroll
           for (int j = 0; j < 32; j += 4) {
             const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col0 + j);
-            zp = fmaf(gelu_f32(__uint_as_float(acc[j + 0])), w4.x, zp);
-            zp = fmaf(gelu_f32(__uint_as_float(acc[j + 1])), w4.y, zp);
-            zp = fmaf(gelu_f32(__uint_as_float(acc[j + 2])), w4.z, zp);
-            zp = fmaf(gelu_f32(__uint_as_float(acc[j + 3])), w4.w, zp);
+            zp = fmaf(gelu2_f32(__uint_as_float(acc[j + 0])), w4.x, zp);
+            zp = fmaf(gelu2_f32(__uint_as_float(acc[j + 1])), w4.y, zp);
+            zp = fmaf(gelu2_f32(__uint_as_float(acc[j + 2])), w4.z, zp);
+            zp = fmaf(gelu2_f32(__uint_as_float(acc[j + 3])), w4.w, zp);
           }
         } else {
 #pragma unroll
           for (int j = 0; j < 32; j += 4) {
             const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col0 + j);
-            const uint32_t g0 = gelu_bf16x2(__uint_as_float(acc[j + 0]), __uint_as_float(acc[j + 1]));
-            const uint32_t g1 = gelu_bf16x2(__uint_as_float(acc[j + 2]), __uint_as_float(acc[j + 3]));
+            const uint32_t g0 = gelu2_bf16x2(__uint_as_float(acc[j + 0]), __uint_as_float(acc[j + 1]));
+            const uint32_t g1 = gelu2_bf16x2(__uint_as_float(acc[j + 2]), __uint_as_float(acc[j + 3]));
             zp = fmaf(__uint_as_float(g0 << 16), w4.x, zp);
             zp = fmaf(__uint_as_float(g0 & 0xffff0000u), w4.y, zp);
             zp = fmaf(__uint_as_float(g1 << 16), w4.z, zp);
@@ -389,9 +365,8 @@ size_t ks_mlp_w2_img_bytes(int h) { return (size_t)(h + 16) * h * 2; }
 cudaError_t ks_launch_mlp(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st) {
 #define KS_CASE(NI, HH) \
   if (n_in == NI && h == HH) return launch<NI, HH>(p, num_sms, st);
-  KS_CASE(8, 64) KS_CASE(8, 128) KS_CASE(8, 256)
-  KS_CASE(12, 64) KS_CASE(12, 128) KS_CASE(12, 256)
-  KS_CASE(32, 64) KS_CASE(32, 128) KS_CASE(32, 256)
+  if (h <= 128) return ks_launch_mlp_ws(p, n_in, h, num_sms, st);   // warp-specialized pipeline (ks_mlp_ws.cu)
+  KS_CASE(8, 256) KS_CASE(12, 256) KS_CASE(32, 256)
 #undef KS_CASE
   return cudaErrorInvalidValue;
 }

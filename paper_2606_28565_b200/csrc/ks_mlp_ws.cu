@@ -1,0 +1,422 @@
+// ks_mlp_ws.cu — Tier-A kernel for H <= 128: a warp-specialized pipeline around the 5th-gen tensor
+// cores.  S1-S3, S4a, S5 of DESIGN.md §1 (PAPER.md:191 Eq. 2, :199-201 per-family heads), fused.
+//
+// One persistent CTA per SM walks a contiguous range of 128-row tiles.  A work item q is one
+// (tile, spec) pair; item q uses buffer q & 1 of every double-buffered resource.
+//
+//   warps 0-3   PRODUCER  thread r owns row r: prefetch next tile's columns, decode + roofline +
+//                         features -> bf16 A1[q&1] row in smem (K-major UMMA image), t_roof -> ring
+//   warp  12    MMA       one thread: MMA1(q): D1[q&1] = A1[q&1] . W1      (b1 rides on two 1-columns)
+//                                     MMA2(q-1): D2 = A2 . W2 (+ ones-block x b2 step)
+//   warps 4-7   EPI1      D1[q&1] -> regs (tcgen05.ld, double-buffered) -> 2 GELU -> bf16 -> A2[q&1]
+//   warps 8-11  EPI2      D2[q&1] -> regs -> 2 GELU -> fp32 dot with w3/2 -> sigmoid -> latency
+//
+// so the tensor core, the activation warps of layer 1 and of layer 2 and the feature warps all work
+// on different items at the same time; nobody waits for its own MMA.  Synchronisation is by
+// mbarriers only (no CTA-wide barrier in the loop):
+//   a1_full[2]   128 producer arrivals      -> MMA may read A1[b]
+//   mma1_done[2] tcgen05.commit             -> EPI1 may read D1[b]; producer may rewrite A1[b]
+//   a2_full[2]   128 EPI1 arrivals          -> MMA may read A2[b]; D1[b] has been drained
+//   mma2_done[2] tcgen05.commit             -> EPI2 may read D2[b]; EPI1 may rewrite A2[b]
+//   d2_free[2]   128 EPI2 arrivals          -> MMA may overwrite D2[b]
+// A waiter for completion k of a barrier always runs before completion k+1 can happen (k+1 depends
+// on the waiter's own progress), so single-bit phase parity is sufficient.
+// The t_roof ring has 8 entries: the producer can be at most 5 items ahead of EPI2 (item q+6 needs
+// mma1_done(q+4), MMA1(q+4) is issued after MMA2(q+2), which waits for d2_free(q)).
+#include "ks_mlp_common.cuh"
+
+namespace {
+
+using namespace ksmlp;
+
+// Each epilogue role has two warpgroups: group g takes the items with q & 1 == g, i.e. it owns
+// buffer g.  Four activation warps per SM sub-partition keep the MUFU pipe fed while any one of
+// them waits for its next accumulator.
+constexpr int kProducerWarps = 4, kEpiWarps = 8;
+constexpr int kWsThreads = (kProducerWarps + 2 * kEpiWarps + 1) * 32;   // 672
+constexpr int kMmaWarp = kProducerWarps + 2 * kEpiWarps;
+constexpr int kRing = 8;
+
+template <int NIN, int H>
+struct WsCfg {
+  static constexpr int K1 = NIN == 32 ? 32 : 16;
+  static constexpr int BIAS_ROW = NIN == 32 ? 22 : NIN;
+  static constexpr int TMEM_COLS = 4 * H;              // D1[2], D2[2]
+  static constexpr int W1_BYTES = K1 * H * 2;
+  static constexpr int W2_BYTES = (H + 16) * H * 2;
+  static constexpr int A1_BYTES = (K1 / 8) * kChunkBytes;
+  static constexpr int A2_BYTES = (H / 8) * kChunkBytes;
+  static constexpr int ONES_BYTES = 2 * kChunkBytes;
+  static constexpr int OFF_W1 = 0;
+  static constexpr int OFF_W2 = OFF_W1 + W1_BYTES;
+  static constexpr int OFF_ONES = OFF_W2 + W2_BYTES;
+  static constexpr int OFF_A1 = OFF_ONES + ONES_BYTES;
+  static constexpr int OFF_A2 = OFF_A1 + 2 * A1_BYTES;
+  static constexpr int OFF_W3 = OFF_A2 + 2 * A2_BYTES;                 // [KS_MLP_MAX_BUCKETS][H] fp32
+  static constexpr int OFF_RING = OFF_W3 + KS_MLP_MAX_BUCKETS * H * 4; // [kRing][128] fp32 t_roof
+  static constexpr int OFF_BAR = OFF_RING + kRing * kRows * 4;
+  static constexpr int SMEM_BYTES = OFF_BAR + 128;
+  static constexpr int NCHUNK = H / 32;
+};
+
+// barrier slots inside the OFF_BAR block
+enum { BAR_W = 0, BAR_DRAIN = 1, BAR_A1_FULL = 2, BAR_MMA1 = 4, BAR_A2_FULL = 6, BAR_MMA2 = 8, BAR_D2_FREE = 10,
+       BAR_D1_FREE = 12, BAR_COUNT = 14 };
+
+struct Range { int lo, hi; };
+KS_DEV Range bucket_range(const KsMlpParams& p, int b, int t_lo, int t_hi) {
+  Range r;
+  r.lo = t_lo > p.tile_begin[b] ? t_lo : p.tile_begin[b];
+  r.hi = t_hi < p.tile_begin[b + 1] ? t_hi : p.tile_begin[b + 1];
+  return r;
+}
+
+// ------------------------------------------------------------------ PRODUCER (warps 0-3)
+template <int NIN, int H, int FAM>
+KS_DEV void producer_bucket(const KsMlpParams& p, const int b, const Range tr, unsigned char* smem, uint64_t* bars,
+                            uint32_t& q) {
+  using C = WsCfg<NIN, H>;
+  constexpr int NC = NCols<FAM>::v;
+  const int r = threadIdx.x;                       // 0..127: row within the tile
+  const KsBucketDev& bk = p.bk[b];
+  const int tile0 = p.tile_begin[b];
+  const bool f32cols = bk.col_f32 != 0;
+  float* ring = reinterpret_cast<float*>(smem + C::OFF_RING);
+
+  int vn[NC];
+  {
+    const int row = (tr.lo - tile0) * kRows + r;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) vn[c] = row < bk.n ? load_col_raw(bk.cols[c], row) : 0;
+  }
+  for (int t = tr.lo; t < tr.hi; ++t) {
+    const int row = (t - tile0) * kRows + r;
+    const bool valid = row < bk.n;
+    int v[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) v[c] = col_value(vn[c], f32cols);
+    {
+      const int rown = row + kRows;
+      const bool ok = t + 1 < tr.hi && rown < bk.n;
+#pragma unroll
+      for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], rown) : 0;
+    }
+    for (int s = 0; s < p.n_specs; ++s, ++q) {
+      const KsSpecDev& sp = p.specs.s[s];
+      uint4 a1[C::K1 / 8];
+      KsWork w;
+      KsRoof rf;
+      const float t_roof = feature_row<FAM, NIN, C::K1, C::BIAS_ROW>(v, bk, sp, a1, w, rf);
+      if (valid) {
+        const long long o = (long long)s * bk.n + row;
+        if (bk.tiles) bk.tiles[o] = (int)w.B;
+        if (bk.waves) bk.waves[o] = (int)rf.W;
+        if (bk.troof) bk.troof[o] = rf.t_roof;
+      }
+      const uint32_t buf = q & 1u;
+      if (q >= 2u) ks_mbar_wait(bars + BAR_MMA1 + buf, ((q >> 1) - 1u) & 1u);   // MMA1(q-2) has consumed A1[buf]
+      unsigned char* A1 = smem + C::OFF_A1 + buf * C::A1_BYTES;
+#pragma unroll
+      for (int kc = 0; kc < C::K1 / 8; ++kc) *reinterpret_cast<uint4*>(A1 + kc * kChunkBytes + r * 16) = a1[kc];
+      ring[(q & (kRing - 1)) * kRows + r] = t_roof;
+      ks_fence_proxy_async();                      // generic-proxy stores -> visible to the tensor core
+      ks_mbar_arrive(bars + BAR_A1_FULL + buf);
+    }
+  }
+}
+
+// ------------------------------------------------------------------ EPI1 (warps 4-7): D1 -> 2 GELU -> A2
+template <int NIN, int H, int GM>
+KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned char* smem, uint64_t* bars,
+                       const uint32_t tmem_base) {
+  using C = WsCfg<NIN, H>;
+  const int e = threadIdx.x - kProducerWarps * 32;
+  const uint32_t grp = (uint32_t)e >> 7;                           // warpgroup of this role: owns buffer grp
+  const int r = e & 127;                                           // TMEM lane = tile row
+  const uint32_t lane_off = (uint32_t)((r >> 5) * 32) << 16;
+  for (uint32_t q = grp; q < n_items; q += 2) {
+    const uint32_t buf = q & 1u, par = (q >> 1) & 1u;
+    unsigned char* A2 = smem + C::OFF_A2 + buf * C::A2_BYTES;
+    const uint32_t d1 = tmem_base + buf * H + lane_off;
+    ks_mbar_wait(bars + BAR_MMA1 + buf, par);                       // D1[buf] holds item q
+    ks_tc_fence_after();
+    // 16-column sub-chunks, double-buffered in registers: the load of sub-chunk c+1 is in flight
+    // while c is activated.  The loop stays rolled (two sub-chunks per trip) so the code of all
+    // roles together fits the 32 KB instruction cache.
+    uint32_t accA[16], accB[16];
+    ks_tmem_ld16(d1, accA);
+    if (q >= 2u) ks_mbar_wait(bars + BAR_MMA2 + buf, par ^ 1u);     // MMA2(q-2) has consumed A2[buf]
+    auto act_store = [&](const uint32_t* a, int c16) {
+      uint32_t pk[8];
+      if (GM == 0) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          pk[j] = ks_pack_bf16x2_alu(gelu2_f32(__uint_as_float(a[2 * j])), gelu2_f32(__uint_as_float(a[2 * j + 1])));
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) pk[j] = gelu2_bf16x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]));
+      }
+      *reinterpret_cast<uint4*>(A2 + (c16 * 2 + 0) * kChunkBytes + r * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+      *reinterpret_cast<uint4*>(A2 + (c16 * 2 + 1) * kChunkBytes + r * 16) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+    };
+#pragma unroll 1
+    for (int c = 0; c < H / 16; c += 2) {
+      ks_tmem_ld_wait();
+      ks_tmem_ld16(d1 + (uint32_t)((c + 1) * 16), accB);
+      act_store(accA, c);
+      ks_tmem_ld_wait();
+      if (c + 2 < H / 16) {
+        ks_tmem_ld16(d1 + (uint32_t)((c + 2) * 16), accA);
+      } else {                                     // D1[buf] is drained: MMA1(q+2) may overwrite it now
+        ks_tc_fence_before();
+        ks_mbar_arrive(bars + BAR_D1_FREE + buf);
+      }
+      act_store(accB, c + 1);
+    }
+    ks_fence_proxy_async();
+    ks_mbar_arrive(bars + BAR_A2_FULL + buf);
+  }
+}
+
+// ------------------------------------------------------------------ EPI2 (warps 8-11): D2 -> 2 GELU . w3/2 -> latency
+template <int NIN, int H, int GM>
+KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
+                     const uint32_t tmem_base) {
+  using C = WsCfg<NIN, H>;
+  const int e = threadIdx.x - (kProducerWarps + kEpiWarps) * 32;
+  const uint32_t grp = (uint32_t)e >> 7;
+  const int r = e & 127;
+  const uint32_t lane_off = (uint32_t)((r >> 5) * 32) << 16;
+  const float* ring = reinterpret_cast<const float*>(smem + C::OFF_RING);
+  uint32_t q = 0;
+  for (int b = 0; b < p.n_buckets; ++b) {
+    const Range tr = bucket_range(p, b, t_lo, t_hi);
+    const KsBucketDev& bk = p.bk[b];
+    const float* sw3 = reinterpret_cast<const float*>(smem + C::OFF_W3) + b * H;
+    const float b3 = p.head[b].b3;
+    const int tile0 = p.tile_begin[b];
+    for (int t = tr.lo; t < tr.hi; ++t) {
+      const int row = (t - tile0) * kRows + r;
+      const bool valid = row < bk.n;
+      for (int s = 0; s < p.n_specs; ++s, ++q) {
+        if ((q & 1u) != grp) continue;
+        const uint32_t buf = q & 1u, par = (q >> 1) & 1u;
+        const uint32_t d2 = tmem_base + 2 * H + buf * H + lane_off;
+        ks_mbar_wait(bars + BAR_MMA2 + buf, par);                   // D2[buf] holds item q
+        ks_tc_fence_after();
+        uint32_t accA[16], accB[16];
+        ks_tmem_ld16(d2, accA);
+        const float t_roof = ring[(q & (kRing - 1)) * kRows + r];
+        float z0 = 0.0f, z1 = 0.0f, z2 = 0.0f, z3 = 0.0f;
+        auto act_dot = [&](const uint32_t* a, int c16) {
+          if (GM == 0) {
+#pragma unroll
+            for (int j = 0; j < 16; j += 4) {
+              const float4 w4 = *reinterpret_cast<const float4*>(sw3 + c16 * 16 + j);
+              z0 = fmaf(gelu2_f32(__uint_as_float(a[j + 0])), w4.x, z0);
+              z1 = fmaf(gelu2_f32(__uint_as_float(a[j + 1])), w4.y, z1);
+              z2 = fmaf(gelu2_f32(__uint_as_float(a[j + 2])), w4.z, z2);
+              z3 = fmaf(gelu2_f32(__uint_as_float(a[j + 3])), w4.w, z3);
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 16; j += 4) {
+              const float4 w4 = *reinterpret_cast<const float4*>(sw3 + c16 * 16 + j);
+              const uint32_t g0 = gelu2_bf16x2(__uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]));
+              const uint32_t g1 = gelu2_bf16x2(__uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]));
+              z0 = fmaf(__uint_as_float(g0 << 16), w4.x, z0);
+              z1 = fmaf(__uint_as_float(g0 & 0xffff0000u), w4.y, z1);
+              z2 = fmaf(__uint_as_float(g1 << 16), w4.z, z2);
+              z3 = fmaf(__uint_as_float(g1 & 0xffff0000u), w4.w, z3);
+            }
+          }
+        };
+#pragma unroll 1
+        for (int c = 0; c < H / 16; c += 2) {
+          ks_tmem_ld_wait();
+          ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
+          act_dot(accA, c);
+          ks_tmem_ld_wait();
+          if (c + 2 < H / 16) ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
+          act_dot(accB, c + 1);
+        }
+        ks_tc_fence_before();                      // orders this thread's tcgen05.ld before MMA2(q+2)
+        ks_mbar_arrive(bars + BAR_D2_FREE + buf);
+        if (valid) {
+          const float z = ((z0 + z1) + (z2 + z3)) + b3;
+          // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
+          const float eta = fminf(1.0f + __expf(-z), 1024.0f);
+          bk.lat[(long long)s * bk.n + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ MMA issuer (one thread of warp 12)
+template <int NIN, int H>
+KS_DEV void mma_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
+                    const uint32_t tmem_base) {
+  using C = WsCfg<NIN, H>;
+  constexpr uint32_t idesc = ks_umma_idesc_bf16(128, H);
+  constexpr uint32_t B_LBO = H * 16;
+  const uint32_t w1_addr = ks_smem_u32(smem + C::OFF_W1);
+  const uint32_t w2_addr = ks_smem_u32(smem + C::OFF_W2);
+  const uint32_t ones_addr = ks_smem_u32(smem + C::OFF_ONES);
+  const uint32_t a1_addr = ks_smem_u32(smem + C::OFF_A1);
+  const uint32_t a2_addr = ks_smem_u32(smem + C::OFF_A2);
+  uint32_t wphase = 0, dphase = 0, q = 0;
+
+  auto mma2 = [&](uint32_t i) {                     // D2[i&1] = A2[i&1] . W2 + ones x b2
+    const uint32_t buf = i & 1u, par = (i >> 1) & 1u;
+    ks_mbar_wait_backoff(bars + BAR_A2_FULL + buf, par);
+    if (i >= 2u) ks_mbar_wait_backoff(bars + BAR_D2_FREE + buf, par ^ 1u);
+    ks_tc_fence_after();
+    const uint32_t d2 = tmem_base + 2 * H + buf * H;
+    const uint32_t a = a2_addr + buf * C::A2_BYTES;
+#pragma unroll
+    for (int k16 = 0; k16 < H / 16; ++k16) {
+      const uint64_t ad = ks_umma_desc(a + k16 * 2 * kChunkBytes, kChunkBytes, 128);
+      const uint64_t bd = ks_umma_desc(w2_addr + k16 * 2 * B_LBO, B_LBO, 128);
+      ks_umma_bf16(d2, ad, bd, idesc, k16 > 0 ? 1u : 0u);
+    }
+    const uint64_t ad = ks_umma_desc(ones_addr, kChunkBytes, 128);
+    const uint64_t bd = ks_umma_desc(w2_addr + (H / 8) * B_LBO, B_LBO, 128);
+    ks_umma_bf16(d2, ad, bd, idesc, 1u);
+    ks_umma_commit(bars + BAR_MMA2 + buf);
+  };
+
+  auto mma1 = [&](uint32_t i) {                     // D1[i&1] = A1[i&1] . W1
+    const uint32_t buf = i & 1u, par = (i >> 1) & 1u;
+    ks_mbar_wait_backoff(bars + BAR_A1_FULL + buf, par);
+    ks_tc_fence_after();
+    const uint32_t d1 = tmem_base + buf * H;
+    const uint32_t a = a1_addr + buf * C::A1_BYTES;
+#pragma unroll
+    for (int k = 0; k < C::K1 / 16; ++k) {
+      const uint64_t ad = ks_umma_desc(a + k * 2 * kChunkBytes, kChunkBytes, 128);
+      const uint64_t bd = ks_umma_desc(w1_addr + k * 2 * B_LBO, B_LBO, 128);
+      ks_umma_bf16(d1, ad, bd, idesc, k > 0 ? 1u : 0u);
+    }
+    ks_umma_commit(bars + BAR_MMA1 + buf);
+  };
+
+  for (int b = 0; b < p.n_buckets; ++b) {
+    const Range tr = bucket_range(p, b, t_lo, t_hi);
+    if (tr.lo >= tr.hi) continue;
+    if (q > 0u) {                                   // every MMA that reads the previous family's weights is done
+      ks_umma_commit(bars + BAR_DRAIN);
+      ks_mbar_wait_backoff(bars + BAR_DRAIN, dphase);
+      dphase ^= 1u;
+    }
+    ks_mbar_expect_tx(bars + BAR_W, (uint32_t)(C::W1_BYTES + C::W2_BYTES));
+    ks_bulk_g2s(smem + C::OFF_W1, p.head[b].w1_img, C::W1_BYTES, bars + BAR_W);
+    for (int off = 0; off < C::W2_BYTES; off += 32768) {
+      const int len = C::W2_BYTES - off < 32768 ? C::W2_BYTES - off : 32768;
+      ks_bulk_g2s(smem + C::OFF_W2 + off, reinterpret_cast<const char*>(p.head[b].w2_img) + off, len, bars + BAR_W);
+    }
+    ks_mbar_wait_backoff(bars + BAR_W, wphase);
+    wphase ^= 1u;
+    const uint32_t q0 = q;
+    const uint32_t q1 = q0 + (uint32_t)(tr.hi - tr.lo) * (uint32_t)p.n_specs;
+    // D1[0], D1[1] are free here: every a2_full of the previous family was waited for before its MMA2
+    mma1(q0);
+    if (q0 + 1u < q1) mma1(q0 + 1u);
+    for (q = q0; q < q1; ++q) {
+      if (q + 2u < q1) {                            // the short layer-1 MMA goes first: EPI1 never waits for MMA2
+        ks_mbar_wait_backoff(bars + BAR_D1_FREE + (q & 1u), (q >> 1) & 1u);
+        mma1(q + 2u);
+      }
+      mma2(q);
+    }
+  }
+}
+
+template <int NIN, int H>
+__global__ void __launch_bounds__(kWsThreads, 1)
+ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
+  using C = WsCfg<NIN, H>;
+  extern __shared__ __align__(1024) unsigned char smem[];
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + BAR_COUNT);
+  const int tid = threadIdx.x;
+  const int warp = tid >> 5;
+
+  if (tid == 0) {
+    ks_mbar_init(bars + BAR_W, 1);
+    ks_mbar_init(bars + BAR_DRAIN, 1);
+    for (int i = 0; i < 2; ++i) {
+      ks_mbar_init(bars + BAR_A1_FULL + i, 128);
+      ks_mbar_init(bars + BAR_MMA1 + i, 1);
+      ks_mbar_init(bars + BAR_A2_FULL + i, 128);
+      ks_mbar_init(bars + BAR_MMA2 + i, 1);
+      ks_mbar_init(bars + BAR_D2_FREE + i, 128);
+      ks_mbar_init(bars + BAR_D1_FREE + i, 128);
+    }
+    ks_fence_mbar_init();
+  }
+  if (warp == 0) { ks_tmem_alloc(tmem_slot, C::TMEM_COLS); ks_tmem_relinquish(); }
+  if (tid < 128) {   // constant ones-block: K chunk 0 = {1, 1, 0, ...} per row, K chunk 1 = 0
+    *reinterpret_cast<uint4*>(smem + C::OFF_ONES + tid * 16) = make_uint4(0x3F803F80u, 0u, 0u, 0u);
+    *reinterpret_cast<uint4*>(smem + C::OFF_ONES + kChunkBytes + tid * 16) = make_uint4(0u, 0u, 0u, 0u);
+  }
+  for (int i = tid; i < p.n_buckets * H; i += kWsThreads)       // layer-3 weights of every family
+    reinterpret_cast<float*>(smem + C::OFF_W3)[i] = __ldg(p.head[i / H].w3 + (i % H));
+  ks_fence_proxy_async();
+  ks_tc_fence_before();
+  __syncthreads();
+  ks_tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  const long long total = p.tile_begin[p.n_buckets];
+  const int t_lo = (int)((long long)blockIdx.x * total / gridDim.x);
+  const int t_hi = (int)((long long)(blockIdx.x + 1) * total / gridDim.x);
+
+  if (warp < kProducerWarps) {
+    uint32_t q = 0;
+    for (int b = 0; b < p.n_buckets; ++b) {
+      const Range tr = bucket_range(p, b, t_lo, t_hi);
+      if (tr.lo >= tr.hi) continue;
+      switch (p.bk[b].family) {
+        case KS_FAM_GEMM: producer_bucket<NIN, H, KS_FAM_GEMM>(p, b, tr, smem, bars, q); break;
+        case KS_FAM_GROUPED_GEMM: producer_bucket<NIN, H, KS_FAM_GROUPED_GEMM>(p, b, tr, smem, bars, q); break;
+        case KS_FAM_ATTN: producer_bucket<NIN, H, KS_FAM_ATTN>(p, b, tr, smem, bars, q); break;
+        default: producer_bucket<NIN, H, KS_FAM_ELEMWISE>(p, b, tr, smem, bars, q); break;
+      }
+    }
+  } else if (warp < kProducerWarps + kEpiWarps) {
+    if (p.gelu_mode == 0) epi1_items<NIN, H, 0>(p, (uint32_t)(t_hi - t_lo) * (uint32_t)p.n_specs, smem, bars, tmem_base);
+    else epi1_items<NIN, H, 1>(p, (uint32_t)(t_hi - t_lo) * (uint32_t)p.n_specs, smem, bars, tmem_base);
+  } else if (warp < kMmaWarp) {
+    if (p.gelu_mode == 0) epi2_all<NIN, H, 0>(p, t_lo, t_hi, smem, bars, tmem_base);
+    else epi2_all<NIN, H, 1>(p, t_lo, t_hi, smem, bars, tmem_base);
+  } else if (tid == kMmaWarp * 32) {
+    mma_all<NIN, H>(p, t_lo, t_hi, smem, bars, tmem_base);
+  }
+  ks_tc_fence_before();
+  __syncthreads();
+  if (warp == 0) ks_tmem_dealloc(tmem_base, C::TMEM_COLS);
+}
+
+template <int NIN, int H>
+cudaError_t launch_ws(const KsMlpParams& p, int num_sms, cudaStream_t st) {
+  using C = WsCfg<NIN, H>;
+  const int total = p.tile_begin[p.n_buckets];
+  if (total <= 0) return cudaSuccess;
+  const int grid = total < num_sms ? total : num_sms;
+  auto kern = ks_mlp_ws_kernel<NIN, H>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  kern<<<grid, kWsThreads, C::SMEM_BYTES, st>>>(p);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t ks_launch_mlp_ws(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st) {
+#define KS_CASE(NI, HH) \
+  if (n_in == NI && h == HH) return launch_ws<NI, HH>(p, num_sms, st);
+  KS_CASE(8, 64) KS_CASE(8, 128) KS_CASE(12, 64) KS_CASE(12, 128) KS_CASE(32, 64) KS_CASE(32, 128)
+#undef KS_CASE
+  return cudaErrorInvalidValue;
+}

@@ -30,6 +30,26 @@ KS_PTX void ks_mbar_wait(uint64_t* bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
+// Same wait for a lone polling thread (the MMA issuer): back off between polls so the spin does
+// not take issue slots from the activation warps that share its SM sub-partition.
+KS_PTX void ks_mbar_wait_backoff(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(done)
+        : "r"(ks_smem_u32(bar)), "r"(parity)
+        : "memory");
+    if (!done) __nanosleep(40);
+  } while (!done);
+}
+KS_PTX void ks_mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ks_smem_u32(bar)) : "memory");
+}
 // make mbarrier.init visible to the async proxy (TMA / tcgen05.commit)
 KS_PTX void ks_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -96,6 +116,16 @@ KS_PTX void ks_tmem_ld32(uint32_t taddr, uint32_t* r) {
       : "r"(taddr)
       : "memory");
 }
+// 32 lanes x 16 consecutive fp32 columns
+KS_PTX void ks_tmem_ld16(uint32_t taddr, uint32_t* r) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+}
 KS_PTX void ks_tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ------------------------------------------------------------------ UMMA descriptors (sm_100)
@@ -132,6 +162,11 @@ KS_PTX uint32_t ks_pack_bf16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
+}
+// Same packing on the ALU pipe (IADD + PRMT) instead of F2FP, which shares the 16-lane XU pipe
+// with MUFU.TANH: round-to-nearest with ties away from zero (differs from RNE only on exact ties).
+KS_PTX uint32_t ks_pack_bf16x2_alu(float lo, float hi) {
+  return __byte_perm(__float_as_uint(lo) + 0x8000u, __float_as_uint(hi) + 0x8000u, 0x7632);
 }
 KS_PTX uint32_t ks_fma_bf16x2(uint32_t a, uint32_t b, uint32_t c) {
   uint32_t d;
