@@ -22,12 +22,12 @@ KS_PTX void ks_mbar_wait(uint64_t* bar, uint32_t parity) {
       "{\n\t"
       ".reg .pred p;\n\t"
       "KS_WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
       "@p bra KS_DONE_%=;\n\t"
       "bra KS_WAIT_%=;\n\t"
       "KS_DONE_%=:\n\t"
       "}" ::"r"(ks_smem_u32(bar)),
-      "r"(parity)
+      "r"(parity), "r"(0x989680u)   // suspend-time hint: sleep in hardware instead of re-polling
       : "memory");
 }
 // Same wait for a lone polling thread (the MMA issuer): back off between polls so the spin does
