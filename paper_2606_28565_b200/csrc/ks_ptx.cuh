@@ -66,6 +66,14 @@ KS_PTX void ks_bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, ui
       : "memory");
 }
 
+// ------------------------------------------------------------------ cp.async (LDGSTS): 16-byte global -> shared, L2 only
+KS_PTX void ks_cp_async16(void* dst_smem, const void* src_gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(ks_smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+KS_PTX void ks_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+KS_PTX void ks_cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // ------------------------------------------------------------------ named barriers (sub-CTA sync)
 KS_PTX void ks_bar_sync(uint32_t id, uint32_t nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
