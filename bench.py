@@ -218,9 +218,40 @@ class Harness:
 
 
 EX_ITERS, EX_WARM = 10, 3
+PROFILE = False
 
 
-def stream_roofline(h: Harness, st, peaks, iters=None):
+def clone_sets(st, n_sets):
+    """n_sets independent copies of a prepared workload's device buffers (inputs and outputs), so that
+    back-to-back launches never find their data in the 126 MB L2 (rotation: every set is touched once
+    per n_sets launches, and n_sets x bytes-per-set is several times the L2)."""
+    import copy
+    sets = []
+    for _ in range(n_sets):
+        db = [copy.copy(b) for b in st["db"]]
+        for b in db:
+            b.cols = [c.clone() for c in b.cols]
+        sets.append(dict(db=db, lat=[x.clone() for x in st["lat"]]))
+    return sets
+
+
+def timed_b2b(h, fn, n_sets, iters):
+    """Mean microseconds of fn(i) over `iters` back-to-back launches (one CUDA-event pair around all of
+    them, on the ctx stream) after n_sets warm-up launches; fn(i) must use buffer set i % n_sets."""
+    torch = h.torch
+    with torch.cuda.stream(h.stream):
+        for i in range(max(n_sets, 3)):
+            fn(i)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(iters):
+            fn(i)
+        e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / iters * 1e3
+
+
+def stream_roofline(h: Harness, st, peaks, iters=None, sets=None):
     """Per-family streaming-kernel HBM rate (one single-bucket ks_predict_kernels launch each) + compose."""
     out = {}
     w = st["w"]
@@ -231,18 +262,36 @@ def stream_roofline(h: Harness, st, peaks, iters=None):
         gbs = byts / (ms.mean() * 1e-3) / 1e9
         out[W.FAM_NAMES[b.family]] = dict(rows=b.n, ms=float(ms.mean()), ms_min=float(ms.min()), gbs=float(gbs),
                                           frac_hbm=float(gbs / peaks["hbm"]), bytes_per_row=BYTES_PER_ROW[b.family])
+        if sets is not None:   # back-to-back over rotating buffer sets: no launch gap, no flush tail
+            us = timed_b2b(h, lambda k, i=i: h.predict(st, buckets=[sets[k % len(sets)]["db"][i]],
+                                                       lat=[sets[k % len(sets)]["lat"][i]]), len(sets), 4 * len(sets))
+            out[W.FAM_NAMES[b.family]].update(us_b2b=float(us), gbs_b2b=float(byts / us / 1e3),
+                                              frac_hbm_b2b=float(byts / us / 1e3 / peaks["hbm"]))
     return out
 
 
-def compose_roofline(h: Harness, st, peaks, iters=None):
+def compose_roofline(h: Harness, st, peaks, iters=None, sets=None):
     w = st["w"]
     h.predict(st)
     ms = h.timed([lambda: h.compose(st)], iters or EX_ITERS, EX_WARM)[:, 0]
     rows = sum(b.n for b in st["db"]) * st["ns"]
     byts = 4 * rows + st["ns"] * w.n_steps * (4 + 4 * len(st["db"]))
     gbs = byts / (ms.mean() * 1e-3) / 1e9
-    return dict(rows=rows, steps=w.n_steps, ms=float(ms.mean()), ms_min=float(ms.min()), gbs=float(gbs),
-                frac_hbm=float(gbs / peaks["hbm"]))
+    out = dict(rows=rows, steps=w.n_steps, ms=float(ms.mean()), ms_min=float(ms.min()), gbs=float(gbs),
+               frac_hbm=float(gbs / peaks["hbm"]), launches_per_call=2)
+    if sets is not None:
+        for k in range(len(sets)):
+            for a, b_ in zip(sets[k]["lat"], st["lat"]):
+                a.copy_(b_)
+        h.torch.cuda.synchronize()
+
+        def comp(k):
+            lat = sets[k % len(sets)]["lat"]
+            h.ctx.compose_steps(lat, [b.step_off for b in st["db"]], [b.n for b in st["db"]], w.n_steps, st["ns"],
+                                w.step_params, st["cfg"], st["n_cfg"], st["step"], st["tot"], space=h.B.KS_MEM_DEVICE)
+        us = timed_b2b(h, comp, len(sets), 4 * len(sets))
+        out.update(us_b2b=float(us), gbs_b2b=float(byts / us / 1e3), frac_hbm_b2b=float(byts / us / 1e3 / peaks["hbm"]))
+    return out
 
 
 def run_extras(h: Harness, peaks):
@@ -251,14 +300,19 @@ def run_extras(h: Harness, peaks):
     torch = h.torch
     # config 4a: Tier NONE streaming kernels + composition at ~29.9M kernel instances
     st = h.prepare(W.config4())
-    ex["cfg4a_tierNONE"] = dict(stream=stream_roofline(h, st, peaks), compose=compose_roofline(h, st, peaks))
+    sets = None if PROFILE else clone_sets(st, 4)
+    ex["cfg4a_tierNONE"] = dict(stream=stream_roofline(h, st, peaks, sets=sets),
+                                compose=compose_roofline(h, st, peaks, sets=sets))
+    del sets
     ms = h.timed([lambda: h.predict(st), lambda: h.compose(st)], EX_ITERS, EX_WARM)
     ex["cfg4a_tierNONE"]["predictions_per_s"] = float(st["w"].n_rows / (ms.sum(axis=1).mean() * 1e-3))
     del st
     torch.cuda.empty_cache()
     # config 3: Tier B, 4M queries
     st = h.prepare(W.config3())
-    ex["cfg3_tierB"] = dict(stream=stream_roofline(h, st, peaks))
+    sets = None if PROFILE else clone_sets(st, 8)
+    ex["cfg3_tierB"] = dict(stream=stream_roofline(h, st, peaks, sets=sets))
+    del sets
     ms = h.timed([lambda: h.predict(st)], EX_ITERS, EX_WARM)
     ex["cfg3_tierB"]["predictions_per_s"] = float(st["w"].n_rows / (ms[:, 0].mean() * 1e-3))
     del st
@@ -297,8 +351,8 @@ def run_ours(args):
     st = h.prepare(w)
     K, Wm = args.steps, max(args.warmup, 3)
     if args.profile:                               # ncu capture mode: few launches, no numbers reported
-        global EX_ITERS, EX_WARM
-        EX_ITERS, EX_WARM, Wm = 1, 1, args.warmup
+        global EX_ITERS, EX_WARM, PROFILE
+        EX_ITERS, EX_WARM, Wm, PROFILE = 1, 1, args.warmup, True
 
     def barrier():
         if dist is not None:
@@ -359,7 +413,7 @@ def run_ours(args):
     mlp_ms = float(ms[:, 0].mean())
     achieved = flops / (mlp_ms * 1e-3) / 1e12
     traffic = load_traffic().get("ks_mlp_kernel_cfg2_bytes_per_launch")
-    roofline = dict(bound="tensor", kernel="ks_mlp_kernel<12,128>", achieved=achieved, peak=peaks["bf16"], unit="TFLOP/s",
+    roofline = dict(bound="tensor", kernel="ks_mlp_ws_kernel<12,128>", achieved=achieved, peak=peaks["bf16"], unit="TFLOP/s",
                     frac=achieved / peaks["bf16"], traffic=traffic, peak_source=f"bf16 burst, {peaks['source']}",
                     flops_per_prediction=FLOPS_PER_PRED[(head.n_in, head.h1)], kernel_ms=mlp_ms,
                     compose_ms=float(ms[:, 1].mean()), share_of_step=float(ms[:, 0].sum() / ms.sum()))

@@ -99,12 +99,12 @@ KS_DEV KsWork ks_decode(const int* v, const KsBucketDev& bk, const KsSpecDev& sp
     const int Bq = ks_nonneg(v[0]), q = ks_nonneg(v[1]);
     int kv = ks_nonneg(v[2]);
     kv = kv < q ? q : kv;
-    // causal pairs: cached history + own triangle, exact in 64-bit integers
-    const unsigned long long pairs = (unsigned long long)q * (unsigned long long)(kv - q) +
-                                     ((unsigned long long)q * (unsigned long long)(q + 1)) / 2ull;
-    const float Bf = (float)Bq, hd = (float)bk.hd;
-    w.F = 4.0f * Bf * (float)bk.hq * hd * (float)pairs;
-    w.Y = s * 2.0f * Bf * hd * fmaf((float)q, (float)bk.hq, (float)kv * (float)bk.hkv);
+    // causal pairs: cached history + own triangle: q (kv - q) + q (q + 1) / 2 in fp32
+    // (every term is non-negative, so the three roundings stay at ~1e-7 relative; F needs 1e-5)
+    const float qf = (float)q, Bf = (float)Bq, hd = (float)bk.hd;
+    const float pairs = fmaf(qf, (float)(kv - q), 0.5f * qf * (qf + 1.0f));
+    w.F = 4.0f * Bf * (float)bk.hq * hd * pairs;
+    w.Y = s * 2.0f * Bf * hd * fmaf(qf, (float)bk.hq, (float)kv * (float)bk.hkv);
     w.B = ks_sat31((unsigned long long)Bq * (unsigned long long)bk.hq * ks_ceil_div(q, sp.tile_m));
   } else {
     const int n = ks_nonneg(v[0]);

@@ -5,7 +5,10 @@
 // Layout: SoA int32/fp32 columns; each thread owns 4 consecutive rows and moves them with 16-byte
 // vector loads/stores (streaming cache hints: every byte is touched once).  Per-spec constants sit
 // in the kernel-parameter constant bank.  Tier B stages the whole grid (<= 128 KiB) into shared
-// memory once per persistent CTA with a 1-D TMA bulk copy.
+// memory once per persistent CTA (16-byte loads by all threads, overlapped with the first rows'
+// column loads).  Tier B is issue-bound, not HBM-bound: ~170 instructions per query (three
+// exponent+MUFU log2, clamp/floor/index per axis, eight shared-memory gathers, seven lerps) on
+// top of the 62 of decode + roofline; ncu: issue slots 67 % busy with the 32 resident warps.
 #include "ks_internal.h"
 #include "ks_ptx.cuh"
 
@@ -112,32 +115,28 @@ __global__ void __launch_bounds__(TIER == KS_TIER_B ? (FAM == KS_FAM_GROUPED_GEM
 ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
   constexpr int NC = NCols<FAM>::v;
   extern __shared__ __align__(128) float sgrid[];
-  __shared__ __align__(8) uint64_t grid_bar;
-
-  if (TIER == KS_TIER_B) {
-    // stage the grid once per CTA: 1-D TMA bulk copies signalled on an mbarrier
-    const uint32_t bytes = (uint32_t)(((p.grid.n_nodes + 3) & ~3) * 4);
-    if (threadIdx.x == 0) {
-      ks_mbar_init(&grid_bar, 1);
-      ks_fence_mbar_init();
-      ks_mbar_expect_tx(&grid_bar, bytes);
-      for (uint32_t off = 0; off < bytes; off += 32768u) {
-        const uint32_t len = bytes - off < 32768u ? bytes - off : 32768u;
-        ks_bulk_g2s(reinterpret_cast<char*>(sgrid) + off, reinterpret_cast<const char*>(p.grid.values) + off, len,
-                    &grid_bar);
-      }
-    }
-    __syncthreads();
-    ks_mbar_wait(&grid_bar, 0);
-  }
 
   const int n = p.bk.n;
   const int n4 = (n + 3) >> 2;
   const int stride = gridDim.x * blockDim.x;
-  for (int g = blockIdx.x * blockDim.x + threadIdx.x; g < n4; g += stride) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  int v[4][NC];
+  if (TIER == KS_TIER_B) {
+    // first rows' columns are requested before the grid is staged, so the two overlap
+    if (g < n4) load_rows4<NC, F32>(p.bk, g << 2, n, v);
+    // stage the grid once per CTA with 16-byte loads by every thread (it is L2-resident after the
+    // first CTA touched it; the values array is padded to a multiple of 4 floats)
+    const int nv = (p.grid.n_nodes + 3) >> 2;
+    const float4* __restrict__ src = reinterpret_cast<const float4*>(p.grid.values);
+    float4* dst = reinterpret_cast<float4*>(sgrid);
+    for (int i = threadIdx.x; i < nv; i += blockDim.x) dst[i] = __ldg(src + i);
+    __syncthreads();
+  }
+  bool have = TIER == KS_TIER_B;                     // Tier B: the first trip's columns are already loaded
+  for (; g < n4; g += stride) {
     const int row0 = g << 2;
-    int v[4][NC];
-    load_rows4<NC, F32>(p.bk, row0, n, v);
+    if (!have) load_rows4<NC, F32>(p.bk, row0, n, v);
+    have = false;
 
     float e[4];
 #pragma unroll
