@@ -25,6 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2606_28565_b200 import sharding as S  # noqa: E402
 from paper_2606_28565_b200 import workloads as W  # noqa: E402
 
 METRIC = "kernel_latency_predictions_per_sec"
@@ -347,7 +348,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     peaks = load_peaks()
     h = Harness(local)
-    w = W.config2(seed=1 + 1000 * rank)            # every rank its own shard of the same recipe
+    w = W.config2(seed=S.shard_seed(1, rank))      # every rank its own shard of the same recipe
     st = h.prepare(w)
     K, Wm = args.steps, max(args.warmup, 3)
     if args.profile:                               # ncu capture mode: few launches, no numbers reported
@@ -371,10 +372,7 @@ def run_ours(args):
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
     launches = h.ctx.launch_count() - launches0
-    total_ms = torch.tensor([float(ms.sum())], device=h.dev, dtype=torch.float64)
-    if dist is not None:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    total_s = float(total_ms.item()) * 1e-3
+    total_s = S.max_over_ranks(float(ms.sum()) * 1e-3, dist, h.dev)      # device time, max over ranks
     value = world * w.n_rows * K / total_s
 
     # end to end through the C ABI with HOST (pinned) buffers: H2D + kernels + D2H inside the timed region
@@ -397,12 +395,10 @@ def run_ours(args):
     for _ in range(Ke):
         e2e_step()
     torch.cuda.synchronize()
-    e2e_s = torch.tensor([time.perf_counter() - t0], device=h.dev, dtype=torch.float64)
-    if dist is not None:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_s = S.max_over_ranks(time.perf_counter() - t0, dist, h.dev)
     h2d = sum(4 * b.n * len(b.cols) + 4 * (w.n_steps + 1) for b in hb) + 4 * (n_cfg + 1)
     d2h = sum(4 * b.n for b in hb) + 4 * w.n_steps + 4 * n_cfg
-    e2e = dict(value=world * w.n_rows * Ke / float(e2e_s.item()), unit=UNIT, h2d_bytes_per_step=int(h2d),
+    e2e = dict(value=world * w.n_rows * Ke / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d),
                d2h_bytes_per_step=int(d2h))
 
     if rank != 0:
