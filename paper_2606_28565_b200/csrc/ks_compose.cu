@@ -30,7 +30,7 @@ KS_DEV float lane_tail(const float* __restrict__ src, int n, int lane) {
   return a0 + a1;
 }
 
-// NB = compile-time bound on the bucket count (4 or 8): the bucket loop is fully unrolled so the
+// NB = compile-time bound on the bucket count (1-4: exact, or 8): the bucket loop is fully unrolled so the
 // loads of every bucket are in flight before the first add
 template <int NB>
 __global__ void __launch_bounds__(kThreads, NB <= 4 ? 4 : 2)
@@ -141,7 +141,8 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
   const long long total = (long long)p.n_specs * p.n_steps;
   if (total > 0) {
     const long long n_pairs = (long long)((p.n_steps + 1) / 2) * p.n_specs;
-    auto kern = p.n_batches <= 4 ? ks_compose_kernel<4> : ks_compose_kernel<8>;
+    auto kern = p.n_batches <= 1 ? ks_compose_kernel<1> : p.n_batches == 2 ? ks_compose_kernel<2> :
+                p.n_batches == 3 ? ks_compose_kernel<3> : p.n_batches == 4 ? ks_compose_kernel<4> : ks_compose_kernel<8>;
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, 0);
     if (e != cudaSuccess) return e;
