@@ -43,6 +43,10 @@ struct ks_ctx {
   // grow-only device workspace with a bump pointer (host-space staging, internal latencies)
   char* ws = nullptr;
   size_t ws_cap = 0, ws_used = 0;
+  // host-space pipeline of ks_run_steps: bucket b's H2D copies run on `h2d` while bucket b-1 is
+  // predicted on `stream` and bucket b-2's latencies return on `d2h` (created on first use)
+  cudaStream_t h2d = nullptr, d2h = nullptr;
+  cudaEvent_t ev_in[KS_MAX_BATCHES] = {}, ev_out[KS_MAX_BATCHES] = {}, ev_start = nullptr;
 };
 
 namespace {
@@ -84,6 +88,18 @@ void* ws_take(ks_ctx* c, size_t bytes) {
   void* p = c->ws + c->ws_used;
   c->ws_used += align_up(bytes, 256);
   return p;
+}
+
+ks_status pipeline_init(ks_ctx* c) {
+  if (c->h2d) return KS_OK;
+  KS_CUDA(c, cudaStreamCreateWithFlags(&c->h2d, cudaStreamNonBlocking));
+  KS_CUDA(c, cudaStreamCreateWithFlags(&c->d2h, cudaStreamNonBlocking));
+  for (int b = 0; b < KS_MAX_BATCHES; ++b) {
+    KS_CUDA(c, cudaEventCreateWithFlags(&c->ev_in[b], cudaEventDisableTiming));
+    KS_CUDA(c, cudaEventCreateWithFlags(&c->ev_out[b], cudaEventDisableTiming));
+  }
+  KS_CUDA(c, cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+  return KS_OK;
 }
 
 // fp32 -> bf16 bits, round to nearest even (NaN kept quiet)
@@ -298,6 +314,13 @@ ks_status ks_destroy(ks_ctx* c) {
     cudaFree(c->grids[f].values);
   }
   cudaFree(c->ws);
+  if (c->h2d) cudaStreamDestroy(c->h2d);
+  if (c->d2h) cudaStreamDestroy(c->d2h);
+  for (int b = 0; b < KS_MAX_BATCHES; ++b) {
+    if (c->ev_in[b]) cudaEventDestroy(c->ev_in[b]);
+    if (c->ev_out[b]) cudaEventDestroy(c->ev_out[b]);
+  }
+  if (c->ev_start) cudaEventDestroy(c->ev_start);
   cudaGetLastError();
   delete c;
   return KS_OK;
@@ -620,48 +643,71 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   DevOut outs[KS_MAX_BATCHES];
   const float* dlat[KS_MAX_BATCHES];
   const int32_t* doff[KS_MAX_BATCHES];
+  if (dev) {
+    for (int b = 0; b < n_batches; ++b) {
+      for (int k = 0; k < batches[b].n_cols; ++k) cols[b][k] = batches[b].cols[k];
+      outs[b].lat = (latency && latency[b]) ? latency[b]
+                                            : static_cast<float*>(ws_take(c, (size_t)batches[b].n * n_specs * 4));
+      dlat[b] = outs[b].lat;
+      doff[b] = step_off[b];
+    }
+    if (n_specs > 0 && n_batches > 0) {
+      st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+      if (st != KS_OK) return st;
+    }
+    return compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg, step_latency,
+                          cfg_latency);
+  }
+
+  // ---- host space: a three-stream pipeline over the buckets (largest copy first is the caller's
+  // order).  h2d: columns + offsets of bucket b; stream: predict bucket b as soon as its inputs have
+  // landed; d2h: bucket b's latencies go back while bucket b+1 is predicted.  Composition and the
+  // small step/config results stay on the ctx stream.  Ends with a synchronisation of both.
+  st = pipeline_init(c);
+  if (st != KS_OK) return st;
+  KS_CUDA(c, cudaEventRecord(c->ev_start, c->stream));            // earlier work on the ctx stream owns the workspace
+  KS_CUDA(c, cudaStreamWaitEvent(c->h2d, c->ev_start, 0));
   for (int b = 0; b < n_batches; ++b) {
     const size_t n = batches[b].n;
     for (int k = 0; k < batches[b].n_cols; ++k) {
-      if (dev) { cols[b][k] = batches[b].cols[k]; continue; }
       void* d = ws_take(c, n * 4);
-      if (n) KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+      if (n) KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[k], n * 4, cudaMemcpyHostToDevice, c->h2d));
       cols[b][k] = d;
     }
-    outs[b].lat = (dev && latency && latency[b]) ? latency[b] : static_cast<float*>(ws_take(c, n * (size_t)n_specs * 4));
-    dlat[b] = outs[b].lat;
-    if (dev) { doff[b] = step_off[b]; continue; }
     int32_t* dofs = static_cast<int32_t*>(ws_take(c, (size_t)(n_steps + 1) * 4));
-    KS_CUDA(c, cudaMemcpyAsync(dofs, step_off[b], (size_t)(n_steps + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    KS_CUDA(c, cudaMemcpyAsync(dofs, step_off[b], (size_t)(n_steps + 1) * 4, cudaMemcpyHostToDevice, c->h2d));
     doff[b] = dofs;
+    outs[b].lat = static_cast<float*>(ws_take(c, n * (size_t)n_specs * 4));
+    dlat[b] = outs[b].lat;
+    KS_CUDA(c, cudaEventRecord(c->ev_in[b], c->h2d));
   }
-  const int32_t* dcfg = cfg_off;
-  float *dstep = step_latency, *dtot = cfg_latency;
-  if (!dev) {
-    int32_t* t = static_cast<int32_t*>(ws_take(c, (size_t)(n_cfg + 1) * 4));
-    if (n_cfg > 0) KS_CUDA(c, cudaMemcpyAsync(t, cfg_off, (size_t)(n_cfg + 1) * 4, cudaMemcpyHostToDevice, c->stream));
-    dcfg = t;
-    dstep = static_cast<float*>(ws_take(c, (size_t)n_steps * n_specs * 4));
-    dtot = static_cast<float*>(ws_take(c, (size_t)n_cfg * n_specs * 4 + 4));
+  int32_t* dcfg = static_cast<int32_t*>(ws_take(c, (size_t)(n_cfg + 1) * 4));
+  if (n_cfg > 0) KS_CUDA(c, cudaMemcpyAsync(dcfg, cfg_off, (size_t)(n_cfg + 1) * 4, cudaMemcpyHostToDevice, c->h2d));
+  KS_CUDA(c, cudaEventRecord(c->ev_start, c->h2d));
+  float* dstep = static_cast<float*>(ws_take(c, (size_t)n_steps * n_specs * 4));
+  float* dtot = static_cast<float*>(ws_take(c, (size_t)n_cfg * n_specs * 4 + 4));
+  for (int b = 0; b < n_batches; ++b) {
+    KS_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[b], 0));
+    if (n_specs > 0 && batches[b].n > 0) {
+      st = predict_device(c, batches + b, cols + b, 1, specs, n_specs, tier, outs + b);
+      if (st != KS_OK) return st;
+    }
+    const size_t ob = (size_t)batches[b].n * n_specs * 4;
+    if (latency && latency[b] && ob) {
+      KS_CUDA(c, cudaEventRecord(c->ev_out[b], c->stream));
+      KS_CUDA(c, cudaStreamWaitEvent(c->d2h, c->ev_out[b], 0));
+      KS_CUDA(c, cudaMemcpyAsync(latency[b], outs[b].lat, ob, cudaMemcpyDeviceToHost, c->d2h));
+    }
   }
-  if (n_specs > 0 && n_batches > 0) {
-    st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
-    if (st != KS_OK) return st;
-  }
+  KS_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_start, 0));     // cfg offsets (and every earlier h2d copy)
   st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot);
   if (st != KS_OK) return st;
-  if (!dev) {
-    for (int b = 0; b < n_batches; ++b) {
-      const size_t ob = (size_t)batches[b].n * n_specs * 4;
-      if (latency && latency[b] && ob)
-        KS_CUDA(c, cudaMemcpyAsync(latency[b], outs[b].lat, ob, cudaMemcpyDeviceToHost, c->stream));
-    }
-    if ((size_t)n_steps * n_specs)
-      KS_CUDA(c, cudaMemcpyAsync(step_latency, dstep, (size_t)n_steps * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
-    if ((size_t)n_cfg * n_specs)
-      KS_CUDA(c, cudaMemcpyAsync(cfg_latency, dtot, (size_t)n_cfg * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
-    KS_CUDA(c, cudaStreamSynchronize(c->stream));
-  }
+  if ((size_t)n_steps * n_specs)
+    KS_CUDA(c, cudaMemcpyAsync(step_latency, dstep, (size_t)n_steps * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
+  if ((size_t)n_cfg * n_specs)
+    KS_CUDA(c, cudaMemcpyAsync(cfg_latency, dtot, (size_t)n_cfg * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
+  KS_CUDA(c, cudaStreamSynchronize(c->stream));
+  KS_CUDA(c, cudaStreamSynchronize(c->d2h));
   return KS_OK;
 }
 
