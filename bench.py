@@ -413,6 +413,13 @@ def run_ours(args):
                     frac=achieved / peaks["bf16"], traffic=traffic, peak_source=f"bf16 burst, {peaks['source']}",
                     flops_per_prediction=FLOPS_PER_PRED[(head.n_in, head.h1)], kernel_ms=mlp_ms,
                     compose_ms=float(ms[:, 1].mean()), share_of_step=float(ms[:, 0].sum() / ms.sum()))
+    # the binding unit of the Tier-A kernel is the MUFU pipe (2H tanh per prediction, 16 lanes/clk/SM):
+    # peak = 16 x SMs x max SM clock
+    tanh_per_s = 2 * head.h1 * w.n_rows / (mlp_ms * 1e-3)
+    mufu_peak = 16 * torch.cuda.get_device_properties(local).multi_processor_count * (clocks.get("sm_max_mhz") or 1965) * 1e6
+    roofline_alu = dict(bound="alu", kernel=roofline["kernel"], achieved=tanh_per_s / 1e12, peak=mufu_peak / 1e12,
+                        unit="Ttanh/s", frac=tanh_per_s / mufu_peak,
+                        note="MUFU.TANH evaluations; peak = 16 lanes/clk/SM x SMs x max SM clock")
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=Wm,
                 ms_per_step=1e3 * total_s / K, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="bf16", data="synthetic",
@@ -421,7 +428,8 @@ def run_ours(args):
                             tier="A", n_steps=w.n_steps, n_cfg=n_cfg, rows_per_gpu=w.n_rows,
                             l2="flushed before every step (256 MiB write, outside the event pairs)",
                             timing="CUDA events on the ctx stream around predict and compose of every step"),
-                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, wall_s_timed_region=t_wall)
+                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, roofline_alu=roofline_alu,
+                wall_s_timed_region=t_wall)
     if world == 1:
         if not args.no_extras:
             line["extras"] = run_extras(h, peaks)

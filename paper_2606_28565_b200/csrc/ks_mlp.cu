@@ -1,21 +1,22 @@
-// ks_mlp.cu — Tier-A kernel: descriptor decode -> roofline -> features -> per-family MLP head on the
-// 5th-gen tensor cores (tcgen05.mma, bf16 x bf16 -> fp32 in TMEM) -> sigmoid -> latency, fused.
-// S1-S3, S4a, S5 of DESIGN.md §1.  PAPER.md:191 Eq. 2, :199-201 (per-family heads).
+// ks_mlp.cu — Tier-A kernel for H = 256 (cfg5): descriptor decode -> roofline -> features ->
+// per-family MLP head on the 5th-gen tensor cores (tcgen05.mma, bf16 x bf16 -> fp32 in TMEM) ->
+// sigmoid -> latency, fused.  S1-S3, S4a, S5 of DESIGN.md §1.  PAPER.md:191 Eq. 2, :199-201.
+// (H <= 128 runs the warp-specialized pipeline in ks_mlp_ws.cu; ks_launch_mlp dispatches.)
 //
-// One persistent CTA per SM.  A CTA holds one family's weights in shared memory (staged by 1-D TMA
-// bulk copies as pre-built UMMA operand images) and walks a contiguous range of 128-row tiles; it
-// reloads weights when its range crosses into the next family bucket.
-//
-// A "slot" = 128 descriptor rows = the 128 TMEM lanes, served by two warpgroups (256 threads) that
-// split the hidden columns in halves.  Per (tile, spec):
+// One persistent CTA per SM holds one family's weights in shared memory (staged by 1-D TMA bulk
+// copies as pre-built UMMA operand images) and walks a contiguous range of 128-row tiles; it
+// reloads weights when its range crosses into the next family bucket.  The W2 image of H = 256 is
+// 136 KiB, so a single A2 buffer fits: one "slot" (128 rows = the 128 TMEM lanes) served by two
+// warpgroups that split the hidden columns in halves.  Per (tile, spec):
 //   WG0: decode + features -> bf16 A1 operand in smem        (A1 aliases the first K chunks of A2)
 //   MMA1  D1[128 x H] = A1[128 x K1] . W1                    (bias b1 rides on two constant-1 feature columns)
-//   epi1  D1 -> regs (tcgen05.ld) -> GELU -> bf16 -> A2 smem, in 32-column chunks; after every chunk
+//   epi1  D1 -> regs (tcgen05.ld) -> 2 GELU -> bf16 -> A2 smem, in 32-column chunks; after every chunk
 //         the finished K range of MMA2 is issued, so layer 2 runs on the tensor core while the
 //         ALUs are still activating the rest of layer 1
-//   MMA2  D2[128 x H] = A2[128 x H] . W2  (+ one K=16 step: ones-block x {b2_hi, b2_lo})
-//   epi2  D2 -> regs -> GELU -> dot with w3 (fp32) -> z -> e = sigmoid(z) -> t = max(t_roof / e, t0)
-// Two slots per CTA (H <= 128) overlap one slot's MMA waits with the other slot's ALU work.
+//   MMA2  D2[128 x H] = A2[128 x H] . W2/2  (+ one K=16 step: ones-block x {b2_hi, b2_lo})
+//   epi2  D2 -> regs -> 2 GELU -> dot with w3/2 (fp32) -> z -> e = sigmoid(z) -> t = max(t_roof / e, t0)
+// (The Cfg template also describes a four-slot layout with D2 aliasing D1 for H <= 128; it is kept
+// compiled-out as the measured predecessor of the warp-specialized kernel: 115 us vs 100 us on cfg2.)
 //
 // Operand layout (both A and B): K-major, no swizzle: [K/8][rows][8] bf16, i.e. each 8-row x 16-byte
 // core matrix is 128 contiguous bytes; SBO = 128 B, LBO = rows * 16 B.  A thread owns one row, so a

@@ -4,25 +4,27 @@
 // One persistent CTA per SM walks a contiguous range of 128-row tiles.  A work item q is one
 // (tile, spec) pair; item q uses buffer q & 1 of every double-buffered resource.
 //
-//   warps 0-3   PRODUCER  thread r owns row r: prefetch next tile's columns, decode + roofline +
-//                         features -> bf16 A1[q&1] row in smem (K-major UMMA image), t_roof -> ring
-//   warp  12    MMA       one thread: MMA1(q): D1[q&1] = A1[q&1] . W1      (b1 rides on two 1-columns)
-//                                     MMA2(q-1): D2 = A2 . W2 (+ ones-block x b2 step)
-//   warps 4-7   EPI1      D1[q&1] -> regs (tcgen05.ld, double-buffered) -> 2 GELU -> bf16 -> A2[q&1]
-//   warps 8-11  EPI2      D2[q&1] -> regs -> 2 GELU -> fp32 dot with w3/2 -> sigmoid -> latency
+//   warps 0-3    PRODUCER  thread r owns row r: prefetch next tile's columns, decode + roofline +
+//                          features -> bf16 A1[q&1] row in smem (K-major UMMA image), t_roof -> ring
+//   warp  20     MMA       one thread: MMA1(q+2): D1 = A1 . W1 (b1 rides on two 1-columns) as soon as
+//                          EPI1 has drained D1[q&1]; then MMA2(q): D2 = A2 . W2 (+ ones-block x b2 step)
+//   warps 4-11   EPI1      two warpgroups, group g owns buffer g: D1 -> regs (tcgen05.ld, 16 columns,
+//                          double-buffered) -> 2 GELU -> bf16 -> A2[g] in smem
+//   warps 12-19  EPI2      same split: D2 -> regs -> 2 GELU -> fp32 dot with w3/2 -> sigmoid -> latency
 //
 // so the tensor core, the activation warps of layer 1 and of layer 2 and the feature warps all work
 // on different items at the same time; nobody waits for its own MMA.  Synchronisation is by
 // mbarriers only (no CTA-wide barrier in the loop):
 //   a1_full[2]   128 producer arrivals      -> MMA may read A1[b]
 //   mma1_done[2] tcgen05.commit             -> EPI1 may read D1[b]; producer may rewrite A1[b]
-//   a2_full[2]   128 EPI1 arrivals          -> MMA may read A2[b]; D1[b] has been drained
+//   d1_free[2]   128 EPI1 arrivals          -> D1[b] has been drained: MMA1(q+2) may overwrite it
+//   a2_full[2]   128 EPI1 arrivals          -> MMA may read A2[b]
 //   mma2_done[2] tcgen05.commit             -> EPI2 may read D2[b]; EPI1 may rewrite A2[b]
 //   d2_free[2]   128 EPI2 arrivals          -> MMA may overwrite D2[b]
 // A waiter for completion k of a barrier always runs before completion k+1 can happen (k+1 depends
 // on the waiter's own progress), so single-bit phase parity is sufficient.
-// The t_roof ring has 8 entries: the producer can be at most 5 items ahead of EPI2 (item q+6 needs
-// mma1_done(q+4), MMA1(q+4) is issued after MMA2(q+2), which waits for d2_free(q)).
+// The t_roof ring has 8 entries: the producer can be at most 7 items ahead of EPI2 (item q+8 needs
+// mma1_done(q+6); MMA1(q+6) is issued after MMA2(q+3), which waits for d2_free(q+1) >= d2_free(q)).
 #include "ks_mlp_common.cuh"
 
 namespace {
@@ -125,7 +127,7 @@ KS_DEV void producer_bucket(const KsMlpParams& p, const int b, const Range tr, u
   }
 }
 
-// ------------------------------------------------------------------ EPI1 (warps 4-7): D1 -> 2 GELU -> A2
+// ------------------------------------------------------------------ EPI1 (warps 4-11): D1 -> 2 GELU -> A2
 template <int NIN, int H, int GM>
 KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned char* smem, uint64_t* bars,
                        const uint32_t tmem_base) {
@@ -178,7 +180,7 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
   }
 }
 
-// ------------------------------------------------------------------ EPI2 (warps 8-11): D2 -> 2 GELU . w3/2 -> latency
+// ------------------------------------------------------------------ EPI2 (warps 12-19): D2 -> 2 GELU . w3/2 -> latency
 template <int NIN, int H, int GM>
 KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
                      const uint32_t tmem_base) {
@@ -253,7 +255,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsig
   }
 }
 
-// ------------------------------------------------------------------ MMA issuer (one thread of warp 12)
+// ------------------------------------------------------------------ MMA issuer (one thread of warp 20)
 template <int NIN, int H>
 KS_DEV void mma_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
                     const uint32_t tmem_base) {
