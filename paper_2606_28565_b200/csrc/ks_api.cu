@@ -20,6 +20,7 @@ struct HeadState {
   void* w1_img = nullptr;
   void* w2_img = nullptr;
   float* w3 = nullptr;
+  float* b2 = nullptr;
   float b3 = 0.0f;
 };
 
@@ -249,6 +250,7 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
           p.head[nb].w1_img = hq.w1_img;
           p.head[nb].w2_img = hq.w2_img;
           p.head[nb].w3 = hq.w3;
+          p.head[nb].b2 = hq.b2;
           p.head[nb].b3 = hq.b3;
           p.tile_begin[nb] = tiles;
           tiles += (batches[q].n + 127) / 128;
@@ -311,6 +313,7 @@ ks_status ks_destroy(ks_ctx* c) {
     cudaFree(c->heads[f].w1_img);
     cudaFree(c->heads[f].w2_img);
     cudaFree(c->heads[f].w3);
+    cudaFree(c->heads[f].b2);
     cudaFree(c->grids[f].values);
   }
   cudaFree(c->ws);
@@ -369,15 +372,16 @@ ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, c
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read the old head
   HeadState& hs = c->heads[family];
-  cudaFree(hs.w1_img); cudaFree(hs.w2_img); cudaFree(hs.w3);
+  cudaFree(hs.w1_img); cudaFree(hs.w2_img); cudaFree(hs.w3); cudaFree(hs.b2);
   hs = HeadState();
-  void *d1 = nullptr, *d2 = nullptr, *d3 = nullptr;
+  void *d1 = nullptr, *d2 = nullptr, *d3 = nullptr, *d4 = nullptr;
   if (cudaMalloc(&d1, i1.size() * 2) != cudaSuccess || cudaMalloc(&d2, i2.size() * 2) != cudaSuccess ||
-      cudaMalloc(&d3, (size_t)H * 4) != cudaSuccess) {
+      cudaMalloc(&d3, (size_t)H * 4) != cudaSuccess || cudaMalloc(&d4, (size_t)H * 4) != cudaSuccess) {
     cudaGetLastError();
-    cudaFree(d1); cudaFree(d2); cudaFree(d3);
+    cudaFree(d1); cudaFree(d2); cudaFree(d3); cudaFree(d4);
     return KS_ENOMEM;
   }
+  KS_CUDA(c, cudaMemcpy(d4, b2, (size_t)H * 4, cudaMemcpyHostToDevice));
   KS_CUDA(c, cudaMemcpy(d1, i1.data(), i1.size() * 2, cudaMemcpyHostToDevice));
   KS_CUDA(c, cudaMemcpy(d2, i2.data(), i2.size() * 2, cudaMemcpyHostToDevice));
   KS_CUDA(c, cudaMemcpy(d3, w3r.data(), (size_t)H * 4, cudaMemcpyHostToDevice));
@@ -387,6 +391,7 @@ ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, c
   hs.w1_img = d1;
   hs.w2_img = d2;
   hs.w3 = static_cast<float*>(d3);
+  hs.b2 = static_cast<float*>(d4);
   hs.b3 = b3;
   return KS_OK;
 }

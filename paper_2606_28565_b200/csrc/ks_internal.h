@@ -22,7 +22,8 @@ cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t 
 struct KsHeadDev {
   const void* w1_img;      // bf16 UMMA image [K1/8][H][8]  (rows n_in, n_in+1 hold b1 hi/lo)
   const void* w2_img;      // bf16 UMMA image [(H+16)/8][H][8] (K rows H, H+1 hold b2 hi/lo)
-  const float* w3;         // fp32 [H]
+  const float* w3;         // fp32 [H], holds w3 / 2
+  const float* b2;         // fp32 [H] (the H = 256 kernel adds b2 in its fp32 epilogue)
   float b3;
   int32_t pad;
 };
@@ -36,6 +37,7 @@ struct KsMlpParams {
 // n_in in {8,12,32}; h in {64,128,256}; all buckets of one launch share (n_in, h)
 cudaError_t ks_launch_mlp(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st);
 cudaError_t ks_launch_mlp_ws(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st);   // h <= 128
+cudaError_t ks_launch_mlp_ws256(const KsMlpParams& p, int n_in, int num_sms, cudaStream_t st);            // h == 256
 // sizes of the device weight images for a head
 size_t ks_mlp_w1_img_bytes(int n_in, int h);
 size_t ks_mlp_w2_img_bytes(int h);

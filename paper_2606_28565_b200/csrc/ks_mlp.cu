@@ -367,6 +367,7 @@ cudaError_t ks_launch_mlp(const KsMlpParams& p, int n_in, int h, int num_sms, cu
 #define KS_CASE(NI, HH) \
   if (n_in == NI && h == HH) return launch<NI, HH>(p, num_sms, st);
   if (h <= 128) return ks_launch_mlp_ws(p, n_in, h, num_sms, st);   // warp-specialized pipeline (ks_mlp_ws.cu)
+  if (h == 256 && p.gelu_mode < 2) return ks_launch_mlp_ws256(p, n_in, num_sms, st);   // ks_mlp_ws256.cu
   KS_CASE(8, 256) KS_CASE(12, 256) KS_CASE(32, 256)
 #undef KS_CASE
   return cudaErrorInvalidValue;
