@@ -1,118 +1,167 @@
 // ks_compose.cu — S6/S7: segmented reduction of kernel latencies into per-step GPU bodies
 // (PAPER.md:231), the host-overlap step formula (Eq. 4) and per-configuration totals.
 //
-// ks_compose_kernel: persistent warps, one PAIR of consecutive steps per warp and trip (rows of a
-// bucket are step-sorted, so the pair is one contiguous range of every bucket's latency array).
-// One load fetches all CSR bounds of the pair (lane 3b+i), and the bounds of the warp's NEXT pair
-// are requested before the current one is summed, so the only exposed memory round trip per trip
-// is the latency data itself.  Per bucket and step the lanes read consecutive elements: five
-// streaming loads (at clamped addresses, masked afterwards) cover segments up to 160 kernels, and
-// the loads of every bucket are issued before the first add; longer segments stream the rest.  One fixed-order shuffle tree
-// per step, Eq. 4 epilogue.  No atomics: bit-reproducible.
-// Measured alternatives (profiles/README.md): staging chunks of 16-32 steps through shared memory
-// with 1-D TMA bulk copies (2-4 stages, with and without a dedicated producer warp) or cp.async
-// sustains 2.4-3.6 TB/s chip-wide on this access pattern and was not faster.
+// ks_compose_kernel: one CTA per chunk of 32 consecutive steps (rows of a bucket are step-sorted, so
+// a chunk is one contiguous range of every bucket's latency array).  The CTA reads the chunk's CSR
+// bounds, then stages every bucket's range into shared memory with 16-byte cp.async copies (fire
+// and forget: ~38 KB in flight per CTA, four CTAs per SM, no registers tied up), and its eight warps
+// sum two steps at a time out of shared memory: per bucket the lanes read consecutive elements
+// (conflict-free LDS with immediate offsets), ten loads per step pair issued before the first add,
+// masked afterwards; one fixed-order shuffle tree per step; Eq. 4 epilogue.  No atomics:
+// bit-reproducible.  A chunk that does not fit the buffer (very long steps) is summed straight
+// from global memory by the same loop.
+// Measured alternatives (profiles/README.md): persistent CTAs with 1-D TMA bulk copies (2-4 stages,
+// with and without a producer warp), persistent cp.async double buffering, and persistent warps
+// reading global memory directly were all slower (34-60 us against 31 us on cfg4a).
 // Config totals: one CTA per (spec, config), fp64 accumulation.
 #include "ks_internal.h"
+#include "ks_ptx.cuh"
+
+#include <type_traits>
 
 namespace {
 
 constexpr int kWarps = 8;
 constexpr int kThreads = kWarps * 32;
 
+constexpr int kS = 32;                 // steps per chunk (one CTA)
+constexpr int kCapFloats = 12032;      // staged floats per CTA (47 KiB + slack): four CTAs per SM
+constexpr int kSlackFloats = 192;      // readable floats behind the staged data (masked lanes of the last step)
+
 // this lane's share of src[0, n) beyond the first 160 elements (rare: very long steps)
 KS_DEV float lane_tail(const float* __restrict__ src, int n, int lane) {
   float a0 = 0.0f, a1 = 0.0f;
   int k = lane + 160;
 #pragma unroll 1
-  for (; k + 32 < n; k += 64) { a0 += __ldcs(src + k); a1 += __ldcs(src + k + 32); }
-  if (k < n) a0 += __ldcs(src + k);
+  for (; k + 32 < n; k += 64) { a0 += src[k]; a1 += src[k + 32]; }
+  if (k < n) a0 += src[k];
   return a0 + a1;
 }
 
-// NB = compile-time bound on the bucket count (1-4: exact, or 8): the bucket loop is fully unrolled so the
-// loads of every bucket are in flight before the first add
+// NB = compile-time bound on the bucket count (1-4: exact, or 8)
 template <int NB>
-__global__ void __launch_bounds__(kThreads, NB <= 4 ? 4 : 2)
+__global__ void __launch_bounds__(kThreads, 4)
 ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
-  const int lane = threadIdx.x & 31;
-  const unsigned wid = blockIdx.x * kWarps + (threadIdx.x >> 5), n_warps = gridDim.x * kWarps;
-  const unsigned pps = (unsigned)(p.n_steps + 1) / 2u;             // step pairs per spec
-  const unsigned n_pairs = pps * (unsigned)p.n_specs;              // < 2^31 (checked by the launcher)
+  extern __shared__ __align__(128) float sdata[];
+  __shared__ int offs[NB][kS + 1];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const unsigned cps = (unsigned)(p.n_steps + kS - 1) / kS;        // chunks per spec
+  const unsigned spec = blockIdx.x / cps;
+  const int s0 = (int)(blockIdx.x - spec * cps) * kS;
+  const int ns = p.n_steps - s0 < kS ? p.n_steps - s0 : kS;
 
-  // CSR offsets of pair q: lane 3b + i holds step_off[b][2c + i], i = 0..2 (clamped to n_steps)
-  auto load_offs = [&](unsigned q) -> int {
-    if (q >= n_pairs || lane >= 3 * p.n_batches) return 0;
-    const int b = lane / 3, i = lane - 3 * b;
-    const int s = 2 * (int)(q % pps) + i;
-    return __ldg(p.step_off[b] + (s < p.n_steps ? s : p.n_steps));
-  };
-
-  int offv = load_offs(wid);
-  for (unsigned q = wid; q < n_pairs; q += n_warps) {
-    const int offn = load_offs(q + n_warps);        // next pair's offsets: in flight under this pair's sums
-    const unsigned spec = q / pps;
-    const int sA = 2 * (int)(q - spec * pps);
-    const bool hasB = sA + 1 < p.n_steps;
-    float x[NB][5], y[NB][5];
-    int nA[NB], nB[NB];
-#pragma unroll
-    for (int b = 0; b < NB; ++b) {
-      const int beg = __shfl_sync(0xffffffffu, offv, 3 * b);
-      const int mid = __shfl_sync(0xffffffffu, offv, 3 * b + 1);
-      const int end = __shfl_sync(0xffffffffu, offv, 3 * b + 2);
-      const bool on = b < p.n_batches;
-      nA[b] = on ? mid - beg : 0;
-      nB[b] = on ? end - mid : 0;
-      // unconditional loads at clamped (always valid) addresses; out-of-segment lanes are masked
-      // after ALL loads have been issued, so nothing waits on a load in between
-      const float* __restrict__ a = nA[b] > 0 ? p.lat[b] + ((long long)spec * p.spec_stride[b] + beg) : p.step_lat;
-      const float* __restrict__ c = nB[b] > 0 ? p.lat[b] + ((long long)spec * p.spec_stride[b] + mid) : p.step_lat;
-      const int lastA = nA[b] > 0 ? nA[b] - 1 : 0, lastB = nB[b] > 0 ? nB[b] - 1 : 0;
-#pragma unroll
-      for (int r = 0; r < 5; ++r) {
-        x[b][r] = __ldcs(a + min(lane + 32 * r, lastA));
-        y[b][r] = __ldcs(c + min(lane + 32 * r, lastB));
-      }
-    }
-#pragma unroll
-    for (int b = 0; b < NB; ++b) {
-#pragma unroll
-      for (int r = 0; r < 5; ++r) {
-        x[b][r] = lane + 32 * r < nA[b] ? x[b][r] : 0.0f;
-        y[b][r] = lane + 32 * r < nB[b] ? y[b][r] : 0.0f;
-      }
-    }
-    float accA = 0.0f, accB = 0.0f;
-    int cntA = 0, cntB = 0;
-#pragma unroll
-    for (int b = 0; b < NB; ++b) {
-      accA += ((x[b][0] + x[b][1]) + (x[b][2] + x[b][3])) + x[b][4];
-      accB += ((y[b][0] + y[b][1]) + (y[b][2] + y[b][3])) + y[b][4];
-      cntA += nA[b];
-      cntB += nB[b];
-      if (nA[b] > 160 || nB[b] > 160) {             // warp-uniform: long steps stream the rest
-        const int beg = __shfl_sync(0xffffffffu, offv, 3 * b);
-        const float* __restrict__ a = p.lat[b] + ((long long)spec * p.spec_stride[b] + beg);
-        if (nA[b] > 160) accA += lane_tail(a, nA[b], lane);
-        if (nB[b] > 160) accB += lane_tail(a + nA[b], nB[b], lane);
-      }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      accA += __shfl_xor_sync(0xffffffffu, accA, o);
-      accB += __shfl_xor_sync(0xffffffffu, accB, o);
-    }
-    if (lane < 2 && (lane == 0 || hasB)) {
-      const float t_gpu = p.sp.body_scale * (lane == 0 ? accA : accB);
-      const int count = lane == 0 ? cntA : cntB;
-      // Eq. 4: t_step = max(t_gpu + n c_disp, l) + max(0, c_ovl - t_gpu) + c_tail
-      const float t = fmaxf(fmaf((float)count, p.sp.c_disp, t_gpu), p.sp.floor_l) +
-                      fmaxf(0.0f, p.sp.c_ovl - t_gpu) + p.sp.c_tail;
-      p.step_lat[(long long)spec * p.n_steps + sA + lane] = t;
-    }
-    offv = offn;
+  for (int idx = tid; idx < p.n_batches * (kS + 1); idx += kThreads) {
+    const int b = idx / (kS + 1), j = idx - b * (kS + 1);
+    offs[b][j] = __ldg(p.step_off[b] + (s0 + j < p.n_steps ? s0 + j : p.n_steps));
   }
+  __syncthreads();
+
+  // The chunk's kernels are one contiguous range per bucket: stage all of them with 16-byte
+  // cp.async copies (fire and forget: ~38 KB in flight per CTA, four CTAs per SM).
+  int sbase[NB], len[NB];
+  long long a0[NB];
+  int used = 0;
+  bool staged = true;
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    sbase[b] = 0; len[b] = 0; a0[b] = 0;
+    if (b < p.n_batches) {
+      const long long sb = (long long)spec * p.spec_stride[b];
+      a0[b] = (sb + offs[b][0]) & ~3ll;
+      long long a1 = (sb + offs[b][kS] + 3) & ~3ll;
+      const long long tot = ((long long)p.n_specs * p.spec_stride[b]) & ~3ll;
+      if (a1 > tot) a1 = tot;                                     // never read past the array end ...
+      if (a1 < sb + offs[b][kS]) staged = false;                  // ... (its last < 4 floats: global path)
+      len[b] = (int)(a1 - a0[b]);
+      sbase[b] = used + (int)(sb - a0[b]);
+      used += len[b];
+    }
+  }
+  if (used > kCapFloats) staged = false;                          // very long steps: straight from global
+  if (staged) {
+    int base = 0;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      if (b < p.n_batches) {
+        const float* __restrict__ src = p.lat[b] + a0[b];
+        for (int i = tid * 4; i < len[b]; i += kThreads * 4) ks_cp_async16(sdata + base + i, src + i);
+        base += len[b];
+      }
+    }
+    ks_cp_async_commit();
+    ks_cp_async_wait<0>();
+    __syncthreads();
+  }
+
+  // a warp sums two steps at a time (w and w + 8, then w + 16 and w + 24): per bucket ten independent
+  // predicated loads before the first add, one fixed-order shuffle tree per step.  Two copies of
+  // the loop so that the staged one uses 32-bit shared-memory addressing (LDS), not generic loads.
+  auto reduce_all = [&](auto staged_tag) {
+    constexpr bool STAGED = decltype(staged_tag)::value;
+#pragma unroll 1
+    for (int jA = warp; jA < ns; jA += 2 * kWarps) {
+      const int jB = jA + kWarps;
+      const bool hasB = jB < ns;
+      float accA = 0.0f, accB = 0.0f;
+      int cntA = 0, cntB = 0;
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        if (b < p.n_batches) {
+          const int begA = offs[b][jA], nA = offs[b][jA + 1] - begA;
+          const int begB = hasB ? offs[b][jB] : begA, nB = hasB ? offs[b][jB + 1] - begB : 0;
+          const float* __restrict__ sA;
+          const float* __restrict__ sB;
+          if (STAGED) {
+            sA = sdata + (sbase[b] + begA + lane);
+            sB = sdata + (sbase[b] + begB + lane);
+          } else {
+            const float* base = p.lat[b] + (long long)spec * p.spec_stride[b];
+            sA = base + begA + lane;
+            sB = base + begB + lane;
+          }
+          const int mA = nA - lane, mB = nB - lane;                // this lane owns elements 32 r < m
+          float x0, x1, x2, x3, x4, y0, y1, y2, y3, y4;
+          if (STAGED) {
+            // unconditional LDS with immediate offsets (the buffer has 160 floats of slack behind the
+            // staged data, so every address is valid), masked after all ten loads are issued
+            x0 = sA[0]; x1 = sA[32]; x2 = sA[64]; x3 = sA[96]; x4 = sA[128];
+            y0 = sB[0]; y1 = sB[32]; y2 = sB[64]; y3 = sB[96]; y4 = sB[128];
+            x0 = 0 < mA ? x0 : 0.0f; x1 = 32 < mA ? x1 : 0.0f; x2 = 64 < mA ? x2 : 0.0f;
+            x3 = 96 < mA ? x3 : 0.0f; x4 = 128 < mA ? x4 : 0.0f;
+            y0 = 0 < mB ? y0 : 0.0f; y1 = 32 < mB ? y1 : 0.0f; y2 = 64 < mB ? y2 : 0.0f;
+            y3 = 96 < mB ? y3 : 0.0f; y4 = 128 < mB ? y4 : 0.0f;
+          } else {
+            x0 = 0 < mA ? sA[0] : 0.0f; y0 = 0 < mB ? sB[0] : 0.0f;
+            x1 = 32 < mA ? sA[32] : 0.0f; y1 = 32 < mB ? sB[32] : 0.0f;
+            x2 = 64 < mA ? sA[64] : 0.0f; y2 = 64 < mB ? sB[64] : 0.0f;
+            x3 = 96 < mA ? sA[96] : 0.0f; y3 = 96 < mB ? sB[96] : 0.0f;
+            x4 = 128 < mA ? sA[128] : 0.0f; y4 = 128 < mB ? sB[128] : 0.0f;
+          }
+          accA += ((x0 + x1) + (x2 + x3)) + x4;
+          accB += ((y0 + y1) + (y2 + y3)) + y4;
+          if (nA > 160) accA += lane_tail(sA - lane, nA, lane);
+          if (nB > 160) accB += lane_tail(sB - lane, nB, lane);
+          cntA += nA;
+          cntB += nB;
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        accA += __shfl_xor_sync(0xffffffffu, accA, o);
+        accB += __shfl_xor_sync(0xffffffffu, accB, o);
+      }
+      if (lane < 2 && (lane == 0 || hasB)) {
+        const float t_gpu = p.sp.body_scale * (lane == 0 ? accA : accB);
+        const int count = lane == 0 ? cntA : cntB;
+        // Eq. 4: t_step = max(t_gpu + n c_disp, l) + max(0, c_ovl - t_gpu) + c_tail
+        const float t = fmaxf(fmaf((float)count, p.sp.c_disp, t_gpu), p.sp.floor_l) +
+                        fmaxf(0.0f, p.sp.c_ovl - t_gpu) + p.sp.c_tail;
+        p.step_lat[(long long)spec * p.n_steps + s0 + (lane == 0 ? jA : jB)] = t;
+      }
+    }
+  };
+  if (staged) reduce_all(std::true_type{});
+  else reduce_all(std::false_type{});
 }
 
 __global__ void __launch_bounds__(256)
@@ -138,19 +187,17 @@ ks_cfg_total_kernel(const __grid_constant__ KsComposeParams p) {
 }  // namespace
 
 cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_t st, int* launches) {
+  (void)num_sms;
   const long long total = (long long)p.n_specs * p.n_steps;
   if (total > 0) {
-    const long long n_pairs = (long long)((p.n_steps + 1) / 2) * p.n_specs;
+    const long long n_chunks = (long long)((p.n_steps + kS - 1) / kS) * p.n_specs;
+    if (n_chunks > 0x7fffffffll) return cudaErrorInvalidValue;
     auto kern = p.n_batches <= 1 ? ks_compose_kernel<1> : p.n_batches == 2 ? ks_compose_kernel<2> :
                 p.n_batches == 3 ? ks_compose_kernel<3> : p.n_batches == 4 ? ks_compose_kernel<4> : ks_compose_kernel<8>;
-    int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, 0);
+    const size_t smem = (size_t)(kCapFloats + kSlackFloats) * 4;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    long long blocks = (long long)num_sms * (per_sm > 0 ? per_sm : 1);   // persistent: exactly one resident wave
-    const long long need = (n_pairs + kWarps - 1) / kWarps;
-    if (blocks > need) blocks = need;
-    if (n_pairs + blocks * kWarps > 0x7fffffffll) return cudaErrorInvalidValue;
-    kern<<<(unsigned)blocks, kThreads, 0, st>>>(p);
+    kern<<<(unsigned)n_chunks, kThreads, smem, st>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (launches) *launches += 1;

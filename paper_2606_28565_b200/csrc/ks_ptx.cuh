@@ -47,6 +47,20 @@ KS_PTX void ks_mbar_wait_backoff(uint64_t* bar, uint32_t parity) {
     if (!done) __nanosleep(40);
   } while (!done);
 }
+// non-blocking: has the phase with this parity completed?
+KS_PTX bool ks_mbar_test(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}"
+      : "=r"(done)
+      : "r"(ks_smem_u32(bar)), "r"(parity)
+      : "memory");
+  return done != 0u;
+}
 KS_PTX void ks_mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ks_smem_u32(bar)) : "memory");
 }
