@@ -46,7 +46,8 @@ extern "C" {
 typedef struct ks_ctx ks_ctx;   /* opaque; owns device copies of heads and grids + workspace */
 
 typedef enum { KS_OK = 0, KS_EINVAL = 1, KS_ENOMEM = 2, KS_ECUDA = 3, KS_ESTATE = 4, KS_EUNSUPPORTED = 5 } ks_status;
-typedef enum { KS_FAM_GEMM = 0, KS_FAM_GROUPED_GEMM = 1, KS_FAM_ATTN = 2, KS_FAM_ELEMWISE = 3, KS_FAM_COUNT = 4 } ks_family;
+typedef enum { KS_FAM_GEMM = 0, KS_FAM_GROUPED_GEMM = 1, KS_FAM_ATTN = 2, KS_FAM_ELEMWISE = 3, KS_FAM_ALLREDUCE = 4,
+               KS_FAM_COUNT = 5 } ks_family;
 typedef enum { KS_TIER_NONE = 0, KS_TIER_A = 1, KS_TIER_B = 2 } ks_tier;
 typedef enum { KS_COL_I32 = 0, KS_COL_F32 = 1 } ks_col_dtype;   /* F32 columns must hold exact integers < 2^24 */
 typedef enum { KS_MEM_DEVICE = 0, KS_MEM_HOST = 1 } ks_mem_space;
@@ -65,6 +66,8 @@ typedef struct {
   int32_t n_sm, ctas_per_sm, tile_m, tile_n, ew_elems_per_cta;
   float l2_bytes;          /* L2 capacity in bytes */
   float t0;                /* launch floor, seconds (>= 0) */
+  float ar_alpha0;         /* interconnect: all-reduce startup/synchronisation term, seconds (>= 0) */
+  float ar_beta_eff;       /* interconnect: effective bandwidth, bytes/s (> 0); Eq. 3 */
 } ks_hw_spec;
 
 /* One family bucket of kernel-instance descriptors in SoA form.
@@ -75,6 +78,10 @@ typedef struct {
  *                        attn_hq / attn_hkv / attn_head_dim are per-bucket constants
  *   KS_FAM_ELEMWISE      cols = {n_elements, subop}     subop: 0 RMSNorm, 1 SiLU*Mul, 2 RoPE,
  *                        3 KV-cache write, 4 embedding, 5 residual add (out-of-range is clamped)
+ *   KS_FAM_ALLREDUCE     cols = {S_bytes, P}            tensor-parallel ring all-reduce of S bytes over P
+ *                        shards: t = ar_alpha0 + 2 (P-1)/P * S / ar_beta_eff (Eq. 3) under
+ *                        every tier (no roofline, no eta, no t0 floor; tiles = waves = 0, t_roof = t);
+ *                        it enters the step sum like a kernel
  * Each column has n elements of col_dtype; pointers live in the call's ks_mem_space. */
 typedef struct {
   int32_t family;          /* ks_family */
@@ -119,7 +126,8 @@ KS_API ks_status ks_load_grid(ks_ctx *ctx, ks_family family, const int32_t dims[
  *   tiles[b], waves[b]   optional out (array pointer or entry may be NULL), int32 [n_specs][n]:
  *                        CTA count B and wave count W = ceil(B/S)
  *   t_roof[b]            optional out, fp32 [n_specs][n]
- * KS_ESTATE if the tier needs a head/grid that was not loaded for a bucket's family. */
+ * KS_ESTATE if the tier needs a head/grid that was not loaded for a bucket's family
+ * (KS_FAM_ALLREDUCE needs neither). */
 KS_API ks_status ks_predict_kernels(ks_ctx *ctx, const ks_desc_batch *batches, int n_batches,
                              const ks_hw_spec *specs, int n_specs, ks_tier tier, ks_mem_space space,
                              float *const *latency, int32_t *const *tiles, int32_t *const *waves,

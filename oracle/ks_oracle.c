@@ -252,9 +252,23 @@ double kso_trilinear(const kso_grid *g, const double v[3]) {
 
 /* ---------------------------------------------------------------- S5: one prediction
  * PAPER.md:191 Eq. 2: t = max(t_roof * eta, t0); eta = 1/e (Q3). */
+/* PAPER.md:219 Eq. 3 */
+double kso_allreduce(int64_t S, int64_t P, const kso_spec *hw) {
+  if (S < 0) S = 0;
+  if (P <= 1) return hw->ar_alpha0;
+  return hw->ar_alpha0 + 2.0 * (double)(P - 1) / (double)P * ((double)S / hw->ar_beta_eff);
+}
+
 double kso_predict_one(const kso_desc *d, const kso_spec *hw, int tier, const kso_head *h,
                        const kso_grid *g, kso_roof *rout, double *e_out) {
   kso_roof r;
+  if (d->family == KSO_ALLREDUCE) {   /* a communication row: Eq. 3 as it stands, for every tier */
+    const double t = kso_allreduce(d->v[0], d->v[1], hw);
+    r.F = 0.0; r.Y = 0.0; r.B = 0; r.W = 0; r.u = 1.0; r.t_comp = 0.0; r.t_mem = 0.0; r.t_roof = t;
+    if (rout) *rout = r;
+    if (e_out) *e_out = 1.0;
+    return t;
+  }
   kso_roofline(d, hw, &r);
   double e = 1.0;
   if (tier == KSO_TIER_A) {
@@ -278,8 +292,8 @@ int kso_predict_batch(int family, int64_t n, const double *const *cols, int n_co
                       int tier, const kso_head *h, const kso_grid *g, double *lat, int64_t *tiles,
                       int64_t *waves, double *troof) {
   if (n < 0 || n_cols < 0 || n_cols > KSO_MAX_COLS) return -1;
-  if (tier == KSO_TIER_A && !h) return -1;
-  if (tier == KSO_TIER_B && !g) return -1;
+  if (tier == KSO_TIER_A && !h && family != KSO_ALLREDUCE) return -1;
+  if (tier == KSO_TIER_B && !g && family != KSO_ALLREDUCE) return -1;
   for (int sp = 0; sp < n_specs; ++sp) {
     for (int64_t i = 0; i < n; ++i) {
       kso_desc d;

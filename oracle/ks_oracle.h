@@ -13,13 +13,14 @@
  *   t_roof                      (Eq. 2, right half)
  *   eta = 1/e  from Tier A head or Tier B grid
  *   t = max(t_roof*eta, t0)     (Eq. 2, left half; floor after eta PAPER.md:193)
+ *   t_ar (all-reduce rows)      (Eq. 3; enters the step sum like a kernel)
  *   t_gpu = body_scale*sum t
  *   t_step                      (Eq. 4)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Fig. 2's worked example, hand-computed
  * rooflines (tests/golden/roofline_cases.txt), brute-force wave/tile/pair counts,
  * numpy+scipy MLP, scipy RegularGridInterpolator, torch bf16 rounding, np.add.reduceat,
- * Eq. 4 regimes.  Parity unpinned: NONE of the functions below — but note the
+ * Eq. 4 regimes, Eq. 3 special cases (P = 1, P = 2, P -> inf, linearity in S, a hand-computed case).  Parity unpinned: NONE of the functions below — but note the
  * *feature list* (kso_features) is a reading (Q2): its closed-form special
  * cases are pinned, the paper prints no values for it.
  */
@@ -31,7 +32,7 @@
 extern "C" {
 #endif
 
-enum { KSO_GEMM = 0, KSO_GROUPED = 1, KSO_ATTN = 2, KSO_ELEMWISE = 3 };
+enum { KSO_GEMM = 0, KSO_GROUPED = 1, KSO_ATTN = 2, KSO_ELEMWISE = 3, KSO_ALLREDUCE = 4 };
 enum { KSO_TIER_NONE = 0, KSO_TIER_A = 1, KSO_TIER_B = 2 };
 #define KSO_MAX_COLS 10
 #define KSO_EXPERTS 8
@@ -40,11 +41,12 @@ typedef struct {           /* hardware-spec vector, PAPER.md:205 (+ tile/CTA fie
   double peak_flops, peak_bw;
   int64_t n_sm, ctas_per_sm, tile_m, tile_n, ew_elems_per_cta;
   double l2_bytes, t0;
+  double ar_alpha0, ar_beta_eff; /* interconnect: all-reduce startup [s] and effective bandwidth [B/s], Eq. 3 */
 } kso_spec;
 
 typedef struct {           /* one kernel-instance descriptor */
   int family;
-  int64_t v[KSO_MAX_COLS]; /* GEMM M,N,K | GROUPED N,K,m0..m7 | ATTN B,q,kv | ELEMWISE n,subop */
+  int64_t v[KSO_MAX_COLS]; /* GEMM M,N,K | GROUPED N,K,m0..m7 | ATTN B,q,kv | ELEMWISE n,subop | ALLREDUCE S,P */
   int64_t s;               /* bytes per element */
   int64_t hq, hkv, d;      /* attention constants */
 } kso_desc;
@@ -75,6 +77,9 @@ double kso_bf16(double x);
 double kso_gelu(double x);
 double kso_sigmoid(double z);
 
+/* Tensor-parallel ring all-reduce, Eq. 3: t_ar = alpha0 + 2 (P - 1) / P * S / beta_eff
+ * (S message bytes, P shards; P <= 1 moves nothing: t_ar = alpha0).  No roofline, no eta, no t0 floor. */
+double kso_allreduce(int64_t S, int64_t P, const kso_spec *hw);
 /* S1: F_comp, F_mem, B for one descriptor (Q1) */
 void kso_work(const kso_desc *d, const kso_spec *hw, double *F, double *Y, int64_t *B);
 /* causal (query, key) pair count of a q-token chunk over kv cached+own tokens */

@@ -34,7 +34,8 @@ def build(force: bool = False) -> str:
 class Spec(C.Structure):
     _fields_ = [("peak_flops", C.c_double), ("peak_bw", C.c_double), ("n_sm", C.c_int64),
                 ("ctas_per_sm", C.c_int64), ("tile_m", C.c_int64), ("tile_n", C.c_int64),
-                ("ew_elems_per_cta", C.c_int64), ("l2_bytes", C.c_double), ("t0", C.c_double)]
+                ("ew_elems_per_cta", C.c_int64), ("l2_bytes", C.c_double), ("t0", C.c_double),
+                ("ar_alpha0", C.c_double), ("ar_beta_eff", C.c_double)]
 
 
 class Desc(C.Structure):
@@ -77,6 +78,8 @@ def lib():
         L.kso_gelu.argtypes = [C.c_double]
         L.kso_sigmoid.restype = C.c_double
         L.kso_sigmoid.argtypes = [C.c_double]
+        L.kso_allreduce.restype = C.c_double
+        L.kso_allreduce.argtypes = [C.c_int64, C.c_int64, C.POINTER(Spec)]
         L.kso_attn_pairs.restype = C.c_int64
         L.kso_attn_pairs.argtypes = [C.c_int64, C.c_int64]
         L.kso_wave.restype = None
@@ -119,7 +122,7 @@ def _ip(a: np.ndarray):
 def make_spec(s: dict) -> Spec:
     return Spec(float(s["peak_flops"]), float(s["peak_bw"]), int(s["n_sm"]), int(s["ctas_per_sm"]),
                 int(s["tile_m"]), int(s["tile_n"]), int(s["ew_elems_per_cta"]), float(s["l2_bytes"]),
-                float(s["t0"]))
+                float(s["t0"]), float(s.get("ar_alpha0", 0.0)), float(s.get("ar_beta_eff", 1.0)))
 
 
 def make_desc(family: int, v: Sequence[int], s: int = 2, hq: int = 0, hkv: int = 0, d: int = 0) -> Desc:

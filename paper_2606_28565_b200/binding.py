@@ -34,7 +34,8 @@ class KsError(RuntimeError):
 class ks_hw_spec(C.Structure):
     _fields_ = [("peak_flops", C.c_float), ("peak_bw", C.c_float), ("n_sm", C.c_int32),
                 ("ctas_per_sm", C.c_int32), ("tile_m", C.c_int32), ("tile_n", C.c_int32),
-                ("ew_elems_per_cta", C.c_int32), ("l2_bytes", C.c_float), ("t0", C.c_float)]
+                ("ew_elems_per_cta", C.c_int32), ("l2_bytes", C.c_float), ("t0", C.c_float),
+                ("ar_alpha0", C.c_float), ("ar_beta_eff", C.c_float)]
 
 
 class ks_desc_batch(C.Structure):
@@ -113,7 +114,7 @@ def _ptr_array(items: Sequence) -> "C.Array":
 def make_spec(s: dict) -> ks_hw_spec:
     return ks_hw_spec(float(s["peak_flops"]), float(s["peak_bw"]), int(s["n_sm"]), int(s["ctas_per_sm"]),
                       int(s["tile_m"]), int(s["tile_n"]), int(s["ew_elems_per_cta"]), float(s["l2_bytes"]),
-                      float(s["t0"]))
+                      float(s["t0"]), float(s.get("ar_alpha0", 0.0)), float(s.get("ar_beta_eff", 1.0)))
 
 
 def make_batch(bucket) -> ks_desc_batch:

@@ -52,7 +52,7 @@ struct ks_ctx {
 
 namespace {
 
-const int kFamCols[KS_FAM_COUNT] = {3, 10, 3, 2};
+const int kFamCols[KS_FAM_COUNT] = {3, 10, 3, 2, 2};
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -136,6 +136,7 @@ bool spec_ok(const ks_hw_spec& s) {
   if (s.n_sm < 1 || s.ctas_per_sm < 1 || s.tile_m < 1 || s.tile_n < 1 || s.ew_elems_per_cta < 1) return false;
   if ((long long)s.n_sm * s.ctas_per_sm > 0x7fffffffll) return false;
   if (!(s.l2_bytes >= 0.0f) || !(s.t0 >= 0.0f) || !isfinite(s.t0)) return false;
+  if (!(s.ar_alpha0 >= 0.0f) || !isfinite(s.ar_alpha0) || !(s.ar_beta_eff > 0.0f) || !isfinite(s.ar_beta_eff)) return false;
   return true;
 }
 
@@ -154,6 +155,9 @@ KsSpecDev make_spec_dev(const ks_hw_spec& s) {
   d.tile_n = make_fastdiv((uint32_t)s.tile_n);
   d.ew = make_fastdiv((uint32_t)s.ew_elems_per_cta);
   d.slots = make_fastdiv(slots);
+  d.ar_alpha0 = s.ar_alpha0;
+  d.ar_inv_beta = (float)(1.0 / (double)s.ar_beta_eff);
+  d.pad0 = d.pad1 = 0.0f;
   return d;
 }
 
@@ -181,6 +185,7 @@ ks_status validate_batches(const ks_ctx* c, const ks_desc_batch* batches, int n_
         if (!k.cols[col]) return KS_EINVAL;
         if (device_ptrs && !aligned16(k.cols[col])) return KS_EINVAL;
       }
+    if (k.family == KS_FAM_ALLREDUCE) continue;               // Eq. 3 needs neither head nor grid
     if (tier == KS_TIER_A && !c->heads[k.family].loaded) return KS_ESTATE;
     if (tier == KS_TIER_B && !c->grids[k.family].loaded) return KS_ESTATE;
   }
@@ -219,31 +224,34 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
                          const ks_hw_spec* specs, int n_specs, int tier, const DevOut* outs) {
   for (int s0 = 0; s0 < n_specs; s0 += KS_MAX_SPECS_PER_LAUNCH) {
     const int ns = n_specs - s0 < KS_MAX_SPECS_PER_LAUNCH ? n_specs - s0 : KS_MAX_SPECS_PER_LAUNCH;
-    if (tier != KS_TIER_A) {
-      for (int b = 0; b < n_batches; ++b) {
-        if (batches[b].n == 0) continue;
+    for (int b = 0; b < n_batches; ++b) {               // streaming kernels: Tier NONE / B, and Eq. 3 rows under any tier
+      const bool ar = batches[b].family == KS_FAM_ALLREDUCE;
+      if (batches[b].n == 0 || (tier == KS_TIER_A && !ar)) continue;
+      {
         KsStreamParams p;
         memset(&p, 0, sizeof(p));
         p.bk = make_bucket_dev(batches[b], cols[b], outs[b], s0);
-        if (tier == KS_TIER_B) p.grid = c->grids[batches[b].family].dev;
+        if (tier == KS_TIER_B && !ar) p.grid = c->grids[batches[b].family].dev;
         p.n_specs = ns;
-        p.tier = tier;
+        p.tier = ar ? KS_TIER_NONE : tier;
         p.spec_stride = batches[b].n;
         for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
         KS_CUDA(c, ks_launch_stream(p, c->num_sms, c->stream));
         c->launches += 1;
       }
-    } else {
+    }
+    if (tier == KS_TIER_A) {
       // group buckets by head dimensions; one persistent launch per group of <= 4 buckets
       bool done[KS_MAX_BATCHES] = {false};
       for (int b = 0; b < n_batches; ++b) {
+        if (batches[b].family == KS_FAM_ALLREDUCE) done[b] = true;
         if (done[b] || batches[b].n == 0) { done[b] = true; continue; }
         const HeadState& h0 = c->heads[batches[b].family];
         KsMlpParams p;
         memset(&p, 0, sizeof(p));
         int nb = 0, tiles = 0;
         for (int q = b; q < n_batches && nb < KS_MLP_MAX_BUCKETS; ++q) {
-          if (done[q] || batches[q].n == 0) continue;
+          if (done[q] || batches[q].n == 0 || batches[q].family == KS_FAM_ALLREDUCE) continue;
           const HeadState& hq = c->heads[batches[q].family];
           if (hq.n_in != h0.n_in || hq.h != h0.h) continue;
           p.bk[nb] = make_bucket_dev(batches[q], cols[q], outs[q], s0);

@@ -28,8 +28,9 @@ struct KsSpecDev {
   float inv_peak_flops, inv_peak_bw, t0, inv_t0;
   float l2_bytes, lg_ridge, inv_slots, slots_f;
   KsFastDiv tile_m, tile_n, ew, slots;
+  float ar_alpha0, ar_inv_beta, pad0, pad1;       // Eq. 3
 };
-static_assert(sizeof(KsSpecDev) == 96, "KsSpecDev layout");
+static_assert(sizeof(KsSpecDev) == 112, "KsSpecDev layout");
 
 #define KS_MAX_SPECS_PER_LAUNCH 64
 
@@ -106,6 +107,8 @@ KS_DEV KsWork ks_decode(const int* v, const KsBucketDev& bk, const KsSpecDev& sp
     w.F = 4.0f * Bf * (float)bk.hq * hd * pairs;
     w.Y = s * 2.0f * Bf * hd * fmaf(qf, (float)bk.hq, (float)kv * (float)bk.hkv);
     w.B = ks_sat31((unsigned long long)Bq * (unsigned long long)bk.hq * ks_ceil_div(q, sp.tile_m));
+  } else if (FAM == KS_FAM_ALLREDUCE) {
+    w.F = 0.0f; w.Y = 0.0f; w.B = 0u;               // a communication row has no roofline (ks_allreduce)
   } else {
     const int n = ks_nonneg(v[0]);
     const int op = ks_ew_op(v[1]);
@@ -115,6 +118,15 @@ KS_DEV KsWork ks_decode(const int* v, const KsBucketDev& bk, const KsSpecDev& sp
   }
   if (w.B == 0u) { w.F = 0.0f; w.Y = 0.0f; }
   return w;
+}
+
+// ------------------------------------------------------------------ TP all-reduce, Eq. 3
+// t_ar = alpha0 + 2 (P - 1) / P * S / beta_eff; P <= 1 moves nothing
+KS_DEV float ks_allreduce(const int* v, const KsSpecDev& sp) {
+  const int S = ks_nonneg(v[0]), P = v[1];
+  if (P <= 1) return sp.ar_alpha0;
+  const float Pf = (float)P;
+  return fmaf(__fdividef(2.0f * (Pf - 1.0f), Pf), (float)S * sp.ar_inv_beta, sp.ar_alpha0);
 }
 
 // ------------------------------------------------------------------ S2: roofline + wave quantization

@@ -17,6 +17,7 @@ namespace {
 template <int FAM> struct NCols { static constexpr int v = 3; };
 template <> struct NCols<KS_FAM_GROUPED_GEMM> { static constexpr int v = 10; };
 template <> struct NCols<KS_FAM_ELEMWISE> { static constexpr int v = 2; };
+template <> struct NCols<KS_FAM_ALLREDUCE> { static constexpr int v = 2; };
 
 template <int NC, bool F32>
 KS_DEV void load_rows4(const KsBucketDev& bk, int row0, int n, int (&v)[4][NC]) {
@@ -163,6 +164,7 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
         tr[j] = r.t_roof;
         // Eq. 2: t = max(t_roof * eta, t0), eta = 1/e; the floor is applied after eta
         t[j] = fmaxf(TIER == KS_TIER_NONE ? r.t_roof : __fdividef(r.t_roof, e[j]), sp.t0);
+        if (FAM == KS_FAM_ALLREDUCE) tr[j] = t[j] = ks_allreduce(v[j], sp);   // Eq. 3 as it stands
       }
       store4<float>(p.bk.lat, off, row0, n, vec, t[0], t[1], t[2], t[3]);
       if (p.bk.tiles) store4<int>(p.bk.tiles, off, row0, n, vec, tiles[0], tiles[1], tiles[2], tiles[3]);
@@ -208,6 +210,7 @@ cudaError_t launch_t(const KsStreamParams& p, int num_sms, cudaStream_t st) {
     case KS_FAM_GROUPED_GEMM: return launch_ft<KS_FAM_GROUPED_GEMM, TIER>(p, num_sms, st);
     case KS_FAM_ATTN: return launch_ft<KS_FAM_ATTN, TIER>(p, num_sms, st);
     case KS_FAM_ELEMWISE: return launch_ft<KS_FAM_ELEMWISE, TIER>(p, num_sms, st);
+    case KS_FAM_ALLREDUCE: return launch_ft<KS_FAM_ALLREDUCE, KS_TIER_NONE>(p, num_sms, st);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -22,8 +22,8 @@ import numpy as np
 
 # kernel families (values match include/ks.h and oracle/ks_oracle.h, each of
 # which declares its own copy)
-FAM_GEMM, FAM_GROUPED, FAM_ATTN, FAM_ELEMWISE = 0, 1, 2, 3
-FAM_NAMES = {0: "gemm", 1: "grouped_gemm", 2: "attention", 3: "elementwise"}
+FAM_GEMM, FAM_GROUPED, FAM_ATTN, FAM_ELEMWISE, FAM_ALLREDUCE = 0, 1, 2, 3, 4
+FAM_NAMES = {0: "gemm", 1: "grouped_gemm", 2: "attention", 3: "elementwise", 4: "allreduce"}
 TIER_NONE, TIER_A, TIER_B = 0, 1, 2
 # elementwise sub-operations (reading Q1)
 SUB_RMSNORM, SUB_SILU_MUL, SUB_ROPE, SUB_KV_WRITE, SUB_EMBED, SUB_RESADD = 0, 1, 2, 3, 4, 5
@@ -88,7 +88,8 @@ class Workload:
 def spec_gb200(**over) -> dict:
     """Config 1's spec vector (Table 5 GB200 peaks; SM/tile fields [BJ])."""
     s = dict(peak_flops=2.25e15, peak_bw=8.0e12, n_sm=148, ctas_per_sm=1, tile_m=128,
-             tile_n=128, ew_elems_per_cta=4096, l2_bytes=126e6, t0=2e-6)
+             tile_n=128, ew_elems_per_cta=4096, l2_bytes=126e6, t0=2e-6,
+             ar_alpha0=10e-6, ar_beta_eff=900e9)   # interconnect (Eq. 3): NVLink 5 datasheet bandwidth, 10 us startup
     s.update(over)
     return s
 
@@ -298,8 +299,10 @@ def _attn_bucket(n_dec, chunk, hist, kv_dec, n_layers):
 
 
 def config4(n_steps: int = 100_000, seed: int = 3, tier: int = TIER_NONE, n_cfg: int = 64,
-            step_params: Optional[dict] = None, n_layers: int = N_LAYERS) -> Workload:
-    """Serving-step composition: 32-layer dense decoder, 9 kernels/layer (+1 prefill attention)."""
+            step_params: Optional[dict] = None, n_layers: int = N_LAYERS, tp: int = 1) -> Workload:
+    """Serving-step composition: 32-layer dense decoder, 9 kernels/layer (+1 prefill attention).
+    tp > 1 (not a BASELINE.json config) adds the two tensor-parallel
+    all-reduces per layer of PAPER.md:221 as a fourth bucket: S = T x hidden x 2 bytes over P = tp."""
     rng = _rng(seed)
     n_dec, chunk, hist, kv_dec, T = _draw_steps(rng, n_steps)
     L = n_layers
@@ -325,7 +328,12 @@ def config4(n_steps: int = 100_000, seed: int = 3, tier: int = TIER_NONE, n_cfg:
         hr = _rng(1)  # cfg-2-sized heads, seed 1 (SURVEY.md §8(d) cfg 4b)
         heads = {f: make_head(hr, 12, 128) for f in (FAM_GEMM, FAM_ATTN, FAM_ELEMWISE)}
     name = "cfg4a_steps_tierNONE" if tier == TIER_NONE else "cfg4b_steps_tierA"
-    return Workload(name, [gemm, attn, elem], [spec_gb200()], tier, heads=heads, n_steps=n_steps,
+    buckets = [gemm, attn, elem]
+    if tp > 1:
+        S = np.repeat(T * HIDDEN * 2, 2 * L)
+        buckets.append(Bucket(FAM_ALLREDUCE, _i32(S, np.full(S.shape[0], tp)), step_off=_csr(np.full(n_steps, 2 * L))))
+        name += f"_tp{tp}"
+    return Workload(name, buckets, [spec_gb200()], tier, heads=heads, n_steps=n_steps,
                     cfg_off=cfg_offsets(rng, n_steps, min(n_cfg, n_steps)),
                     step_params=dict(step_params or STEP_PARAMS_CFG4), seed=seed)
 

@@ -284,3 +284,40 @@ def test_status_codes_on_device(ks):
     empty = W.Workload("empty", [W.Bucket(W.FAM_GEMM, W._i32([], [], []))], w.specs, W.TIER_NONE)
     ctx.predict_kernels(D.to_device(empty), w.specs, W.TIER_NONE, [torch.empty((1, 0), device="cuda")])   # n = 0 no-op
     ctx.close()
+
+
+# ------------------------------------------------------------------ TP all-reduce rows (Eq. 3, NEXT-3)
+@pytest.mark.parametrize("tier", [W.TIER_NONE, W.TIER_A])
+def test_allreduce_family_and_tp_steps(ks, tier):
+    B, D = ks
+    w = W.config4(n_steps=37, n_layers=3, tier=tier, tp=4)
+    w.specs = [W.spec_gb200(ar_alpha0=7e-6, ar_beta_eff=450e9), W.spec_gb200(ar_alpha0=0.0, ar_beta_eff=900e9, t0=5e-6)]
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        db = D.to_device(w)
+        g = D.predict(ctx, w, dbuckets=db)
+        step, tot = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+    finally:
+        ctx.close()
+    o = oracle_all(w, tier)
+    assert w.buckets[-1].family == W.FAM_ALLREDUCE
+    for i, (gi, oi) in enumerate(zip(g, o)):
+        check_bucket(gi, oi, TOL_F32 if (tier == W.TIER_NONE or i == 3) else TOL_MLP, what=f"{w.name}/bucket{i}")
+    assert np.all(g[3]["tiles"] == 0) and np.all(g[3]["waves"] == 0)
+    for s in range(2):                                 # the all-reduce rows enter the step sum like kernels
+        so, to = O.compose([x["lat"][s] for x in g], [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off)
+        assert rel_err(step[s], so).max() <= TOL_F32 and rel_err(tot[s], to).max() <= TOL_F32
+
+
+def test_allreduce_degenerate_rows(ks):
+    B, D = ks
+    cols = [np.array([0, 1, 1 << 30, 4096, 4096, 4096], np.int32), np.array([8, 1, 2, 0, -3, 1 << 20], np.int32)]
+    w = W.Workload("ar_edge", [W.Bucket(W.FAM_ALLREDUCE, cols)], [W.spec_gb200(ar_alpha0=3e-6, ar_beta_eff=100e9)], W.TIER_B)
+    ctx = B.Context(0)
+    try:
+        g = D.predict(ctx, w)                          # Tier B without any grid loaded: Eq. 3 rows need none
+    finally:
+        ctx.close()
+    o = oracle_all(w, W.TIER_NONE)
+    check_bucket(g[0], o[0], TOL_F32, what="ar_edge")
