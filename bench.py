@@ -32,7 +32,7 @@ METRIC = "kernel_latency_predictions_per_sec"
 UNIT = "predictions/s"
 FLOPS_PER_PRED = {(12, 128): 2 * (16 * 128 + 128 * 128 + 128), (8, 64): 2 * (8 * 64 + 64 * 64 + 64),
                   (32, 256): 2 * (32 * 256 + 256 * 256 + 256)}
-BYTES_PER_ROW = {W.FAM_GEMM: 16, W.FAM_ATTN: 16, W.FAM_ELEMWISE: 12, W.FAM_GROUPED: 44}
+BYTES_PER_ROW = {W.FAM_GEMM: 16, W.FAM_ATTN: 16, W.FAM_ELEMWISE: 12, W.FAM_GROUPED: 44, W.FAM_ALLREDUCE: 12}
 
 
 def load_peaks():
@@ -185,6 +185,15 @@ class Harness:
         torch.cuda.synchronize()                     # uploads ran on the default stream
         return dict(w=w, db=db, lat=lat, cfg=cfg, n_cfg=n_cfg, step=step, tot=tot, ns=ns)
 
+    def prepare_rows(self, w):
+        """prepare() for a workload without step segmentation (per-kernel predictions only)."""
+        torch = self.torch
+        self.D.load_models(self.ctx, w)
+        db = self.D.to_device(w, self.dev)
+        lat = [torch.empty((len(w.specs), b.n), dtype=torch.float32, device=self.dev) for b in db]
+        torch.cuda.synchronize()
+        return dict(w=w, db=db, lat=lat, ns=len(w.specs))
+
     def predict(self, st, buckets=None, lat=None):
         db = st["db"] if buckets is None else buckets
         self.ctx.predict_kernels(db, st["w"].specs, st["w"].tier, st["lat"] if lat is None else lat,
@@ -308,6 +317,12 @@ def run_extras(h: Harness, peaks):
     ms = h.timed([lambda: h.predict(st), lambda: h.compose(st)], EX_ITERS, EX_WARM)
     ex["cfg4a_tierNONE"]["predictions_per_s"] = float(st["w"].n_rows / (ms.sum(axis=1).mean() * 1e-3))
     del st
+    torch.cuda.empty_cache()
+    # NEXT-3: tensor-parallel all-reduce rows (Eq. 3), 6.4M rows = two per layer of cfg4's 100k steps
+    st = h.prepare_rows(W.allreduce_rows())
+    sets = None if PROFILE else clone_sets(st, 6)
+    ex["allreduce_eq3"] = dict(stream=stream_roofline(h, st, peaks, sets=sets))
+    del st, sets
     torch.cuda.empty_cache()
     # config 3: Tier B, 4M queries
     st = h.prepare(W.config3())

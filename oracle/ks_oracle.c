@@ -287,6 +287,52 @@ double kso_predict_one(const kso_desc *d, const kso_spec *hw, int tier, const ks
   return dmax(r.t_roof / e, hw->t0);                            /* floor applied after eta */
 }
 
+/* PAPER.md:197 Fig. 6, :201; Q15 */
+double kso_bounded_e(const kso_bounded *bh, const double *x, int64_t W) {
+  double zg = bh->b_gamma, za = bh->b_alpha;
+  for (int i = 0; i < bh->n_in; ++i) { zg += bh->w_gamma[i] * x[i]; za += bh->w_alpha[i] * x[i]; }
+  const double gamma = kso_sigmoid(zg);
+  const double alpha = dmax(za, 0.0);
+  double e = gamma;
+  if (W > 0) e = gamma - alpha / (double)W;
+  if (e > 1.0) e = 1.0;
+  return dmax(e, ldexp(1.0, -10));
+}
+
+double kso_predict_one_bounded(const kso_desc *d, const kso_spec *hw, const kso_bounded *bh, kso_roof *rout,
+                               double *e_out) {
+  if (d->family == KSO_ALLREDUCE) return kso_predict_one(d, hw, KSO_TIER_NONE, NULL, NULL, rout, e_out);
+  kso_roof r;
+  kso_roofline(d, hw, &r);
+  double x[32];
+  kso_features(d, hw, &r, bh->n_in, x);
+  const double e = kso_bounded_e(bh, x, r.W);
+  if (rout) *rout = r;
+  if (e_out) *e_out = e;
+  return dmax(r.t_roof / e, hw->t0);
+}
+
+int kso_predict_batch_bounded(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
+                              int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
+                              const kso_bounded *bh, double *lat, int64_t *tiles, int64_t *waves, double *troof) {
+  if (n < 0 || n_cols < 0 || n_cols > KSO_MAX_COLS || !bh) return -1;
+  for (int sp = 0; sp < n_specs; ++sp) {
+    for (int64_t i = 0; i < n; ++i) {
+      kso_desc d;
+      d.family = family; d.s = s; d.hq = hq; d.hkv = hkv; d.d = dh;
+      for (int c = 0; c < KSO_MAX_COLS; ++c) d.v[c] = (c < n_cols) ? (int64_t)llround(cols[c][i]) : 0;
+      kso_roof r;
+      const double t = kso_predict_one_bounded(&d, &specs[sp], bh, &r, NULL);
+      const size_t o = (size_t)sp * (size_t)n + (size_t)i;
+      lat[o] = t;
+      if (tiles) tiles[o] = r.B;
+      if (waves) waves[o] = r.W;
+      if (troof) troof[o] = r.t_roof;
+    }
+  }
+  return 0;
+}
+
 int kso_predict_batch(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
                       int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
                       int tier, const kso_head *h, const kso_grid *g, double *lat, int64_t *tiles,

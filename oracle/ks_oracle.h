@@ -20,7 +20,7 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Fig. 2's worked example, hand-computed
  * rooflines (tests/golden/roofline_cases.txt), brute-force wave/tile/pair counts,
  * numpy+scipy MLP, scipy RegularGridInterpolator, torch bf16 rounding, np.add.reduceat,
- * Eq. 4 regimes, Eq. 3 special cases (P = 1, P = 2, P -> inf, linearity in S, a hand-computed case).  Parity unpinned: NONE of the functions below — but note the
+ * Eq. 4 regimes, the bounded head's closed forms (alpha = 0, constant maps, W -> inf, numpy dot), Eq. 3 special cases (P = 1, P = 2, P -> inf, linearity in S, a hand-computed case).  Parity unpinned: NONE of the functions below — but note the
  * *feature list* (kso_features) is a reading (Q2): its closed-form special
  * cases are pinned, the paper prints no values for it.
  */
@@ -69,6 +69,12 @@ typedef struct {           /* Tier B measured-efficiency grid */
   const double *values;    /* [d0][d1][d2], last fastest */
 } kso_grid;
 
+typedef struct {           /* bounded analytical head, PAPER.md:197 Fig. 6, :201; maps = DESIGN.md Q15 */
+  int n_in;
+  const double *w_gamma, *w_alpha; /* [n_in] */
+  double b_gamma, b_alpha;
+} kso_bounded;
+
 typedef struct { double c_disp, floor_l, c_ovl, c_tail, body_scale; } kso_step_params; /* Eq. 4 */
 
 /* round-to-nearest-even to bfloat16 precision (8 significant bits), returned as double */
@@ -97,6 +103,17 @@ double kso_trilinear(const kso_grid *g, const double v[3]);
 /* Tier-B axis values of a descriptor: GEMM (M,N,K); GROUPED (sum m,N,K); ATTN (B,q,kv);
  * ELEMWISE (n, 2^subop, 1) */
 void kso_grid_axes(const kso_desc *d, double v[3]);
+/* Bounded analytical head: utilisation e = gamma(x) - alpha(x) / W, eta = 1 / e, with
+ * gamma(x) = sigmoid(w_gamma . x + b_gamma) in (0,1) and alpha(x) = max(0, w_alpha . x + b_alpha)
+ * (Q15); x = the dimensionless features in full precision (no tensor core on this path);
+ * e is clamped to [2^-10, 1]; W = 0 (empty kernel) gives e = gamma. */
+double kso_bounded_e(const kso_bounded *bh, const double *x, int64_t W);
+/* One full prediction with the bounded head: t = max(t_roof / e, t0). */
+double kso_predict_one_bounded(const kso_desc *d, const kso_spec *hw, const kso_bounded *bh, kso_roof *r,
+                               double *e_out);
+int kso_predict_batch_bounded(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
+                              int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
+                              const kso_bounded *bh, double *lat, int64_t *tiles, int64_t *waves, double *troof);
 /* S5: one full prediction. head/grid may be NULL unless the tier needs them.
  * Returns latency; optional outputs via r (may be NULL) and e_out (may be NULL). */
 double kso_predict_one(const kso_desc *d, const kso_spec *hw, int tier, const kso_head *h,

@@ -78,6 +78,13 @@ def lib():
         L.kso_gelu.argtypes = [C.c_double]
         L.kso_sigmoid.restype = C.c_double
         L.kso_sigmoid.argtypes = [C.c_double]
+        L.kso_bounded_e.restype = C.c_double
+        L.kso_bounded_e.argtypes = [C.POINTER(BoundedC), C.POINTER(C.c_double), C.c_int64]
+        L.kso_predict_batch_bounded.restype = C.c_int
+        L.kso_predict_batch_bounded.argtypes = [C.c_int, C.c_int64, C.POINTER(C.POINTER(C.c_double)), C.c_int,
+                                                C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.POINTER(Spec), C.c_int,
+                                                C.POINTER(BoundedC), C.POINTER(C.c_double), C.POINTER(C.c_int64),
+                                                C.POINTER(C.c_int64), C.POINTER(C.c_double)]
         L.kso_allreduce.restype = C.c_double
         L.kso_allreduce.argtypes = [C.c_int64, C.c_int64, C.POINTER(Spec)]
         L.kso_attn_pairs.restype = C.c_int64
@@ -152,6 +159,21 @@ class Head:
                        _dp(self.b2), _dp(self.w3), float(h.b3))
 
 
+class BoundedC(C.Structure):
+    _fields_ = [("n_in", C.c_int), ("w_gamma", C.POINTER(C.c_double)), ("w_alpha", C.POINTER(C.c_double)),
+                ("b_gamma", C.c_double), ("b_alpha", C.c_double)]
+
+
+class Bounded:
+    """The bounded analytical head's weights as the library receives them (fp32 values, held as double)."""
+
+    def __init__(self, h):
+        self.wg = np.ascontiguousarray(np.asarray(h.w_gamma, np.float32), dtype=np.float64)
+        self.wa = np.ascontiguousarray(np.asarray(h.w_alpha, np.float32), dtype=np.float64)
+        self.c = BoundedC(int(h.n_in), _dp(self.wg), _dp(self.wa), float(np.float32(h.b_gamma)),
+                          float(np.float32(h.b_alpha)))
+
+
 class Grid:
     def __init__(self, g):
         self.values = np.ascontiguousarray(g.values, dtype=np.float64)
@@ -199,8 +221,14 @@ def predict_one(desc: Desc, spec: Spec, tier: int, head: Optional[Head] = None,
     return t, r, e.value
 
 
+def bounded_e(bh: "Bounded", x, W: int) -> float:
+    xa = np.ascontiguousarray(x, dtype=np.float64)
+    return float(lib().kso_bounded_e(C.byref(bh.c), _dp(xa), int(W)))
+
+
 def predict_bucket(bucket, specs: Sequence[dict], tier: int, head: Optional[Head] = None,
-                   grid: Optional[Grid] = None, rows: Optional[np.ndarray] = None):
+                   grid: Optional[Grid] = None, rows: Optional[np.ndarray] = None,
+                   bounded: Optional["Bounded"] = None):
     """Run the oracle over one workloads.Bucket (optionally only ``rows``) for every spec.
 
     Returns dict(lat [n_specs,n] f64, tiles i64, waves i64, troof f64).
@@ -214,6 +242,13 @@ def predict_bucket(bucket, specs: Sequence[dict], tier: int, head: Optional[Head
     troof = np.zeros((ns, n), np.float64)
     tiles = np.zeros((ns, n), np.int64)
     waves = np.zeros((ns, n), np.int64)
+    if bounded is not None and tier == 1:      # Tier A with the bounded analytical head for this family
+        rc = lib().kso_predict_batch_bounded(int(bucket.family), n, colp, len(cols), int(bucket.dtype_bytes),
+                                             int(bucket.hq), int(bucket.hkv), int(bucket.head_dim), sp, ns,
+                                             C.byref(bounded.c), _dp(lat), _ip(tiles), _ip(waves), _dp(troof))
+        if rc != 0:
+            raise ValueError("kso_predict_batch_bounded: bad arguments")
+        return dict(lat=lat, tiles=tiles, waves=waves, troof=troof)
     rc = lib().kso_predict_batch(int(bucket.family), n, colp, len(cols), int(bucket.dtype_bytes),
                                  int(bucket.hq), int(bucket.hkv), int(bucket.head_dim), sp, ns, int(tier),
                                  C.byref(head.c) if head else None, C.byref(grid.c) if grid else None,

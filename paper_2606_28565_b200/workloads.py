@@ -60,6 +60,17 @@ class Head:
 
 
 @dataclass
+class BoundedHead:
+    """Bounded analytical head: gamma(x) = sigmoid(w_gamma.x + b_gamma),
+    alpha(x) = max(0, w_alpha.x + b_alpha); utilisation e = gamma - alpha / W."""
+    n_in: int
+    w_gamma: np.ndarray  # [n_in] fp32
+    b_gamma: float
+    w_alpha: np.ndarray  # [n_in] fp32
+    b_alpha: float
+
+
+@dataclass
 class Grid:
     dims: np.ndarray      # int32[3]
     lo_log2: np.ndarray   # float32[3]
@@ -75,6 +86,7 @@ class Workload:
     tier: int
     heads: Dict[int, Head] = field(default_factory=dict)
     grids: Dict[int, Grid] = field(default_factory=dict)
+    bounded: Dict[int, BoundedHead] = field(default_factory=dict)   # families whose Tier-A head is the bounded form
     n_steps: int = 0
     cfg_off: Optional[np.ndarray] = None  # CSR [n_cfg+1] int32 over steps
     step_params: Optional[dict] = None
@@ -122,6 +134,12 @@ def make_head(rng, n_in: int, h: int, bias_std: float = 0.1, w_std: float = 0.1)
         b2 = np.zeros(h, np.float32)
         b3 = 0.0
     return Head(n_in, h, h, W1, b1, W2, b2, w3, b3)
+
+
+def make_bounded_head(rng, n_in: int) -> BoundedHead:
+    """Random bounded head: peak utilisation gamma around sigmoid(1) = 0.73, partial-wave overhead alpha ~ 0.2."""
+    return BoundedHead(n_in, rng.normal(0.0, 0.3, n_in).astype(np.float32), float(np.float32(rng.normal(1.0, 0.3))),
+                       rng.normal(0.0, 0.15, n_in).astype(np.float32), float(np.float32(rng.uniform(0.05, 0.4))))
 
 
 def _box3(v: np.ndarray) -> np.ndarray:
@@ -336,6 +354,15 @@ def config4(n_steps: int = 100_000, seed: int = 3, tier: int = TIER_NONE, n_cfg:
     return Workload(name, buckets, [spec_gb200()], tier, heads=heads, n_steps=n_steps,
                     cfg_off=cfg_offsets(rng, n_steps, min(n_cfg, n_steps)),
                     step_params=dict(step_params or STEP_PARAMS_CFG4), seed=seed)
+
+
+def allreduce_rows(n: int = 6_400_000, seed: int = 5, tp: int = 4) -> Workload:
+    """n tensor-parallel all-reduce rows: the two per-layer all-reduces of
+    100,000 steps of config 4's decoder (T tokens x hidden x 2 bytes over P = tp), as one bucket."""
+    rng = _rng(seed)
+    T = np.clip(rng.poisson(64, size=n), 1, 256) + 512 * (rng.random(n) < 0.25)
+    return Workload(f"allreduce_tp{tp}", [Bucket(FAM_ALLREDUCE, _i32(T * HIDDEN * 2, np.full(n, tp)))],
+                    [spec_gb200()], TIER_NONE, seed=seed)
 
 
 # ----------------------------------------------------------------------------- config 5
