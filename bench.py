@@ -324,6 +324,17 @@ def run_extras(h: Harness, peaks):
     ex["allreduce_eq3"] = dict(stream=stream_roofline(h, st, peaks, sets=sets))
     del st, sets
     torch.cuda.empty_cache()
+    # NEXT-2: bounded analytical head for every family of cfg2 (Tier A without the contraction)
+    wb = W.config2()
+    rng = np.random.Generator(np.random.PCG64(12))
+    wb.bounded = {f: W.make_bounded_head(rng, 12) for f in list(wb.heads)}
+    wb.heads = {}
+    st = h.prepare(wb)
+    ms = h.timed([lambda: h.predict(st)], EX_ITERS, EX_WARM)[:, 0]
+    ex["cfg2_bounded_head"] = dict(ms=float(ms.mean()), predictions_per_s=float(wb.n_rows / (ms.mean() * 1e-3)),
+                                   launches=3, note="streaming kernel, ~300 instructions per row: issue-bound")
+    del st
+    torch.cuda.empty_cache()
     # config 3: Tier B, 4M queries
     st = h.prepare(W.config3())
     sets = None if PROFILE else clone_sets(st, 8)

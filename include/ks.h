@@ -110,6 +110,15 @@ KS_API ks_status ks_create(ks_ctx **out, int device, void *cuda_stream);
 KS_API ks_status ks_load_heads(ks_ctx *ctx, ks_family family, int n_in, int h1, int h2, const float *W1,
                         const float *b1, const float *W2, const float *b2, const float *w3, float b3);
 
+/* Load (or replace) the Tier-A head of `family` with the BOUNDED ANALYTICAL form (PAPER.md:197 Fig. 6, :201;
+ * DESIGN.md Q15): utilisation e = gamma(x) - alpha(x) / W with W the kernel's wave count,
+ * gamma(x) = sigmoid(w_gamma . x + b_gamma), alpha(x) = max(0, w_alpha . x + b_alpha), e clamped to
+ * [2^-10, 1], eta = 1 / e.  x = the library's dimensionless features (Q2) in fp32; n_in in {8, 12, 32}.
+ * w_gamma[n_in], w_alpha[n_in]: HOST fp32, copied.  A family holds ONE Tier-A head: this call replaces
+ * an MLP head loaded with ks_load_heads and vice versa.  Runs in the streaming kernel (no contraction). */
+KS_API ks_status ks_load_bounded_head(ks_ctx *ctx, ks_family family, int n_in, const float *w_gamma, float b_gamma,
+                               const float *w_alpha, float b_alpha);
+
 /* Load (or replace) the Tier-B measured-efficiency grid of `family` (Q5).
  * values: HOST fp32 [dims[0]][dims[1]][dims[2]], last index fastest, copied; each dims[a] >= 1 and
  * the product <= KS_MAX_GRID_NODES.  Axis a spans [lo_log2[a], hi_log2[a]] in log2 units with

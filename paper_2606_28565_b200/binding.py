@@ -21,7 +21,7 @@ KS_TIER_NONE, KS_TIER_A, KS_TIER_B = range(3)
 KS_COL_I32, KS_COL_F32 = 0, 1
 KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
-EXPORTS = ["ks_create", "ks_load_heads", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
+EXPORTS = ["ks_create", "ks_load_heads", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
            "ks_run_steps", "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
 
 
@@ -64,6 +64,7 @@ def load() -> C.CDLL:
     vp, i32, fp = C.c_void_p, C.c_int, C.POINTER(C.c_float)
     L.ks_create.argtypes = [C.POINTER(vp), i32, vp]
     L.ks_load_heads.argtypes = [vp, i32, i32, i32, i32, fp, fp, fp, fp, fp, C.c_float]
+    L.ks_load_bounded_head.argtypes = [vp, i32, i32, fp, C.c_float, fp, C.c_float]
     L.ks_load_grid.argtypes = [vp, i32, C.POINTER(C.c_int32), fp, fp, fp]
     L.ks_predict_kernels.argtypes = [vp, C.POINTER(ks_desc_batch), i32, C.POINTER(ks_hw_spec), i32, i32, i32,
                                      C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
@@ -168,6 +169,13 @@ class Context:
         fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
         _check(self._lib.ks_load_heads(self._h, int(family), int(head.n_in), int(head.h1), int(head.h2), fp(W1),
                                        fp(b1), fp(W2), fp(b2), fp(w3), float(head.b3)), "ks_load_heads")
+
+    def load_bounded_head(self, family: int, head) -> None:
+        wg = np.ascontiguousarray(head.w_gamma, dtype=np.float32)
+        wa = np.ascontiguousarray(head.w_alpha, dtype=np.float32)
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        _check(self._lib.ks_load_bounded_head(self._h, int(family), int(head.n_in), fp(wg), float(head.b_gamma),
+                                              fp(wa), float(head.b_alpha)), "ks_load_bounded_head")
 
     def load_grid(self, family: int, grid) -> None:
         dims = np.ascontiguousarray(grid.dims, dtype=np.int32)

@@ -16,6 +16,8 @@ namespace {
 
 struct HeadState {
   bool loaded = false;
+  bool bounded = false;      // the family's Tier-A head is the bounded analytical form (host-resident weights)
+  KsBoundedDev bw;
   int n_in = 0, h = 0;
   void* w1_img = nullptr;
   void* w2_img = nullptr;
@@ -226,14 +228,16 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
     const int ns = n_specs - s0 < KS_MAX_SPECS_PER_LAUNCH ? n_specs - s0 : KS_MAX_SPECS_PER_LAUNCH;
     for (int b = 0; b < n_batches; ++b) {               // streaming kernels: Tier NONE / B, and Eq. 3 rows under any tier
       const bool ar = batches[b].family == KS_FAM_ALLREDUCE;
-      if (batches[b].n == 0 || (tier == KS_TIER_A && !ar)) continue;
+      const bool bnd = tier == KS_TIER_A && !ar && c->heads[batches[b].family].bounded;
+      if (batches[b].n == 0 || (tier == KS_TIER_A && !ar && !bnd)) continue;
       {
         KsStreamParams p;
         memset(&p, 0, sizeof(p));
         p.bk = make_bucket_dev(batches[b], cols[b], outs[b], s0);
         if (tier == KS_TIER_B && !ar) p.grid = c->grids[batches[b].family].dev;
         p.n_specs = ns;
-        p.tier = ar ? KS_TIER_NONE : tier;
+        p.tier = ar ? KS_TIER_NONE : bnd ? KS_TIER_BOUNDED : tier;
+        if (bnd) p.bounded = c->heads[batches[b].family].bw;
         p.spec_stride = batches[b].n;
         for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
         KS_CUDA(c, ks_launch_stream(p, c->num_sms, c->stream));
@@ -244,14 +248,15 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
       // group buckets by head dimensions; one persistent launch per group of <= 4 buckets
       bool done[KS_MAX_BATCHES] = {false};
       for (int b = 0; b < n_batches; ++b) {
-        if (batches[b].family == KS_FAM_ALLREDUCE) done[b] = true;
+        if (batches[b].family == KS_FAM_ALLREDUCE || c->heads[batches[b].family].bounded) done[b] = true;
         if (done[b] || batches[b].n == 0) { done[b] = true; continue; }
         const HeadState& h0 = c->heads[batches[b].family];
         KsMlpParams p;
         memset(&p, 0, sizeof(p));
         int nb = 0, tiles = 0;
         for (int q = b; q < n_batches && nb < KS_MLP_MAX_BUCKETS; ++q) {
-          if (done[q] || batches[q].n == 0 || batches[q].family == KS_FAM_ALLREDUCE) continue;
+          if (done[q] || batches[q].n == 0 || batches[q].family == KS_FAM_ALLREDUCE ||
+              c->heads[batches[q].family].bounded) continue;
           const HeadState& hq = c->heads[batches[q].family];
           if (hq.n_in != h0.n_in || hq.h != h0.h) continue;
           p.bk[nb] = make_bucket_dev(batches[q], cols[q], outs[q], s0);
@@ -401,6 +406,30 @@ ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, c
   hs.w3 = static_cast<float*>(d3);
   hs.b2 = static_cast<float*>(d4);
   hs.b3 = b3;
+  return KS_OK;
+}
+
+ks_status ks_load_bounded_head(ks_ctx* c, ks_family family, int n_in, const float* w_gamma, float b_gamma,
+                               const float* w_alpha, float b_alpha) {
+  if (!c || family < 0 || family >= KS_FAM_COUNT || family == KS_FAM_ALLREDUCE || !w_gamma || !w_alpha) return KS_EINVAL;
+  if (n_in <= 0 || !isfinite(b_gamma) || !isfinite(b_alpha)) return KS_EINVAL;
+  for (int i = 0; i < n_in && i < 64; ++i)
+    if (!isfinite(w_gamma[i]) || !isfinite(w_alpha[i])) return KS_EINVAL;
+  if (c->sticky) return KS_ECUDA;
+  if (n_in != 8 && n_in != 12 && n_in != 32) return KS_EUNSUPPORTED;
+  KS_CUDA(c, cudaSetDevice(c->device));
+  KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read an MLP head being replaced
+  HeadState& hs = c->heads[family];
+  cudaFree(hs.w1_img); cudaFree(hs.w2_img); cudaFree(hs.w3); cudaFree(hs.b2);
+  hs = HeadState();
+  memset(&hs.bw, 0, sizeof(hs.bw));
+  const int n_real = n_in == 32 ? KS_BOUNDED_NF : n_in;   // features 22..31 are identically zero (Q2)
+  for (int i = 0; i < n_real; ++i) { hs.bw.w_gamma[i] = w_gamma[i]; hs.bw.w_alpha[i] = w_alpha[i]; }
+  hs.bw.b_gamma = b_gamma;
+  hs.bw.b_alpha = b_alpha;
+  hs.loaded = true;
+  hs.bounded = true;
+  hs.n_in = n_in;
   return KS_OK;
 }
 

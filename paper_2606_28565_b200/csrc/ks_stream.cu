@@ -147,6 +147,7 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
       for (int j = 0; j < 4; ++j) e[j] = fmaxf(trilinear<FAM>(v[j], p.grid, sgrid), 0.0009765625f);
     }
 
+    // (Tier A, bounded analytical head: e depends on the spec through the features, see below)
     // ONE: a single spec -> its constants are read straight from the constant bank (no index math)
     const int n_specs = ONE ? 1 : p.n_specs;
     for (int s = 0; s < n_specs; ++s) {
@@ -163,6 +164,20 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
         waves[j] = (int)r.W;
         tr[j] = r.t_roof;
         // Eq. 2: t = max(t_roof * eta, t0), eta = 1/e; the floor is applied after eta
+        if (TIER == KS_TIER_BOUNDED) {
+          // bounded analytical head (Q15): e = gamma(x) - alpha(x) / W
+          float x[KS_BOUNDED_NF];
+          ks_features<FAM, KS_BOUNDED_NF>(v[j], p.bk, sp, w, r, x);
+          float zg = p.bounded.b_gamma, za = p.bounded.b_alpha;
+#pragma unroll
+          for (int i = 0; i < KS_BOUNDED_NF; ++i) {
+            zg = fmaf(p.bounded.w_gamma[i], x[i], zg);
+            za = fmaf(p.bounded.w_alpha[i], x[i], za);
+          }
+          const float gamma = __fdividef(1.0f, 1.0f + __expf(-zg));
+          const float ev = r.W > 0u ? gamma - __fdividef(fmaxf(za, 0.0f), (float)r.W) : gamma;
+          e[j] = fmaxf(fminf(ev, 1.0f), 0.0009765625f);
+        }
         t[j] = fmaxf(TIER == KS_TIER_NONE ? r.t_roof : __fdividef(r.t_roof, e[j]), sp.t0);
         if (FAM == KS_FAM_ALLREDUCE) tr[j] = t[j] = ks_allreduce(v[j], sp);   // Eq. 3 as it stands
       }
@@ -218,5 +233,6 @@ cudaError_t launch_t(const KsStreamParams& p, int num_sms, cudaStream_t st) {
 }  // namespace
 
 cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st) {
+  if (p.tier == KS_TIER_BOUNDED) return launch_t<KS_TIER_BOUNDED>(p, num_sms, st);
   return p.tier == KS_TIER_B ? launch_t<KS_TIER_B>(p, num_sms, st) : launch_t<KS_TIER_NONE>(p, num_sms, st);
 }

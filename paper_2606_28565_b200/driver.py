@@ -61,6 +61,8 @@ def to_pinned(w: Workload) -> List[DeviceBucket]:
 def load_models(ctx: B.Context, w: Workload) -> None:
     for fam, h in w.heads.items():
         ctx.load_heads(fam, h)
+    for fam, bh in getattr(w, "bounded", {}).items():      # families whose Tier-A head is the bounded analytical form
+        ctx.load_bounded_head(fam, bh)
     for fam, g in w.grids.items():
         ctx.load_grid(fam, g)
 

@@ -38,7 +38,9 @@ def oracle_all(w, tier=None, rows=None):
     out = []
     for i, b in enumerate(w.buckets):
         r = None if rows is None else rows[i]
-        out.append(O.predict_bucket(b, w.specs, tier, head=heads.get(b.family), grid=grids.get(b.family), rows=r))
+        bnd = O.Bounded(w.bounded[b.family]) if (tier == W.TIER_A and b.family in getattr(w, "bounded", {})) else None
+        out.append(O.predict_bucket(b, w.specs, tier, head=heads.get(b.family), grid=grids.get(b.family), rows=r,
+                                    bounded=bnd))
     return out
 
 
@@ -321,3 +323,57 @@ def test_allreduce_degenerate_rows(ks):
         ctx.close()
     o = oracle_all(w, W.TIER_NONE)
     check_bucket(g[0], o[0], TOL_F32, what="ar_edge")
+
+
+# ------------------------------------------------------------------ bounded analytical head (NEXT-2)
+TOL_BOUNDED = TOL_F32   # an fp32 path: features through MUFU log2 into two 22-term dot products (measured 1.3e-6)
+
+
+@pytest.mark.parametrize("make,n_in", [(lambda: W.config2(n=30011), 12), (lambda: W.config1(), 8),
+                                       (lambda: W.config5(n_rows=20003, n_specs=3, n_layers=4), 32)])
+def test_bounded_head_parity(ks, make, n_in):
+    B, D = ks
+    w = make()
+    rng = np.random.Generator(np.random.PCG64(11 + n_in))
+    fams = [b.family for b in w.buckets]
+    # every other family gets the bounded form, the rest keep their MLP heads: both kinds in one call
+    w.bounded = {f: W.make_bounded_head(rng, n_in) for f in fams[::2]}
+    w.heads = {f: h for f, h in w.heads.items() if f not in w.bounded}
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        g = D.predict(ctx, w)
+    finally:
+        ctx.close()
+    o = oracle_all(w, W.TIER_A)
+    errs = [check_bucket(gi, oi, TOL_BOUNDED if b.family in w.bounded else TOL_MLP, what=f"{w.name}/bucket{i}")
+            for i, (b, gi, oi) in enumerate(zip(w.buckets, g, o))]
+    print("bounded head max rel err per bucket", errs, "bounded families", sorted(w.bounded))
+
+
+def test_bounded_head_closed_forms_and_replacement(ks):
+    B, D = ks
+    w = W.config1()
+    fam = w.buckets[0].family
+    zero = np.zeros(8, np.float32)
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)                                     # MLP head first ...
+        ctx.load_bounded_head(fam, W.BoundedHead(8, zero, 0.0, zero, -1.0))   # ... replaced: gamma = 1/2, alpha = 0
+        g = D.predict(ctx, w)
+        half = np.maximum(2.0 * g[0]["troof"].astype(np.float64), w.specs[0]["t0"])
+        assert rel_err(g[0]["lat"], half).max() <= 1e-6           # eta = 2 exactly, floor after eta
+        ctx.load_bounded_head(fam, W.BoundedHead(8, zero, 60.0, zero, -1.0))  # gamma -> 1: attains the bound
+        g = D.predict(ctx, w)
+        assert rel_err(g[0]["lat"], np.maximum(g[0]["troof"].astype(np.float64), w.specs[0]["t0"])).max() <= 1e-6
+        ctx.load_heads(fam, w.heads[fam])                         # and back to the MLP head
+        g = D.predict(ctx, w)
+    finally:
+        ctx.close()
+    check_bucket(g[0], oracle_all(w)[0], TOL_MLP, what="cfg1 after reloading the MLP head")
+    with pytest.raises(Exception):
+        c2 = B.Context(0)
+        try:
+            c2.load_bounded_head(fam, W.BoundedHead(9, np.zeros(9, np.float32), 0.0, np.zeros(9, np.float32), 0.0))
+        finally:
+            c2.close()
