@@ -333,6 +333,55 @@ int kso_predict_batch_bounded(int family, int64_t n, const double *const *cols, 
   return 0;
 }
 
+/* PAPER.md:211 density routing; Q16 */
+int kso_in_hull(const kso_grid *g, const kso_desc *d) {
+  double v[3];
+  kso_grid_axes(d, v);
+  for (int a = 0; a < 3; ++a) {
+    if (g->dims[a] <= 1) continue;                      /* a flat axis measures nothing: no constraint */
+    if (!(v[a] > 0.0)) return 0;
+    const double vmin = ceil(exp2(g->lo[a])), vmax = floor(exp2(g->hi[a]));
+    if (v[a] < vmin || v[a] > vmax) return 0;
+  }
+  return 1;
+}
+
+double kso_predict_one_routed(const kso_desc *d, const kso_spec *hw, const kso_grid *g, const kso_head *h,
+                              const kso_bounded *bh, kso_roof *r, double *e_out, int *routed_out) {
+  if (d->family == KSO_ALLREDUCE || kso_in_hull(g, d)) {
+    if (routed_out) *routed_out = 0;
+    return kso_predict_one(d, hw, KSO_TIER_B, NULL, g, r, e_out);
+  }
+  if (routed_out) *routed_out = 1;
+  if (h) return kso_predict_one(d, hw, KSO_TIER_A, h, NULL, r, e_out);
+  return kso_predict_one_bounded(d, hw, bh, r, e_out);
+}
+
+int kso_predict_batch_routed(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
+                             int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
+                             const kso_grid *g, const kso_head *h, const kso_bounded *bh, double *lat,
+                             int64_t *tiles, int64_t *waves, double *troof, int64_t *routed) {
+  if (n < 0 || n_cols < 0 || n_cols > KSO_MAX_COLS) return -1;
+  if (family != KSO_ALLREDUCE && (!g || (!h && !bh))) return -1;
+  for (int sp = 0; sp < n_specs; ++sp) {
+    for (int64_t i = 0; i < n; ++i) {
+      kso_desc d;
+      d.family = family; d.s = s; d.hq = hq; d.hkv = hkv; d.d = dh;
+      for (int c = 0; c < KSO_MAX_COLS; ++c) d.v[c] = (c < n_cols) ? (int64_t)llround(cols[c][i]) : 0;
+      kso_roof r;
+      int fell = 0;
+      const double t = kso_predict_one_routed(&d, &specs[sp], g, h, bh, &r, NULL, &fell);
+      const size_t o = (size_t)sp * (size_t)n + (size_t)i;
+      lat[o] = t;
+      if (tiles) tiles[o] = r.B;
+      if (waves) waves[o] = r.W;
+      if (troof) troof[o] = r.t_roof;
+      if (routed && sp == 0) routed[i] = fell;
+    }
+  }
+  return 0;
+}
+
 int kso_predict_batch(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
                       int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
                       int tier, const kso_head *h, const kso_grid *g, double *lat, int64_t *tiles,

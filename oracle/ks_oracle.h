@@ -33,7 +33,7 @@ extern "C" {
 #endif
 
 enum { KSO_GEMM = 0, KSO_GROUPED = 1, KSO_ATTN = 2, KSO_ELEMWISE = 3, KSO_ALLREDUCE = 4 };
-enum { KSO_TIER_NONE = 0, KSO_TIER_A = 1, KSO_TIER_B = 2 };
+enum { KSO_TIER_NONE = 0, KSO_TIER_A = 1, KSO_TIER_B = 2, KSO_TIER_B_ROUTED = 3 };
 #define KSO_MAX_COLS 10
 #define KSO_EXPERTS 8
 
@@ -114,6 +114,18 @@ double kso_predict_one_bounded(const kso_desc *d, const kso_spec *hw, const kso_
 int kso_predict_batch_bounded(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
                               int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
                               const kso_bounded *bh, double *lat, int64_t *tiles, int64_t *waves, double *troof);
+/* Density routing: 1 iff the query lies inside the measured hull, here the grid's box:
+ * lo_a <= log2 v_a <= hi_a on every axis with more than one node, decided on integers as
+ * ceil(2^lo_a) <= v_a <= floor(2^hi_a) (Q16); a non-positive axis value is outside. */
+int kso_in_hull(const kso_grid *g, const kso_desc *d);
+/* Density-routed Tier B: interpolate the grid inside the hull, otherwise fall back to the family's learned
+ * Tier-A head (MLP `h`, or the bounded form `bh` when h is NULL).  routed_out (may be NULL): 1 = fell back. */
+double kso_predict_one_routed(const kso_desc *d, const kso_spec *hw, const kso_grid *g, const kso_head *h,
+                              const kso_bounded *bh, kso_roof *r, double *e_out, int *routed_out);
+int kso_predict_batch_routed(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
+                             int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
+                             const kso_grid *g, const kso_head *h, const kso_bounded *bh, double *lat,
+                             int64_t *tiles, int64_t *waves, double *troof, int64_t *routed);
 /* S5: one full prediction. head/grid may be NULL unless the tier needs them.
  * Returns latency; optional outputs via r (may be NULL) and e_out (may be NULL). */
 double kso_predict_one(const kso_desc *d, const kso_spec *hw, int tier, const kso_head *h,

@@ -85,6 +85,12 @@ def lib():
                                                 C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.POINTER(Spec), C.c_int,
                                                 C.POINTER(BoundedC), C.POINTER(C.c_double), C.POINTER(C.c_int64),
                                                 C.POINTER(C.c_int64), C.POINTER(C.c_double)]
+        L.kso_predict_batch_routed.restype = C.c_int
+        L.kso_predict_batch_routed.argtypes = [C.c_int, C.c_int64, C.POINTER(C.POINTER(C.c_double)), C.c_int,
+                                               C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.POINTER(Spec), C.c_int,
+                                               C.POINTER(GridC), C.POINTER(HeadC), C.POINTER(BoundedC),
+                                               C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_int64),
+                                               C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.kso_allreduce.restype = C.c_double
         L.kso_allreduce.argtypes = [C.c_int64, C.c_int64, C.POINTER(Spec)]
         L.kso_attn_pairs.restype = C.c_int64
@@ -242,6 +248,16 @@ def predict_bucket(bucket, specs: Sequence[dict], tier: int, head: Optional[Head
     troof = np.zeros((ns, n), np.float64)
     tiles = np.zeros((ns, n), np.int64)
     waves = np.zeros((ns, n), np.int64)
+    if tier == 3:                               # density-routed Tier B: grid inside the hull, head outside
+        routed = np.zeros(n, np.int64)
+        rc = lib().kso_predict_batch_routed(int(bucket.family), n, colp, len(cols), int(bucket.dtype_bytes),
+                                            int(bucket.hq), int(bucket.hkv), int(bucket.head_dim), sp, ns,
+                                            C.byref(grid.c) if grid else None, C.byref(head.c) if head else None,
+                                            C.byref(bounded.c) if bounded else None, _dp(lat), _ip(tiles),
+                                            _ip(waves), _dp(troof), _ip(routed))
+        if rc != 0:
+            raise ValueError("kso_predict_batch_routed: bad arguments")
+        return dict(lat=lat, tiles=tiles, waves=waves, troof=troof, routed=routed)
     if bounded is not None and tier == 1:      # Tier A with the bounded analytical head for this family
         rc = lib().kso_predict_batch_bounded(int(bucket.family), n, colp, len(cols), int(bucket.dtype_bytes),
                                              int(bucket.hq), int(bucket.hkv), int(bucket.head_dim), sp, ns,

@@ -24,7 +24,7 @@ import numpy as np
 # which declares its own copy)
 FAM_GEMM, FAM_GROUPED, FAM_ATTN, FAM_ELEMWISE, FAM_ALLREDUCE = 0, 1, 2, 3, 4
 FAM_NAMES = {0: "gemm", 1: "grouped_gemm", 2: "attention", 3: "elementwise", 4: "allreduce"}
-TIER_NONE, TIER_A, TIER_B = 0, 1, 2
+TIER_NONE, TIER_A, TIER_B, TIER_B_ROUTED = 0, 1, 2, 3
 # elementwise sub-operations (reading Q1)
 SUB_RMSNORM, SUB_SILU_MUL, SUB_ROPE, SUB_KV_WRITE, SUB_EMBED, SUB_RESADD = 0, 1, 2, 3, 4, 5
 N_EXPERTS = 8
@@ -262,8 +262,10 @@ def _grid_queries(rng, n: int, lo, hi):
     return np.maximum(np.rint(np.exp2(x)), 1.0).astype(np.int64)
 
 
-def config3(n: int = 4_194_304, seed: int = 2) -> Workload:
-    """Tier B: GEMM/attention queries against 32^3 measured-efficiency grids, 10% OOB (clamped)."""
+def config3(n: int = 4_194_304, seed: int = 2, routed: bool = False, n_in: int = 12, h: int = 128) -> Workload:
+    """Tier B: GEMM/attention queries against 32^3 measured-efficiency grids, 10% OOB (clamped).
+    routed=True (not a BASELINE.json config): the 10 % out-of-hull queries fall
+    back to per-family Tier-A heads (cfg-2-sized, seed 1) instead of being clamped."""
     rng = _rng(seed)
     ng = n // 2
     na = n - ng
@@ -276,7 +278,12 @@ def config3(n: int = 4_194_304, seed: int = 2) -> Workload:
     n_steps = max(1, n // 256)
     for b in buckets:
         b.step_off = uniform_step_offsets(rng, b.n, n_steps)
-    return Workload("cfg3_tierB_4M", buckets, [spec_gb200()], TIER_B, grids=grids,
+    heads = {}
+    if routed:
+        hr = _rng(1)
+        heads = {f: make_head(hr, n_in, h) for f in (FAM_GEMM, FAM_ATTN)}
+    return Workload("cfg3_tierB_routed" if routed else "cfg3_tierB_4M", buckets, [spec_gb200()],
+                    TIER_B_ROUTED if routed else TIER_B, grids=grids, heads=heads,
                     n_steps=n_steps, cfg_off=cfg_offsets(rng, n_steps, min(16, n_steps)),
                     step_params=dict(STEP_PARAMS_ZERO), seed=seed)
 
