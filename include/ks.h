@@ -48,7 +48,7 @@ typedef struct ks_ctx ks_ctx;   /* opaque; owns device copies of heads and grids
 typedef enum { KS_OK = 0, KS_EINVAL = 1, KS_ENOMEM = 2, KS_ECUDA = 3, KS_ESTATE = 4, KS_EUNSUPPORTED = 5 } ks_status;
 typedef enum { KS_FAM_GEMM = 0, KS_FAM_GROUPED_GEMM = 1, KS_FAM_ATTN = 2, KS_FAM_ELEMWISE = 3, KS_FAM_ALLREDUCE = 4,
                KS_FAM_COUNT = 5 } ks_family;
-typedef enum { KS_TIER_NONE = 0, KS_TIER_A = 1, KS_TIER_B = 2 } ks_tier;
+typedef enum { KS_TIER_NONE = 0, KS_TIER_A = 1, KS_TIER_B = 2, KS_TIER_B_ROUTED = 3 } ks_tier;
 typedef enum { KS_COL_I32 = 0, KS_COL_F32 = 1 } ks_col_dtype;   /* F32 columns must hold exact integers < 2^24 */
 typedef enum { KS_MEM_DEVICE = 0, KS_MEM_HOST = 1 } ks_mem_space;
 
@@ -130,7 +130,11 @@ KS_API ks_status ks_load_grid(ks_ctx *ctx, ks_family family, const int32_t dims[
 /* Predict the latency of every (spec, descriptor) pair (steps S1-S5 of DESIGN.md §1).
  *   batches[n_batches]   family buckets (<= KS_MAX_BATCHES)
  *   specs[n_specs]       hardware-spec vectors (host)
- *   tier                 KS_TIER_NONE (e = 1), KS_TIER_A (heads), KS_TIER_B (grids, clamped)
+ *   tier                 KS_TIER_NONE (e = 1), KS_TIER_A (heads), KS_TIER_B (grids, clamped),
+ *                        KS_TIER_B_ROUTED (density routing: the grid inside the measured hull,
+ *                        the family's Tier-A head outside it; needs both loaded.  The hull is the grid's
+ *                        box, decided on integers: ceil(2^lo_a) <= v_a <= floor(2^hi_a) on every axis with
+ *                        more than one node, Q16.  Uses 4 bytes per row of library workspace.)
  *   latency[b]           out, fp32 [n_specs][batches[b].n] seconds
  *   tiles[b], waves[b]   optional out (array pointer or entry may be NULL), int32 [n_specs][n]:
  *                        CTA count B and wave count W = ceil(B/S)

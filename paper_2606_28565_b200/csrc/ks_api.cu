@@ -172,7 +172,7 @@ ks_status validate_batches(const ks_ctx* c, const ks_desc_batch* batches, int n_
   if (n_batches < 0 || n_batches > KS_MAX_BATCHES || n_specs < 0) return KS_EINVAL;
   if (n_batches > 0 && !batches) return KS_EINVAL;
   if (n_specs > 0 && !specs) return KS_EINVAL;
-  if (tier != KS_TIER_NONE && tier != KS_TIER_A && tier != KS_TIER_B) return KS_EINVAL;
+  if (tier != KS_TIER_NONE && tier != KS_TIER_A && tier != KS_TIER_B && tier != KS_TIER_B_ROUTED) return KS_EINVAL;
   for (int s = 0; s < n_specs; ++s)
     if (!spec_ok(specs[s])) return KS_EINVAL;
   for (int b = 0; b < n_batches; ++b) {
@@ -188,8 +188,8 @@ ks_status validate_batches(const ks_ctx* c, const ks_desc_batch* batches, int n_
         if (device_ptrs && !aligned16(k.cols[col])) return KS_EINVAL;
       }
     if (k.family == KS_FAM_ALLREDUCE) continue;               // Eq. 3 needs neither head nor grid
-    if (tier == KS_TIER_A && !c->heads[k.family].loaded) return KS_ESTATE;
-    if (tier == KS_TIER_B && !c->grids[k.family].loaded) return KS_ESTATE;
+    if ((tier == KS_TIER_A || tier == KS_TIER_B_ROUTED) && !c->heads[k.family].loaded) return KS_ESTATE;
+    if ((tier == KS_TIER_B || tier == KS_TIER_B_ROUTED) && !c->grids[k.family].loaded) return KS_ESTATE;
   }
   return KS_OK;
 }
@@ -221,20 +221,57 @@ KsBucketDev make_bucket_dev(const ks_desc_batch& k, const void* const* cols, con
   return d;
 }
 
+// Density routing scratch: per bucket a row list (n ints) and its length (one int, in its own 256-byte slot).
+struct RouteBuf {
+  int32_t* idx = nullptr;
+  int32_t* count = nullptr;
+};
+size_t route_need(const ks_desc_batch* batches, int n_batches, int tier) {
+  size_t need = 0;
+  if (tier != KS_TIER_B_ROUTED) return 0;
+  for (int b = 0; b < n_batches; ++b)
+    if (batches[b].family != KS_FAM_ALLREDUCE) need += align_up((size_t)batches[b].n * 4, 256) + 256;
+  return need;
+}
+void route_take(ks_ctx* c, const ks_desc_batch* batches, int n_batches, int tier, RouteBuf* rb) {
+  for (int b = 0; b < n_batches; ++b) {
+    rb[b] = RouteBuf();
+    if (tier != KS_TIER_B_ROUTED || batches[b].family == KS_FAM_ALLREDUCE) continue;
+    rb[b].idx = static_cast<int32_t*>(ws_take(c, (size_t)batches[b].n * 4));
+    rb[b].count = static_cast<int32_t*>(ws_take(c, 4));
+  }
+}
+
 // Enqueue S1-S5 for device-resident columns/outputs.  Arguments are already validated.
+// tier == KS_TIER_B_ROUTED: pass 1 = the Tier-B kernel on every row, which also lists
+// the rows outside the measured hull in rb[b]; pass 2 = the family's Tier-A head (tcgen05 MLP kernel
+// or bounded form) on that row list, overwriting those rows' latencies.
 ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* const (*cols)[KS_MAX_COLS], int n_batches,
-                         const ks_hw_spec* specs, int n_specs, int tier, const DevOut* outs) {
+                         const ks_hw_spec* specs, int n_specs, int tier_in, const DevOut* outs,
+                         const RouteBuf* rb = nullptr) {
+  const bool routed = tier_in == KS_TIER_B_ROUTED;
+  if (routed && !rb) return KS_EINVAL;
+  for (int pass = 0; pass < (routed ? 2 : 1); ++pass) {
+  const int tier = routed ? (pass == 0 ? KS_TIER_B : KS_TIER_A) : tier_in;
+  const bool lists = routed && pass == 1;
   for (int s0 = 0; s0 < n_specs; s0 += KS_MAX_SPECS_PER_LAUNCH) {
     const int ns = n_specs - s0 < KS_MAX_SPECS_PER_LAUNCH ? n_specs - s0 : KS_MAX_SPECS_PER_LAUNCH;
     for (int b = 0; b < n_batches; ++b) {               // streaming kernels: Tier NONE / B, and Eq. 3 rows under any tier
       const bool ar = batches[b].family == KS_FAM_ALLREDUCE;
+      if (ar && lists) continue;                        // Eq. 3 rows were finished by pass 1
       const bool bnd = tier == KS_TIER_A && !ar && c->heads[batches[b].family].bounded;
       if (batches[b].n == 0 || (tier == KS_TIER_A && !ar && !bnd)) continue;
       {
         KsStreamParams p;
         memset(&p, 0, sizeof(p));
         p.bk = make_bucket_dev(batches[b], cols[b], outs[b], s0);
+        if (lists) { p.bk.idx = rb[b].idx; p.bk.count = rb[b].count; }
         if (tier == KS_TIER_B && !ar) p.grid = c->grids[batches[b].family].dev;
+        if (routed && pass == 0 && !ar && s0 == 0) {    // the hull test depends on the row only: list it once
+          KS_CUDA(c, cudaMemsetAsync(rb[b].count, 0, 4, c->stream));
+          p.grid.route_idx = rb[b].idx;
+          p.grid.route_count = rb[b].count;
+        }
         p.n_specs = ns;
         p.tier = ar ? KS_TIER_NONE : bnd ? KS_TIER_BOUNDED : tier;
         if (bnd) p.bounded = c->heads[batches[b].family].bw;
@@ -260,6 +297,7 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
           const HeadState& hq = c->heads[batches[q].family];
           if (hq.n_in != h0.n_in || hq.h != h0.h) continue;
           p.bk[nb] = make_bucket_dev(batches[q], cols[q], outs[q], s0);
+          if (lists) { p.bk[nb].idx = rb[q].idx; p.bk[nb].count = rb[q].count; }
           p.head[nb].w1_img = hq.w1_img;
           p.head[nb].w2_img = hq.w2_img;
           p.head[nb].w3 = hq.w3;
@@ -279,6 +317,7 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
         c->launches += 1;
       }
     }
+  }
   }
   return KS_OK;
 }
@@ -463,7 +502,15 @@ ks_status ks_load_grid(ks_ctx* c, ks_family family, const int32_t dims[3], const
     g.dev.stride[a] = dims[a] > 1 ? strides[a] : 0;
     g.dev.lo[a] = lo_log2[a];
     g.dev.scale[a] = dims[a] > 1 ? (float)((double)(dims[a] - 1) / ((double)hi_log2[a] - (double)lo_log2[a])) : 0.0f;
+    // the measured hull on integers (density routing, Q16): ceil(2^lo) <= v <= floor(2^hi); a flat axis is unconstrained
+    double vmin = dims[a] > 1 ? ceil(exp2((double)lo_log2[a])) : -2147483648.0;
+    double vmax = dims[a] > 1 ? floor(exp2((double)hi_log2[a])) : 2147483647.0;
+    if (dims[a] > 1 && vmin < 1.0) vmin = 1.0;                      // a non-positive axis value is outside
+    g.dev.vmin[a] = (int32_t)fmax(vmin, -2147483648.0);
+    g.dev.vmax[a] = (int32_t)fmin(vmax, 2147483647.0);
   }
+  g.dev.route_idx = nullptr;
+  g.dev.route_count = nullptr;
   g.values = d;
   g.loaded = true;
   return KS_OK;
@@ -567,7 +614,13 @@ ks_status ks_predict_kernels(ks_ctx* c, const ks_desc_batch* batches, int n_batc
       outs[b].waves = waves ? waves[b] : nullptr;
       outs[b].troof = t_roof ? t_roof[b] : nullptr;
     }
-    return predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+    RouteBuf rb[KS_MAX_BATCHES];
+    if (tier == KS_TIER_B_ROUTED) {                  // the row lists live in the library workspace (stream-ordered reuse)
+      st = ws_reserve(c, route_need(batches, n_batches, tier));
+      if (st != KS_OK) return st;
+      route_take(c, batches, n_batches, tier, rb);
+    }
+    return predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs, rb);
   }
   // host space: stage through the workspace
   size_t need = 0;
@@ -578,8 +631,11 @@ ks_status ks_predict_kernels(ks_ctx* c, const ks_desc_batch* batches, int n_batc
     if (waves && waves[b]) need += o;
     if (t_roof && t_roof[b]) need += o;
   }
+  need += route_need(batches, n_batches, tier);
   st = ws_reserve(c, need);
   if (st != KS_OK) return st;
+  RouteBuf rb[KS_MAX_BATCHES];
+  route_take(c, batches, n_batches, tier, rb);
   for (int b = 0; b < n_batches; ++b) {
     const size_t n = batches[b].n, ob = n * (size_t)n_specs * 4;
     for (int k = 0; k < batches[b].n_cols; ++k) {
@@ -592,7 +648,7 @@ ks_status ks_predict_kernels(ks_ctx* c, const ks_desc_batch* batches, int n_batc
     if (waves && waves[b]) outs[b].waves = static_cast<int32_t*>(ws_take(c, ob));
     if (t_roof && t_roof[b]) outs[b].troof = static_cast<float*>(ws_take(c, ob));
   }
-  st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+  st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs, rb);
   if (st != KS_OK) return st;
   for (int b = 0; b < n_batches; ++b) {
     const size_t ob = (size_t)batches[b].n * n_specs * 4;
@@ -678,8 +734,11 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   if (!dev)
     need += align_up((size_t)(n_cfg + 1) * 4, 256) + align_up((size_t)n_steps * n_specs * 4, 256) +
             align_up((size_t)n_cfg * n_specs * 4 + 4, 256);
+  need += route_need(batches, n_batches, tier);
   st = ws_reserve(c, need);
   if (st != KS_OK) return st;
+  RouteBuf rb[KS_MAX_BATCHES];
+  route_take(c, batches, n_batches, tier, rb);
 
   const void* cols[KS_MAX_BATCHES][KS_MAX_COLS] = {};
   DevOut outs[KS_MAX_BATCHES];
@@ -694,7 +753,7 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
       doff[b] = step_off[b];
     }
     if (n_specs > 0 && n_batches > 0) {
-      st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs);
+      st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs, rb);
       if (st != KS_OK) return st;
     }
     return compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg, step_latency,
@@ -731,7 +790,7 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   for (int b = 0; b < n_batches; ++b) {
     KS_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[b], 0));
     if (n_specs > 0 && batches[b].n > 0) {
-      st = predict_device(c, batches + b, cols + b, 1, specs, n_specs, tier, outs + b);
+      st = predict_device(c, batches + b, cols + b, 1, specs, n_specs, tier, outs + b, rb + b);
       if (st != KS_OK) return st;
     }
     const size_t ob = (size_t)batches[b].n * n_specs * 4;

@@ -43,6 +43,10 @@ struct KsBucketDev {
   float* troof;        // optional
   int32_t family, n, col_f32, s;
   int32_t hq, hkv, hd, n_cols;
+  // density routing (KS_TIER_B_ROUTED): when idx != nullptr the kernel works on the row LIST
+  // idx[0 .. *count) instead of rows 0 .. n (outputs still go to the listed rows' own slots)
+  const int32_t* idx;
+  const int32_t* count;
 };
 
 // Tier-B grid constants
@@ -54,6 +58,9 @@ struct KsGridDev {
   int32_t pad;
   float lo[3];
   float scale[3];        // (dims-1)/(hi-lo); 0 for a flat axis
+  int32_t vmin[3], vmax[3];   // the hull on integers: ceil(2^lo) <= v <= floor(2^hi) (INT_MIN/INT_MAX on a flat axis)
+  int32_t* route_idx;    // KS_TIER_B_ROUTED pass 1: out-of-hull rows are appended here ...
+  int32_t* route_count;  // ... at *route_count (zeroed before the launch); nullptr = plain Tier B
 };
 
 // ------------------------------------------------------------------ S1: descriptor decode

@@ -7,7 +7,7 @@ struct KsSpecTable {
 };
 
 // ---- streaming kernels (Tier NONE / Tier B): ks_stream.cu
-#define KS_TIER_BOUNDED 3    // internal: Tier A with the bounded analytical head (streaming kernel)
+#define KS_TIER_BOUNDED 100  // internal: Tier A with the bounded analytical head (streaming kernel)
 #define KS_BOUNDED_NF 22    // real features of the largest feature vector (Q2: 22..31 are zero)
 struct KsBoundedDev {
   float w_gamma[KS_BOUNDED_NF], w_alpha[KS_BOUNDED_NF];   // zero beyond the head's n_in

@@ -53,6 +53,27 @@ KS_DEV float feature_row(const int* v, const KsBucketDev& bk, const KsSpecDev& s
   return rf.t_roof;
 }
 
+// Tile bookkeeping of a launch, computed in the kernel: a bucket may be a row LIST whose length is
+// only known on the device (density routing: idx[0 .. *count)), so the tile prefix cannot come from
+// the host.  ne[b] = rows (or list entries) of bucket b, tb[b] = first 128-row tile of bucket b.
+struct TileMap {
+  int tb[KS_MLP_MAX_BUCKETS + 1];
+  int ne[KS_MLP_MAX_BUCKETS];
+};
+KS_DEV void tile_map_init(const KsMlpParams& p, TileMap* tm) {   // one thread
+  int t = 0;
+  for (int b = 0; b < p.n_buckets; ++b) {
+    int n = p.bk[b].n;
+    if (p.bk[b].count) { const int c = __ldg(p.bk[b].count); n = c < n ? c : n; }
+    tm->ne[b] = n;
+    tm->tb[b] = t;
+    t += (n + kRows - 1) / kRows;
+  }
+  for (int b = p.n_buckets; b <= KS_MLP_MAX_BUCKETS; ++b) tm->tb[b] = t;
+}
+// position i of a bucket -> descriptor row (identity unless the bucket is a row list)
+KS_DEV int map_row(const KsBucketDev& bk, int i) { return bk.idx ? __ldg(bk.idx + i) : i; }
+
 // raw 32-bit column load (int32 or fp32 bits); converted at the point of use so a prefetch does
 // not stall on the conversion
 KS_DEV int load_col_raw(const void* col, int i) { return __ldg((const int*)col + i); }

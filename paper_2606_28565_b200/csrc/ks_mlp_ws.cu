@@ -57,7 +57,7 @@ struct WsCfg {
   static constexpr int OFF_W3 = OFF_A2 + 2 * A2_BYTES;                 // [KS_MLP_MAX_BUCKETS][H] fp32
   static constexpr int OFF_RING = OFF_W3 + KS_MLP_MAX_BUCKETS * H * 4; // [kRing][128] fp32 t_roof
   static constexpr int OFF_BAR = OFF_RING + kRing * kRows * 4;
-  static constexpr int SMEM_BYTES = OFF_BAR + 128;
+  static constexpr int SMEM_BYTES = OFF_BAR + 192;   // barriers + TMEM slot (128) + TileMap
   static constexpr int NCHUNK = H / 32;
 };
 
@@ -66,42 +66,45 @@ enum { BAR_W = 0, BAR_DRAIN = 1, BAR_A1_FULL = 2, BAR_MMA1 = 4, BAR_A2_FULL = 6,
        BAR_D1_FREE = 12, BAR_COUNT = 14 };
 
 struct Range { int lo, hi; };
-KS_DEV Range bucket_range(const KsMlpParams& p, int b, int t_lo, int t_hi) {
+KS_DEV Range bucket_range(const TileMap& tm, int b, int t_lo, int t_hi) {
   Range r;
-  r.lo = t_lo > p.tile_begin[b] ? t_lo : p.tile_begin[b];
-  r.hi = t_hi < p.tile_begin[b + 1] ? t_hi : p.tile_begin[b + 1];
+  r.lo = t_lo > tm.tb[b] ? t_lo : tm.tb[b];
+  r.hi = t_hi < tm.tb[b + 1] ? t_hi : tm.tb[b + 1];
   return r;
 }
 
 // ------------------------------------------------------------------ PRODUCER (warps 0-3)
 template <int NIN, int H, int FAM>
-KS_DEV void producer_bucket(const KsMlpParams& p, const int b, const Range tr, unsigned char* smem, uint64_t* bars,
-                            uint32_t& q) {
+KS_DEV void producer_bucket(const KsMlpParams& p, const TileMap& tm, const int b, const Range tr, unsigned char* smem,
+                            uint64_t* bars, uint32_t& q) {
   using C = WsCfg<NIN, H>;
   constexpr int NC = NCols<FAM>::v;
   const int r = threadIdx.x;                       // 0..127: row within the tile
   const KsBucketDev& bk = p.bk[b];
-  const int tile0 = p.tile_begin[b];
+  const int tile0 = tm.tb[b], ne = tm.ne[b];
   const bool f32cols = bk.col_f32 != 0;
   float* ring = reinterpret_cast<float*>(smem + C::OFF_RING);
 
   int vn[NC];
+  int row_next;                                    // descriptor row whose columns sit in vn
   {
-    const int row = (tr.lo - tile0) * kRows + r;
+    const int pos = (tr.lo - tile0) * kRows + r;
+    row_next = pos < ne ? map_row(bk, pos) : 0;
 #pragma unroll
-    for (int c = 0; c < NC; ++c) vn[c] = row < bk.n ? load_col_raw(bk.cols[c], row) : 0;
+    for (int c = 0; c < NC; ++c) vn[c] = pos < ne ? load_col_raw(bk.cols[c], row_next) : 0;
   }
   for (int t = tr.lo; t < tr.hi; ++t) {
-    const int row = (t - tile0) * kRows + r;
-    const bool valid = row < bk.n;
+    const int pos = (t - tile0) * kRows + r;
+    const bool valid = pos < ne;
+    const int row = row_next;                        // descriptor row of this list position
     int v[NC];
 #pragma unroll
     for (int c = 0; c < NC; ++c) v[c] = col_value(vn[c], f32cols);
     {
-      const int rown = row + kRows;
-      const bool ok = t + 1 < tr.hi && rown < bk.n;
+      const bool ok = t + 1 < tr.hi && pos + kRows < ne;
+      row_next = ok ? map_row(bk, pos + kRows) : 0;
 #pragma unroll
-      for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], rown) : 0;
+      for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], row_next) : 0;
     }
     for (int s = 0; s < p.n_specs; ++s, ++q) {
       const KsSpecDev& sp = p.specs.s[s];
@@ -182,8 +185,8 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
 
 // ------------------------------------------------------------------ EPI2 (warps 12-19): D2 -> 2 GELU . w3/2 -> latency
 template <int NIN, int H, int GM>
-KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
-                     const uint32_t tmem_base) {
+KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
+                     uint64_t* bars, const uint32_t tmem_base) {
   using C = WsCfg<NIN, H>;
   const int e = threadIdx.x - (kProducerWarps + kEpiWarps) * 32;
   const uint32_t grp = (uint32_t)e >> 7;
@@ -192,14 +195,15 @@ KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsig
   const float* ring = reinterpret_cast<const float*>(smem + C::OFF_RING);
   uint32_t q = 0;
   for (int b = 0; b < p.n_buckets; ++b) {
-    const Range tr = bucket_range(p, b, t_lo, t_hi);
+    const Range tr = bucket_range(tm, b, t_lo, t_hi);
     const KsBucketDev& bk = p.bk[b];
     const float* sw3 = reinterpret_cast<const float*>(smem + C::OFF_W3) + b * H;
     const float b3 = p.head[b].b3;
-    const int tile0 = p.tile_begin[b];
+    const int tile0 = tm.tb[b], ne = tm.ne[b];
     for (int t = tr.lo; t < tr.hi; ++t) {
-      const int row = (t - tile0) * kRows + r;
-      const bool valid = row < bk.n;
+      const int pos = (t - tile0) * kRows + r;
+      const bool valid = pos < ne;
+      const int row = valid ? map_row(bk, pos) : 0;
       for (int s = 0; s < p.n_specs; ++s, ++q) {
         if ((q & 1u) != grp) continue;
         const uint32_t buf = q & 1u, par = (q >> 1) & 1u;
@@ -257,8 +261,8 @@ KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsig
 
 // ------------------------------------------------------------------ MMA issuer (one thread of warp 20)
 template <int NIN, int H>
-KS_DEV void mma_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
-                    const uint32_t tmem_base) {
+KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
+                    uint64_t* bars, const uint32_t tmem_base) {
   using C = WsCfg<NIN, H>;
   constexpr uint32_t idesc = ks_umma_idesc_bf16(128, H);
   constexpr uint32_t B_LBO = H * 16;
@@ -304,7 +308,7 @@ KS_DEV void mma_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsign
   };
 
   for (int b = 0; b < p.n_buckets; ++b) {
-    const Range tr = bucket_range(p, b, t_lo, t_hi);
+    const Range tr = bucket_range(tm, b, t_lo, t_hi);
     if (tr.lo >= tr.hi) continue;
     if (q > 0u) {                                   // every MMA that reads the previous family's weights is done
       ks_umma_commit(bars + BAR_DRAIN);
@@ -341,9 +345,11 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + BAR_COUNT);
+  TileMap* tmp = reinterpret_cast<TileMap*>(smem + C::OFF_BAR + 128);
   const int tid = threadIdx.x;
   const int warp = tid >> 5;
 
+  if (tid == 32) tile_map_init(p, tmp);
   if (tid == 0) {
     ks_mbar_init(bars + BAR_W, 1);
     ks_mbar_init(bars + BAR_DRAIN, 1);
@@ -369,31 +375,32 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
   __syncthreads();
   ks_tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  const TileMap& tm = *tmp;
 
-  const long long total = p.tile_begin[p.n_buckets];
+  const long long total = tm.tb[p.n_buckets];
   const int t_lo = (int)((long long)blockIdx.x * total / gridDim.x);
   const int t_hi = (int)((long long)(blockIdx.x + 1) * total / gridDim.x);
 
   if (warp < kProducerWarps) {
     uint32_t q = 0;
     for (int b = 0; b < p.n_buckets; ++b) {
-      const Range tr = bucket_range(p, b, t_lo, t_hi);
+      const Range tr = bucket_range(tm, b, t_lo, t_hi);
       if (tr.lo >= tr.hi) continue;
       switch (p.bk[b].family) {
-        case KS_FAM_GEMM: producer_bucket<NIN, H, KS_FAM_GEMM>(p, b, tr, smem, bars, q); break;
-        case KS_FAM_GROUPED_GEMM: producer_bucket<NIN, H, KS_FAM_GROUPED_GEMM>(p, b, tr, smem, bars, q); break;
-        case KS_FAM_ATTN: producer_bucket<NIN, H, KS_FAM_ATTN>(p, b, tr, smem, bars, q); break;
-        default: producer_bucket<NIN, H, KS_FAM_ELEMWISE>(p, b, tr, smem, bars, q); break;
+        case KS_FAM_GEMM: producer_bucket<NIN, H, KS_FAM_GEMM>(p, tm, b, tr, smem, bars, q); break;
+        case KS_FAM_GROUPED_GEMM: producer_bucket<NIN, H, KS_FAM_GROUPED_GEMM>(p, tm, b, tr, smem, bars, q); break;
+        case KS_FAM_ATTN: producer_bucket<NIN, H, KS_FAM_ATTN>(p, tm, b, tr, smem, bars, q); break;
+        default: producer_bucket<NIN, H, KS_FAM_ELEMWISE>(p, tm, b, tr, smem, bars, q); break;
       }
     }
   } else if (warp < kProducerWarps + kEpiWarps) {
     if (p.gelu_mode == 0) epi1_items<NIN, H, 0>(p, (uint32_t)(t_hi - t_lo) * (uint32_t)p.n_specs, smem, bars, tmem_base);
     else epi1_items<NIN, H, 1>(p, (uint32_t)(t_hi - t_lo) * (uint32_t)p.n_specs, smem, bars, tmem_base);
   } else if (warp < kMmaWarp) {
-    if (p.gelu_mode == 0) epi2_all<NIN, H, 0>(p, t_lo, t_hi, smem, bars, tmem_base);
-    else epi2_all<NIN, H, 1>(p, t_lo, t_hi, smem, bars, tmem_base);
+    if (p.gelu_mode == 0) epi2_all<NIN, H, 0>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    else epi2_all<NIN, H, 1>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   } else if (tid == kMmaWarp * 32) {
-    mma_all<NIN, H>(p, t_lo, t_hi, smem, bars, tmem_base);
+    mma_all<NIN, H>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   }
   ks_tc_fence_before();
   __syncthreads();

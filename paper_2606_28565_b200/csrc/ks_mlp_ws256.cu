@@ -59,43 +59,46 @@ enum { BAR_W = 0, BAR_DRAIN, BAR_A1_FULL, BAR_MMA1, BAR_D1_FREE, BAR_MMA2, BAR_D
        BAR_A2_FREE = BAR_A2_FULL + kGroups, BAR_COUNT = BAR_A2_FREE + kGroups };
 
 struct Range { int lo, hi; };
-KS_DEV Range bucket_range(const KsMlpParams& p, int b, int t_lo, int t_hi) {
+KS_DEV Range bucket_range(const TileMap& tm, int b, int t_lo, int t_hi) {
   Range r;
-  r.lo = t_lo > p.tile_begin[b] ? t_lo : p.tile_begin[b];
-  r.hi = t_hi < p.tile_begin[b + 1] ? t_hi : p.tile_begin[b + 1];
+  r.lo = t_lo > tm.tb[b] ? t_lo : tm.tb[b];
+  r.hi = t_hi < tm.tb[b + 1] ? t_hi : tm.tb[b + 1];
   return r;
 }
 
 // ------------------------------------------------------------------ PRODUCER (warps 0-3)
 template <int NIN, int FAM>
-KS_DEV void producer_bucket(const KsMlpParams& p, const int b, const Range tr, unsigned char* smem, uint64_t* bars,
-                            uint32_t& q) {
+KS_DEV void producer_bucket(const KsMlpParams& p, const TileMap& tm, const int b, const Range tr, unsigned char* smem,
+                            uint64_t* bars, uint32_t& q) {
   using C = Cfg256<NIN>;
   constexpr int NC = NCols<FAM>::v;
   const int r = threadIdx.x;
   const KsBucketDev& bk = p.bk[b];
-  const int tile0 = p.tile_begin[b];
+  const int tile0 = tm.tb[b], ne = tm.ne[b];
   const bool f32cols = bk.col_f32 != 0;
   float* ring = reinterpret_cast<float*>(smem + C::OFF_RING);
   unsigned char* A1 = smem + C::OFF_A1;
 
   int vn[NC];
+  int row_next;                                    // descriptor row whose columns sit in vn
   {
-    const int row = (tr.lo - tile0) * kRows + r;
+    const int pos = (tr.lo - tile0) * kRows + r;
+    row_next = pos < ne ? map_row(bk, pos) : 0;
 #pragma unroll
-    for (int c = 0; c < NC; ++c) vn[c] = row < bk.n ? load_col_raw(bk.cols[c], row) : 0;
+    for (int c = 0; c < NC; ++c) vn[c] = pos < ne ? load_col_raw(bk.cols[c], row_next) : 0;
   }
   for (int t = tr.lo; t < tr.hi; ++t) {
-    const int row = (t - tile0) * kRows + r;
-    const bool valid = row < bk.n;
+    const int pos = (t - tile0) * kRows + r;
+    const bool valid = pos < ne;
+    const int row = row_next;                        // descriptor row of this list position
     int v[NC];
 #pragma unroll
     for (int c = 0; c < NC; ++c) v[c] = col_value(vn[c], f32cols);
     {
-      const int rown = row + kRows;
-      const bool ok = t + 1 < tr.hi && rown < bk.n;
+      const bool ok = t + 1 < tr.hi && pos + kRows < ne;
+      row_next = ok ? map_row(bk, pos + kRows) : 0;
 #pragma unroll
-      for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], rown) : 0;
+      for (int c = 0; c < NC; ++c) vn[c] = ok ? load_col_raw(bk.cols[c], row_next) : 0;
     }
     for (int s = 0; s < p.n_specs; ++s, ++q) {
       const KsSpecDev& sp = p.specs.s[s];
@@ -175,8 +178,8 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
 
 // ------------------------------------------------------------------ EPI2 (warps 12-19)
 template <int NIN, int GM>
-KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
-                     const uint32_t tmem_base) {
+KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
+                     uint64_t* bars, const uint32_t tmem_base) {
   using C = Cfg256<NIN>;
   const int e = threadIdx.x - (kProducerWarps + kEpiWarps) * 32;   // 0..255
   const int wg = e >> 7;
@@ -189,7 +192,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsig
   const uint32_t d2 = tmem_base + (uint32_t)H + lane_off + (uint32_t)(wg * 128);
   uint32_t q = 0;
   for (int b = 0; b < p.n_buckets; ++b) {
-    const Range tr = bucket_range(p, b, t_lo, t_hi);
+    const Range tr = bucket_range(tm, b, t_lo, t_hi);
     if (tr.lo >= tr.hi) continue;
     const KsBucketDev& bk = p.bk[b];
     // this family's layer-3 weights and layer-2 bias (all 256 EPI2 threads; nobody still reads the old ones)
@@ -198,10 +201,11 @@ KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsig
     sb2[e] = __ldg(p.head[b].b2 + e);
     ks_bar_sync(2, 2 * 128);
     const float b3 = p.head[b].b3;
-    const int tile0 = p.tile_begin[b];
+    const int tile0 = tm.tb[b], ne = tm.ne[b];
     for (int t = tr.lo; t < tr.hi; ++t) {
-      const int row = (t - tile0) * kRows + r;
-      const bool valid = row < bk.n;
+      const int pos = (t - tile0) * kRows + r;
+      const bool valid = pos < ne;
+      const int row = valid ? map_row(bk, pos) : 0;
       for (int s = 0; s < p.n_specs; ++s, ++q) {
         ks_mbar_wait(bars + BAR_MMA2, q & 1u);                      // D2 holds item q
         ks_tc_fence_after();
@@ -262,8 +266,8 @@ KS_DEV void epi2_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsig
 
 // ------------------------------------------------------------------ MMA issuer (one thread of warp 20)
 template <int NIN>
-KS_DEV void mma_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsigned char* smem, uint64_t* bars,
-                    const uint32_t tmem_base) {
+KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
+                    uint64_t* bars, const uint32_t tmem_base) {
   using C = Cfg256<NIN>;
   constexpr uint32_t idesc = ks_umma_idesc_bf16(128, H);
   constexpr uint32_t B_LBO = H * 16;
@@ -301,7 +305,7 @@ KS_DEV void mma_all(const KsMlpParams& p, const int t_lo, const int t_hi, unsign
   };
 
   for (int b = 0; b < p.n_buckets; ++b) {
-    const Range tr = bucket_range(p, b, t_lo, t_hi);
+    const Range tr = bucket_range(tm, b, t_lo, t_hi);
     if (tr.lo >= tr.hi) continue;
     if (q > 0u) {                                   // every MMA that reads the previous family's weights is done
       ks_umma_commit(bars + BAR_DRAIN);
@@ -336,9 +340,11 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + BAR_COUNT);
+  TileMap* tmp = reinterpret_cast<TileMap*>(smem + C::OFF_BAR + 128);
   const int tid = threadIdx.x;
   const int warp = tid >> 5;
 
+  if (tid == 32) tile_map_init(p, tmp);
   if (tid == 0) {
     ks_mbar_init(bars + BAR_W, 1);
     ks_mbar_init(bars + BAR_DRAIN, 1);
@@ -358,21 +364,22 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
   __syncthreads();
   ks_tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  const TileMap& tm = *tmp;
 
-  const long long total = p.tile_begin[p.n_buckets];
+  const long long total = tm.tb[p.n_buckets];
   const int t_lo = (int)((long long)blockIdx.x * total / gridDim.x);
   const int t_hi = (int)((long long)(blockIdx.x + 1) * total / gridDim.x);
 
   if (warp < kProducerWarps) {
     uint32_t q = 0;
     for (int b = 0; b < p.n_buckets; ++b) {
-      const Range tr = bucket_range(p, b, t_lo, t_hi);
+      const Range tr = bucket_range(tm, b, t_lo, t_hi);
       if (tr.lo >= tr.hi) continue;
       switch (p.bk[b].family) {
-        case KS_FAM_GEMM: producer_bucket<NIN, KS_FAM_GEMM>(p, b, tr, smem, bars, q); break;
-        case KS_FAM_GROUPED_GEMM: producer_bucket<NIN, KS_FAM_GROUPED_GEMM>(p, b, tr, smem, bars, q); break;
-        case KS_FAM_ATTN: producer_bucket<NIN, KS_FAM_ATTN>(p, b, tr, smem, bars, q); break;
-        default: producer_bucket<NIN, KS_FAM_ELEMWISE>(p, b, tr, smem, bars, q); break;
+        case KS_FAM_GEMM: producer_bucket<NIN, KS_FAM_GEMM>(p, tm, b, tr, smem, bars, q); break;
+        case KS_FAM_GROUPED_GEMM: producer_bucket<NIN, KS_FAM_GROUPED_GEMM>(p, tm, b, tr, smem, bars, q); break;
+        case KS_FAM_ATTN: producer_bucket<NIN, KS_FAM_ATTN>(p, tm, b, tr, smem, bars, q); break;
+        default: producer_bucket<NIN, KS_FAM_ELEMWISE>(p, tm, b, tr, smem, bars, q); break;
       }
     }
   } else if (warp < kProducerWarps + kEpiWarps) {
@@ -380,10 +387,10 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
     if (p.gelu_mode == 0) epi1_items<NIN, 0>(p, n_items, smem, bars, tmem_base);
     else epi1_items<NIN, 1>(p, n_items, smem, bars, tmem_base);
   } else if (warp < kMmaWarp) {
-    if (p.gelu_mode == 0) epi2_all<NIN, 0>(p, t_lo, t_hi, smem, bars, tmem_base);
-    else epi2_all<NIN, 1>(p, t_lo, t_hi, smem, bars, tmem_base);
+    if (p.gelu_mode == 0) epi2_all<NIN, 0>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    else epi2_all<NIN, 1>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   } else if (tid == kMmaWarp * 32) {
-    mma_all<NIN>(p, t_lo, t_hi, smem, bars, tmem_base);
+    mma_all<NIN>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   }
   ks_tc_fence_before();
   __syncthreads();

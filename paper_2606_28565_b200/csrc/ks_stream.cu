@@ -81,6 +81,33 @@ KS_DEV void grid_log2_axes(const int* v, float (&lg)[3], bool (&pos)[3]) {
   if (FAM == KS_FAM_ELEMWISE) lg[1] = (float)ks_ew_op(v[1]);
 }
 
+// Density routing (Q16): inside the measured hull = inside the grid's box,
+// decided on integers (ceil(2^lo) <= v <= floor(2^hi) per non-flat axis, bounds computed on the host).
+template <int FAM>
+KS_DEV bool in_hull(const int* v, const KsGridDev& g) {
+  long long a[3];
+  if (FAM == KS_FAM_GEMM) {
+    a[0] = v[0]; a[1] = v[1]; a[2] = v[2];
+  } else if (FAM == KS_FAM_GROUPED_GEMM) {
+    long long sum = 0;
+#pragma unroll
+    for (int e = 0; e < KS_N_EXPERTS; ++e) sum += ks_nonneg(v[2 + e]);
+    a[0] = sum; a[1] = v[0]; a[2] = v[1];
+  } else if (FAM == KS_FAM_ATTN) {
+    a[0] = v[0]; a[1] = v[1]; a[2] = v[2] < v[1] ? v[1] : v[2];
+  } else {
+    a[0] = v[0]; a[1] = 1; a[2] = 1;                 // (n, 2^subop, 1): axis 1 is checked on the sub-op below
+  }
+  bool in = true;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) in = in && a[k] >= (long long)g.vmin[k] && a[k] <= (long long)g.vmax[k];
+  if (FAM == KS_FAM_ELEMWISE) {
+    const long long b = 1ll << ks_ew_op(v[1]);
+    in = a[0] >= (long long)g.vmin[0] && a[0] <= (long long)g.vmax[0] && b >= (long long)g.vmin[1] && b <= (long long)g.vmax[1];
+  }
+  return in;
+}
+
 // trilinear interpolation of the stored efficiency; grid values in shared memory
 template <int FAM>
 KS_DEV float trilinear(const int* v, const KsGridDev& g, const float* __restrict__ sg) {
@@ -117,7 +144,9 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
   constexpr int NC = NCols<FAM>::v;
   extern __shared__ __align__(128) float sgrid[];
 
-  const int n = p.bk.n;
+  // row-list mode (the learned fallback of density routing): rows idx[0 .. *count) instead of 0 .. n
+  const bool gather = TIER == KS_TIER_BOUNDED && p.bk.idx != nullptr;
+  const int n = gather ? min(__ldg(p.bk.count), p.bk.n) : p.bk.n;
   const int n4 = (n + 3) >> 2;
   const int stride = gridDim.x * blockDim.x;
   int g = blockIdx.x * blockDim.x + threadIdx.x;
@@ -136,8 +165,25 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
   bool have = TIER == KS_TIER_B;                     // Tier B: the first trip's columns are already loaded
   for (; g < n4; g += stride) {
     const int row0 = g << 2;
-    if (!have) load_rows4<NC, F32>(p.bk, row0, n, v);
+    int rr[4] = {row0, row0 + 1, row0 + 2, row0 + 3};
+    if (gather) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        rr[j] = row0 + j < n ? __ldg(p.bk.idx + row0 + j) : 0;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) v[j][c] = row0 + j < n ? ks_load_col(p.bk.cols[c], rr[j], F32) : 0;
+      }
+    } else if (!have) {
+      load_rows4<NC, F32>(p.bk, row0, n, v);
+    }
     have = false;
+    if (TIER == KS_TIER_B && p.grid.route_idx != nullptr) {
+      // density routing, pass 1: remember the rows outside the hull for the learned head (their
+      // clamped Tier-B value written below is overwritten by pass 2, which runs after this kernel)
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (row0 + j < n && !in_hull<FAM>(v[j], p.grid)) p.grid.route_idx[atomicAdd(p.grid.route_count, 1)] = row0 + j;
+    }
 
     float e[4];
 #pragma unroll
@@ -180,6 +226,18 @@ ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
         }
         t[j] = fmaxf(TIER == KS_TIER_NONE ? r.t_roof : __fdividef(r.t_roof, e[j]), sp.t0);
         if (FAM == KS_FAM_ALLREDUCE) tr[j] = t[j] = ks_allreduce(v[j], sp);   // Eq. 3 as it stands
+      }
+      if (gather) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (row0 + j < n) {
+            p.bk.lat[off + rr[j]] = t[j];
+            if (p.bk.tiles) p.bk.tiles[off + rr[j]] = tiles[j];
+            if (p.bk.waves) p.bk.waves[off + rr[j]] = waves[j];
+            if (p.bk.troof) p.bk.troof[off + rr[j]] = tr[j];
+          }
+        }
+        continue;
       }
       store4<float>(p.bk.lat, off, row0, n, vec, t[0], t[1], t[2], t[3]);
       if (p.bk.tiles) store4<int>(p.bk.tiles, off, row0, n, vec, tiles[0], tiles[1], tiles[2], tiles[3]);

@@ -377,3 +377,89 @@ def test_bounded_head_closed_forms_and_replacement(ks):
             c2.load_bounded_head(fam, W.BoundedHead(9, np.zeros(9, np.float32), 0.0, np.zeros(9, np.float32), 0.0))
         finally:
             c2.close()
+
+
+# ------------------------------------------------------------------ density-routed Tier B (NEXT-1)
+def routed_oracle(w):
+    heads = {f: O.Head(h) for f, h in w.heads.items()}
+    grids = {f: O.Grid(g) for f, g in w.grids.items()}
+    return [O.predict_bucket(b, w.specs, W.TIER_B_ROUTED, head=heads.get(b.family), grid=grids[b.family],
+                             bounded=O.Bounded(w.bounded[b.family]) if b.family in w.bounded else None)
+            for b in w.buckets]
+
+
+def check_routed(g, o, what):
+    """In-hull rows are an fp32 path (1e-5), rows routed to an MLP head the bf16 path (1e-2)."""
+    for i, (gi, oi) in enumerate(zip(g, o)):
+        assert np.array_equal(gi["tiles"], oi["tiles"]) and np.array_equal(gi["waves"], oi["waves"])
+        e = rel_err(gi["lat"], oi["lat"])
+        out = oi["routed"] == 1
+        assert e[:, ~out].max(initial=0) <= TOL_F32, f"{what}/bucket{i}: in-hull rel err {e[:, ~out].max()}"
+        assert e[:, out].max(initial=0) <= TOL_MLP, f"{what}/bucket{i}: routed rel err {e[:, out].max()}"
+        assert out.any() and (~out).any()
+
+
+@pytest.mark.parametrize("n,n_specs", [(30011, 1), (5003, 3)])
+def test_density_routing_parity(ks, n, n_specs):
+    B, D = ks
+    w = W.config3(n=n, routed=True)
+    w.specs = [W.spec_gb200(), W.spec_gb200(n_sm=132, peak_flops=1.0e15, peak_bw=3.35e12, t0=3e-6),
+               W.spec_gb200(ctas_per_sm=2)][:n_specs]
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        db = D.to_device(w)
+        g = D.predict(ctx, w, dbuckets=db)
+        g2 = D.predict(ctx, w, dbuckets=db)                           # the row lists are rebuilt per call
+        step, tot = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+    finally:
+        ctx.close()
+    o = routed_oracle(w)
+    check_routed(g, o, w.name)
+    for a, b_ in zip(g, g2):                                           # list order varies, results must not
+        assert np.array_equal(a["lat"], b_["lat"])
+    so, to = O.compose([x["lat"][0] for x in g], [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off)
+    assert rel_err(step[0], so).max() <= TOL_F32 and rel_err(tot[0], to).max() <= TOL_F32
+
+
+def test_density_routing_with_bounded_fallback_and_256_heads(ks):
+    B, D = ks
+    rng = np.random.Generator(np.random.PCG64(21))
+    w = W.config3(n=9001, routed=True, n_in=32, h=256)                # attention keeps a 32->256->256->1 MLP head ...
+    w.bounded = {W.FAM_GEMM: W.make_bounded_head(rng, 12)}             # ... GEMM falls back to the bounded form
+    del w.heads[W.FAM_GEMM]
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        g = D.predict(ctx, w)
+    finally:
+        ctx.close()
+    check_routed(g, routed_oracle(w), w.name)
+
+
+def test_density_routing_host_space_and_missing_models(ks):
+    B, D = ks
+    import torch
+    w = W.config3(n=4001, routed=True)
+    ctx = B.Context(0)
+    try:
+        for fam, gr in w.grids.items():
+            ctx.load_grid(fam, gr)
+        db = D.to_device(w)
+        lat = [torch.empty((1, b.n), dtype=torch.float32, device="cuda:0") for b in db]
+        with pytest.raises(B.KsError) as ei:                           # grids alone are not enough: the fallback needs heads
+            ctx.predict_kernels(db, w.specs, W.TIER_B_ROUTED, lat, space=B.KS_MEM_DEVICE)
+        assert ei.value.status == B.KS_ESTATE
+        D.load_models(ctx, w)
+        g = D.predict(ctx, w, dbuckets=db, aux=False)
+        hb = D.to_pinned(w)
+        step_h = torch.empty((1, w.n_steps), dtype=torch.float32).pin_memory()
+        tot_h = torch.empty((1, len(w.cfg_off) - 1), dtype=torch.float32).pin_memory()
+        lat_h = [torch.empty((1, b.n), dtype=torch.float32).pin_memory() for b in hb]
+        cfg_h = torch.from_numpy(np.ascontiguousarray(w.cfg_off, dtype=np.int32)).pin_memory()
+        ctx.run_steps(hb, [b.step_off for b in hb], w.specs, W.TIER_B_ROUTED, w.n_steps, w.step_params, cfg_h,
+                      len(w.cfg_off) - 1, step_h, tot_h, latency=lat_h, space=B.KS_MEM_HOST)
+    finally:
+        ctx.close()
+    for a, b_ in zip(g, lat_h):
+        assert np.array_equal(a["lat"], b_.numpy())                    # host space runs the same kernels
