@@ -50,6 +50,9 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
   const int s0 = (int)(blockIdx.x - spec * cps) * kS;
   const int ns = p.n_steps - s0 < kS ? p.n_steps - s0 : kS;
 
+  // launched with programmatic stream serialization: the launch itself overlaps the tail of the
+  // prediction kernel; nothing it produced (nor anything copied in for this call) is read before this
+  cudaGridDependencySynchronize();
   for (int idx = tid; idx < p.n_batches * (kS + 1); idx += kThreads) {
     const int b = idx / (kS + 1), j = idx - b * (kS + 1);
     offs[b][j] = __ldg(p.step_off[b] + (s0 + j < p.n_steps ? s0 + j : p.n_steps));
@@ -169,7 +172,10 @@ ks_cfg_total_kernel(const __grid_constant__ KsComposeParams p) {
   const int cfg = blockIdx.x % p.n_cfg;
   const int spec = blockIdx.x / p.n_cfg;
   const int beg = __ldg(p.cfg_off + cfg), end = __ldg(p.cfg_off + cfg + 1);
-  const float* __restrict__ sl = p.step_lat + (long long)spec * p.n_steps;
+  // launched with programmatic stream serialization: everything above overlaps the tail of the step
+  // kernel; the step latencies may only be read once that kernel has completed and flushed
+  cudaGridDependencySynchronize();
+  const float* sl = p.step_lat + (long long)spec * p.n_steps;
   double acc = 0.0;
   for (int s = beg + threadIdx.x; s < end; s += blockDim.x) acc += (double)sl[s];
 #pragma unroll
@@ -197,14 +203,31 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
     const size_t smem = (size_t)(kCapFloats + kSlackFloats) * 4;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)n_chunks, kThreads, smem, st>>>(p);
-    e = cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)n_chunks);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, kern, p);
     if (e != cudaSuccess) return e;
     if (launches) *launches += 1;
   }
   if (p.n_cfg > 0 && p.n_specs > 0 && p.cfg_lat) {
-    ks_cfg_total_kernel<<<(unsigned)(p.n_cfg * p.n_specs), 256, 0, st>>>(p);
-    cudaError_t e = cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(p.n_cfg * p.n_specs));
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // hide this launch under the step kernel's tail
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = total > 0 ? 1 : 0;               // (no preceding kernel of ours: plain launch)
+    cudaError_t e = cudaLaunchKernelEx(&cfg, ks_cfg_total_kernel, p);
     if (e != cudaSuccess) return e;
     if (launches) *launches += 1;
   }
