@@ -427,3 +427,27 @@ void kso_compose(int n_buckets, const double *const *lat, const int64_t *const *
     cfg_lat[c] = tot;
   }
 }
+
+/* PAPER.md:231, layer-homogeneous aggregation */
+void kso_compose_weighted(int n_buckets, const double *const *lat, const int64_t *const *mult,
+                          const int64_t *const *step_off, int64_t n_steps, const kso_step_params *p,
+                          const int64_t *cfg_off, int64_t n_cfg, double *step_lat, double *cfg_lat) {
+  for (int64_t s = 0; s < n_steps; ++s) {
+    double sum = 0.0;
+    int64_t cnt = 0;
+    for (int b = 0; b < n_buckets; ++b) {
+      for (int64_t k = step_off[b][s]; k < step_off[b][s + 1]; ++k) {
+        const int64_t m = (mult && mult[b]) ? mult[b][k] : 1;
+        sum += (double)m * lat[b][k];
+        cnt += m;
+      }
+    }
+    double t_gpu = p->body_scale * sum;
+    step_lat[s] = dmax(t_gpu + (double)cnt * p->c_disp, p->floor_l) + dmax(0.0, p->c_ovl - t_gpu) + p->c_tail;
+  }
+  for (int64_t c = 0; c < n_cfg; ++c) {
+    double tot = 0.0;
+    for (int64_t s = cfg_off[c]; s < cfg_off[c + 1]; ++s) tot += step_lat[s];
+    cfg_lat[c] = tot;
+  }
+}

@@ -144,6 +144,14 @@ void kso_compose(int n_buckets, const double *const *lat, const int64_t *const *
                  int64_t n_steps, const kso_step_params *p, const int64_t *cfg_off, int64_t n_cfg,
                  double *step_lat, double *cfg_lat);
 
+/* Layer-homogeneous form of S6 ("since decoder layers are homogeneous, the GPU body of a
+ * step is t_gpu = L t_layer + t_lm_head + t_embed"): every descriptor row carries a multiplicity m_k >= 0
+ * (how many identical kernels of the step it stands for; mult[b] == NULL means all ones):
+ * t_gpu = body_scale * sum_k m_k t_k, and Eq. 4's launch count is n = sum_k m_k. */
+void kso_compose_weighted(int n_buckets, const double *const *lat, const int64_t *const *mult,
+                          const int64_t *const *step_off, int64_t n_steps, const kso_step_params *p,
+                          const int64_t *cfg_off, int64_t n_cfg, double *step_lat, double *cfg_lat);
+
 #ifdef __cplusplus
 }
 #endif

@@ -120,6 +120,11 @@ def lib():
                                   C.POINTER(C.POINTER(C.c_int64)), C.c_int64, C.POINTER(StepParams),
                                   C.POINTER(C.c_int64), C.c_int64, C.POINTER(C.c_double),
                                   C.POINTER(C.c_double)]
+        L.kso_compose_weighted.restype = None
+        L.kso_compose_weighted.argtypes = [C.c_int, C.POINTER(C.POINTER(C.c_double)), C.POINTER(C.POINTER(C.c_int64)),
+                                           C.POINTER(C.POINTER(C.c_int64)), C.c_int64, C.POINTER(StepParams),
+                                           C.POINTER(C.c_int64), C.c_int64, C.POINTER(C.c_double),
+                                           C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -275,8 +280,9 @@ def predict_bucket(bucket, specs: Sequence[dict], tier: int, head: Optional[Head
 
 
 def compose(lats: Sequence[np.ndarray], step_offs: Sequence[np.ndarray], n_steps: int, params: dict,
-            cfg_off: np.ndarray):
-    """lats[b]: [n_b] float64 for ONE spec; returns (step_lat [n_steps], cfg_lat [n_cfg])."""
+            cfg_off: np.ndarray, mults: Optional[Sequence[Optional[np.ndarray]]] = None):
+    """lats[b]: [n_b] float64 for ONE spec; returns (step_lat [n_steps], cfg_lat [n_cfg]).
+    mults[b] (optional): per-row multiplicities of the layer-homogeneous form."""
     nb = len(lats)
     la = [np.ascontiguousarray(x, dtype=np.float64) for x in lats]
     so = [np.ascontiguousarray(x, dtype=np.int64) for x in step_offs]
@@ -288,5 +294,11 @@ def compose(lats: Sequence[np.ndarray], step_offs: Sequence[np.ndarray], n_steps
                    float(params["c_tail"]), float(params["body_scale"]))
     step_lat = np.zeros(n_steps, np.float64)
     cfg_lat = np.zeros(max(n_cfg, 0), np.float64)
+    if mults is not None and any(m is not None for m in mults):
+        ma = [None if m is None else np.ascontiguousarray(m, dtype=np.int64) for m in mults]
+        mp = (C.POINTER(C.c_int64) * nb)(*[_ip(x) if x is not None else C.POINTER(C.c_int64)() for x in ma])
+        lib().kso_compose_weighted(nb, lp, mp, sp, int(n_steps), C.byref(p), _ip(co), int(n_cfg), _dp(step_lat),
+                                   _dp(cfg_lat))
+        return step_lat, cfg_lat
     lib().kso_compose(nb, lp, sp, int(n_steps), C.byref(p), _ip(co), int(n_cfg), _dp(step_lat), _dp(cfg_lat))
     return step_lat, cfg_lat

@@ -40,6 +40,7 @@ class Bucket:
     hkv: int = 0
     head_dim: int = 0
     step_off: Optional[np.ndarray] = None  # CSR [n_steps+1] int32 into this bucket
+    mult: Optional[np.ndarray] = None      # per-row multiplicity (layer-homogeneous form); None = ones
 
     @property
     def n(self) -> int:
@@ -324,13 +325,18 @@ def _attn_bucket(n_dec, chunk, hist, kv_dec, n_layers):
 
 
 def config4(n_steps: int = 100_000, seed: int = 3, tier: int = TIER_NONE, n_cfg: int = 64,
-            step_params: Optional[dict] = None, n_layers: int = N_LAYERS, tp: int = 1) -> Workload:
+            step_params: Optional[dict] = None, n_layers: int = N_LAYERS, tp: int = 1,
+            dedupe: bool = False) -> Workload:
     """Serving-step composition: 32-layer dense decoder, 9 kernels/layer (+1 prefill attention).
     tp > 1 (not a BASELINE.json config) adds the two tensor-parallel
-    all-reduces per layer of PAPER.md:221 as a fourth bucket: S = T x hidden x 2 bytes over P = tp."""
+    all-reduces per layer of PAPER.md:221 as a fourth bucket: S = T x hidden x 2 bytes over P = tp.
+    dedupe=True emits the SAME steps in the paper's layer-homogeneous form (PAPER.md:231,
+    t_gpu = L t_layer + t_lm_head + t_embed): one layer's kernels per step, each with multiplicity L."""
     rng = _rng(seed)
     n_dec, chunk, hist, kv_dec, T = _draw_steps(rng, n_steps)
     L = n_layers
+    if dedupe:
+        return _config4_dedupe(rng, n_dec, chunk, hist, kv_dec, T, L, n_steps, tier, n_cfg, step_params, tp, seed)
     # GEMM bucket: per layer QKV, O, Gate-Up, Down at M=T; then the LM head once per step
     gN = np.array([QKV_N, HIDDEN, 2 * FFN, HIDDEN] * L + [VOCAB], np.int64)
     gK = np.array([HIDDEN, HIDDEN, HIDDEN, FFN] * L + [HIDDEN], np.int64)
@@ -370,6 +376,34 @@ def allreduce_rows(n: int = 6_400_000, seed: int = 5, tp: int = 4) -> Workload:
     T = np.clip(rng.poisson(64, size=n), 1, 256) + 512 * (rng.random(n) < 0.25)
     return Workload(f"allreduce_tp{tp}", [Bucket(FAM_ALLREDUCE, _i32(T * HIDDEN * 2, np.full(n, tp)))],
                     [spec_gb200()], TIER_NONE, seed=seed)
+
+
+def _config4_dedupe(rng, n_dec, chunk, hist, kv_dec, T, L, n_steps, tier, n_cfg, step_params, tp, seed):
+    i32 = lambda a: np.ascontiguousarray(a, dtype=np.int32)
+    gN = np.array([QKV_N, HIDDEN, 2 * FFN, HIDDEN, VOCAB], np.int64)
+    gK = np.array([HIDDEN, HIDDEN, HIDDEN, FFN, HIDDEN], np.int64)
+    gM = np.repeat(T, 5).reshape(n_steps, 5)
+    gM[:, -1] = n_dec + chunk
+    gemm = Bucket(FAM_GEMM, _i32(gM.reshape(-1), np.tile(gN, n_steps), np.tile(gK, n_steps)),
+                  step_off=_csr(np.full(n_steps, 5)), mult=i32(np.tile([L, L, L, L, 1], n_steps)))
+    mult_e = np.array([HIDDEN, HIDDEN, (HQ + HKV) * HEAD_DIM, 2 * HKV * HEAD_DIM, FFN, HIDDEN], np.int64)
+    sub = np.array([SUB_EMBED, SUB_RMSNORM, SUB_ROPE, SUB_KV_WRITE, SUB_SILU_MUL, SUB_RMSNORM], np.int64)
+    elem = Bucket(FAM_ELEMWISE, _i32((T[:, None] * mult_e[None, :]).reshape(-1), np.tile(sub, n_steps)),
+                  step_off=_csr(np.full(n_steps, 6)), mult=i32(np.tile([1, L, L, L, L, 1], n_steps)))
+    B_, q, kv, aoff = _attn_bucket(n_dec, chunk, hist, kv_dec, 1)
+    attn = Bucket(FAM_ATTN, _i32(B_, q, kv), hq=HQ, hkv=HKV, head_dim=HEAD_DIM, step_off=aoff,
+                  mult=i32(np.full(B_.shape[0], L)))
+    buckets = [gemm, attn, elem]
+    if tp > 1:
+        buckets.append(Bucket(FAM_ALLREDUCE, _i32(T * HIDDEN * 2, np.full(n_steps, tp)), step_off=_csr(np.full(n_steps, 1)),
+                              mult=i32(np.full(n_steps, 2 * L))))
+    heads = {}
+    if tier == TIER_A:
+        hr = _rng(1)
+        heads = {f: make_head(hr, 12, 128) for f in (FAM_GEMM, FAM_ATTN, FAM_ELEMWISE)}
+    return Workload("cfg4_steps_layer_homogeneous", buckets, [spec_gb200()], tier, heads=heads, n_steps=n_steps,
+                    cfg_off=cfg_offsets(rng, n_steps, min(n_cfg, n_steps)),
+                    step_params=dict(step_params or STEP_PARAMS_CFG4), seed=seed)
 
 
 # ----------------------------------------------------------------------------- config 5
