@@ -318,6 +318,22 @@ def run_extras(h: Harness, peaks):
     ex["cfg4a_tierNONE"]["predictions_per_s"] = float(st["w"].n_rows / (ms.sum(axis=1).mean() * 1e-3))
     del st
     torch.cuda.empty_cache()
+    # config 4b: the same 100k steps with Tier-A heads, materialised (29.9M rows) and in the paper's
+    # layer-homogeneous form (one layer per step with multiplicity L, ~1.2M rows)
+    for key, wl in (("cfg4b_tierA", W.config4(tier=W.TIER_A)), ("cfg4b_layer_homogeneous", W.config4(tier=W.TIER_A, dedupe=True))):
+        st = h.prepare(wl)
+        mult = [b.mult for b in st["db"]]
+
+        def comp(st=st, wl=wl, mult=mult):
+            h.ctx.compose_steps(st["lat"], [b.step_off for b in st["db"]], [b.n for b in st["db"]], wl.n_steps, st["ns"],
+                                wl.step_params, st["cfg"], st["n_cfg"], st["step"], st["tot"], space=h.B.KS_MEM_DEVICE,
+                                mult=mult)
+        ms = h.timed([lambda st=st: h.predict(st), comp], 5 if not PROFILE else 1, 2 if not PROFILE else 1)
+        t = float(ms.sum(axis=1).mean())
+        ex[key] = dict(rows=wl.n_rows, steps=wl.n_steps, ms=t, predict_ms=float(ms[:, 0].mean()), compose_ms=float(ms[:, 1].mean()),
+                       steps_per_s=float(wl.n_steps / (t * 1e-3)), kernel_instances_per_s=float(29898400 / (t * 1e-3)))
+        del st
+        torch.cuda.empty_cache()
     # NEXT-3: tensor-parallel all-reduce rows (Eq. 3), 6.4M rows = two per layer of cfg4's 100k steps
     st = h.prepare_rows(W.allreduce_rows())
     sets = None if PROFILE else clone_sets(st, 6)

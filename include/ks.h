@@ -91,6 +91,10 @@ typedef struct {
   int32_t n_cols;          /* columns supplied; must equal the family's count */
   int32_t attn_hq, attn_hkv, attn_head_dim;
   const void *cols[KS_MAX_COLS];
+  const int32_t *mult;     /* optional (may be NULL = all ones): per-row multiplicity m_k >= 0, int32 [n], in the
+                              call's memory space.  Layer-homogeneous form of PAPER.md:231 (t_gpu = L t_layer +
+                              t_lm_head + t_embed): a row stands for m_k identical kernels of its step.  Read by
+                              ks_run_steps only (ks_predict_kernels predicts a row once whatever its multiplicity). */
 } ks_desc_batch;
 
 /* Host-overlap constants of Eq. 4; body_scale multiplies sum t (Q7). */
@@ -158,8 +162,16 @@ KS_API ks_status ks_compose_steps(ks_ctx *ctx, const float *const *latency, cons
                            const ks_step_params *params, const int32_t *cfg_off, int n_cfg,
                            ks_mem_space space, float *step_latency, float *cfg_latency);
 
+/* ks_compose_steps with per-row multiplicities (layer-homogeneous form):
+ *   mult[b]   optional int32 [batch_n[b]] (the array pointer or an entry may be NULL = all ones), shared
+ *             by all specs: t_gpu = body_scale * sum_k m_k t_k, and Eq. 4's launch count n = sum_k m_k. */
+KS_API ks_status ks_compose_steps_weighted(ks_ctx *ctx, const float *const *latency, const int32_t *const *mult,
+                                    const int32_t *const *step_off, const int32_t *batch_n, int n_batches,
+                                    int n_steps, int n_specs, const ks_step_params *params, const int32_t *cfg_off,
+                                    int n_cfg, ks_mem_space space, float *step_latency, float *cfg_latency);
+
 /* Convenience: ks_predict_kernels followed by ks_compose_steps in one call (one pass of the whole
- * hot path).  latency may be NULL (or hold NULL entries): per-kernel latencies then stay in the
+ * hot path; rows with batches[b].mult are weighted as in ks_compose_steps_weighted).  latency may be NULL (or hold NULL entries): per-kernel latencies then stay in the
  * library workspace and only the step/config results are returned.  With KS_MEM_HOST this is the
  * end-to-end call: descriptors and offsets go host->device, results device->host, then sync. */
 KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const int32_t *const *step_off,

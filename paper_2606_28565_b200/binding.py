@@ -22,6 +22,7 @@ KS_COL_I32, KS_COL_F32 = 0, 1
 KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
 EXPORTS = ["ks_create", "ks_load_heads", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
+           "ks_compose_steps_weighted",
            "ks_run_steps", "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
 
 
@@ -41,7 +42,7 @@ class ks_hw_spec(C.Structure):
 class ks_desc_batch(C.Structure):
     _fields_ = [("family", C.c_int32), ("n", C.c_int32), ("col_dtype", C.c_int32), ("dtype_bytes", C.c_int32),
                 ("n_cols", C.c_int32), ("attn_hq", C.c_int32), ("attn_hkv", C.c_int32),
-                ("attn_head_dim", C.c_int32), ("cols", C.c_void_p * KS_MAX_COLS)]
+                ("attn_head_dim", C.c_int32), ("cols", C.c_void_p * KS_MAX_COLS), ("mult", C.c_void_p)]
 
 
 class ks_step_params(C.Structure):
@@ -70,6 +71,8 @@ def load() -> C.CDLL:
                                      C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.ks_compose_steps.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int32), i32, i32, i32,
                                    C.POINTER(ks_step_params), vp, i32, i32, vp, vp]
+    L.ks_compose_steps_weighted.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int32), i32,
+                                            i32, i32, C.POINTER(ks_step_params), vp, i32, i32, vp, vp]
     L.ks_run_steps.argtypes = [vp, C.POINTER(ks_desc_batch), C.POINTER(vp), i32, C.POINTER(ks_hw_spec), i32, i32,
                                i32, C.POINTER(ks_step_params), vp, i32, i32, C.POINTER(vp), vp, vp]
     L.ks_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
@@ -134,8 +137,11 @@ def make_batch(bucket) -> ks_desc_batch:
         if hasattr(c, "is_contiguous") and not c.is_contiguous():
             raise ValueError("descriptor columns must be contiguous")
         arr[i] = _ptr(c)
+    mult = getattr(bucket, "mult", None)             # optional per-row multiplicities (int32)
+    if mult is not None and "int32" not in str(mult.dtype):
+        raise TypeError("multiplicities must be int32")
     return ks_desc_batch(int(bucket.family), n, cd, int(bucket.dtype_bytes), len(cols), int(bucket.hq),
-                         int(bucket.hkv), int(bucket.head_dim), arr)
+                         int(bucket.hkv), int(bucket.head_dim), arr, _ptr(mult) if mult is not None else None)
 
 
 def make_step_params(p: dict) -> ks_step_params:
@@ -210,12 +216,19 @@ class Context:
 
     def compose_steps(self, latency: Sequence, step_off: Sequence, batch_n: Sequence[int], n_steps: int,
                       n_specs: int, params: dict, cfg_off, n_cfg: int, step_latency, cfg_latency,
-                      space: Optional[int] = None) -> None:
+                      space: Optional[int] = None, mult: Optional[Sequence] = None) -> None:
         nb = len(latency)
         bn = (C.c_int32 * max(nb, 1))(*[int(x) for x in batch_n])
         p = make_step_params(params)
         if space is None:
             space = KS_MEM_HOST if _is_host(step_latency) else KS_MEM_DEVICE
+        if mult is not None and any(m is not None for m in mult):
+            _check(self._lib.ks_compose_steps_weighted(self._h, _ptr_array(latency), _ptr_array(mult),
+                                                       _ptr_array(step_off), bn, nb, int(n_steps), int(n_specs),
+                                                       C.byref(p), _ptr(cfg_off), int(n_cfg), int(space),
+                                                       _ptr(step_latency), _ptr(cfg_latency)),
+                   "ks_compose_steps_weighted")
+            return
         _check(self._lib.ks_compose_steps(self._h, _ptr_array(latency), _ptr_array(step_off), bn, nb, int(n_steps),
                                           int(n_specs), C.byref(p), _ptr(cfg_off), int(n_cfg), int(space),
                                           _ptr(step_latency), _ptr(cfg_latency)), "ks_compose_steps")

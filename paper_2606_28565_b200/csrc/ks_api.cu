@@ -535,7 +535,8 @@ bool csr_ok(const int32_t* off, int n, long long limit) {       // host-resident
 
 ks_status compose_device(ks_ctx* c, const float* const* lat, const int32_t* const* step_off, const int32_t* batch_n,
                          int n_batches, int n_steps, int n_specs, const ks_step_params* params,
-                         const int32_t* cfg_off, int n_cfg, float* step_lat, float* cfg_lat) {
+                         const int32_t* cfg_off, int n_cfg, float* step_lat, float* cfg_lat,
+                         const int32_t* const* mult = nullptr) {
   if (n_steps == 0 || n_specs == 0) {
     if (n_cfg > 0 && n_specs > 0) KS_CUDA(c, cudaMemsetAsync(cfg_lat, 0, (size_t)n_cfg * n_specs * 4, c->stream));
     return KS_OK;
@@ -545,6 +546,7 @@ ks_status compose_device(ks_ctx* c, const float* const* lat, const int32_t* cons
   for (int b = 0; b < n_batches; ++b) {
     p.lat[b] = lat[b];
     p.step_off[b] = step_off[b];
+    p.mult[b] = mult ? mult[b] : nullptr;
     p.spec_stride[b] = batch_n[b];
   }
   p.n_batches = n_batches;
@@ -666,6 +668,14 @@ ks_status ks_compose_steps(ks_ctx* c, const float* const* latency, const int32_t
                            const int32_t* batch_n, int n_batches, int n_steps, int n_specs,
                            const ks_step_params* params, const int32_t* cfg_off, int n_cfg, ks_mem_space space,
                            float* step_latency, float* cfg_latency) {
+  return ks_compose_steps_weighted(c, latency, nullptr, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off,
+                                   n_cfg, space, step_latency, cfg_latency);
+}
+
+ks_status ks_compose_steps_weighted(ks_ctx* c, const float* const* latency, const int32_t* const* mult,
+                                    const int32_t* const* step_off, const int32_t* batch_n, int n_batches,
+                                    int n_steps, int n_specs, const ks_step_params* params, const int32_t* cfg_off,
+                                    int n_cfg, ks_mem_space space, float* step_latency, float* cfg_latency) {
   ks_status st = validate_compose(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg,
                                   space, step_latency, cfg_latency, false);
   if (st != KS_OK) return st;
@@ -673,16 +683,23 @@ ks_status ks_compose_steps(ks_ctx* c, const float* const* latency, const int32_t
   KS_CUDA(c, cudaSetDevice(c->device));
   if (space == KS_MEM_DEVICE)
     return compose_device(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg,
-                          step_latency, cfg_latency);
+                          step_latency, cfg_latency, mult);
   size_t need = align_up((size_t)(n_cfg + 1) * 4, 256) + align_up((size_t)n_steps * n_specs * 4, 256) +
                 align_up((size_t)n_cfg * n_specs * 4 + 4, 256);
   for (int b = 0; b < n_batches; ++b)
-    need += align_up((size_t)batch_n[b] * n_specs * 4, 256) + align_up((size_t)(n_steps + 1) * 4, 256);
+    need += align_up((size_t)batch_n[b] * n_specs * 4, 256) + align_up((size_t)(n_steps + 1) * 4, 256) +
+            align_up((size_t)batch_n[b] * 4, 256);
   st = ws_reserve(c, need);
   if (st != KS_OK) return st;
   const float* dlat[KS_MAX_BATCHES];
   const int32_t* doff[KS_MAX_BATCHES];
+  const int32_t* dmult[KS_MAX_BATCHES] = {};
   for (int b = 0; b < n_batches; ++b) {
+    if (mult && mult[b] && batch_n[b] > 0) {
+      int32_t* dm = static_cast<int32_t*>(ws_take(c, (size_t)batch_n[b] * 4));
+      KS_CUDA(c, cudaMemcpyAsync(dm, mult[b], (size_t)batch_n[b] * 4, cudaMemcpyHostToDevice, c->stream));
+      dmult[b] = dm;
+    }
     const size_t lb = (size_t)batch_n[b] * n_specs * 4, ob = (size_t)(n_steps + 1) * 4;
     float* dl = static_cast<float*>(ws_take(c, lb));
     int32_t* dofs = static_cast<int32_t*>(ws_take(c, ob));
@@ -695,7 +712,7 @@ ks_status ks_compose_steps(ks_ctx* c, const float* const* latency, const int32_t
   float* dstep = static_cast<float*>(ws_take(c, (size_t)n_steps * n_specs * 4));
   float* dtot = static_cast<float*>(ws_take(c, (size_t)n_cfg * n_specs * 4 + 4));
   if (n_cfg > 0) KS_CUDA(c, cudaMemcpyAsync(dcfg, cfg_off, (size_t)(n_cfg + 1) * 4, cudaMemcpyHostToDevice, c->stream));
-  st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot);
+  st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot, dmult);
   if (st != KS_OK) return st;
   if ((size_t)n_steps * n_specs)
     KS_CUDA(c, cudaMemcpyAsync(step_latency, dstep, (size_t)n_steps * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));
@@ -729,7 +746,7 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
     const size_t n = batches[b].n;
     const bool user_lat = dev && latency && latency[b];
     if (!user_lat) need += align_up(n * (size_t)n_specs * 4, 256);
-    if (!dev) need += batches[b].n_cols * align_up(n * 4, 256) + align_up((size_t)(n_steps + 1) * 4, 256);
+    if (!dev) need += (batches[b].n_cols + 1) * align_up(n * 4, 256) + align_up((size_t)(n_steps + 1) * 4, 256);
   }
   if (!dev)
     need += align_up((size_t)(n_cfg + 1) * 4, 256) + align_up((size_t)n_steps * n_specs * 4, 256) +
@@ -744,6 +761,7 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   DevOut outs[KS_MAX_BATCHES];
   const float* dlat[KS_MAX_BATCHES];
   const int32_t* doff[KS_MAX_BATCHES];
+  const int32_t* dmult[KS_MAX_BATCHES] = {};       // layer-homogeneous multiplicities, optional
   if (dev) {
     for (int b = 0; b < n_batches; ++b) {
       for (int k = 0; k < batches[b].n_cols; ++k) cols[b][k] = batches[b].cols[k];
@@ -751,13 +769,14 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
                                             : static_cast<float*>(ws_take(c, (size_t)batches[b].n * n_specs * 4));
       dlat[b] = outs[b].lat;
       doff[b] = step_off[b];
+      dmult[b] = batches[b].mult;
     }
     if (n_specs > 0 && n_batches > 0) {
       st = predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs, rb);
       if (st != KS_OK) return st;
     }
     return compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg, step_latency,
-                          cfg_latency);
+                          cfg_latency, dmult);
   }
 
   // ---- host space: a three-stream pipeline over the buckets (largest copy first is the caller's
@@ -778,6 +797,11 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
     int32_t* dofs = static_cast<int32_t*>(ws_take(c, (size_t)(n_steps + 1) * 4));
     KS_CUDA(c, cudaMemcpyAsync(dofs, step_off[b], (size_t)(n_steps + 1) * 4, cudaMemcpyHostToDevice, c->h2d));
     doff[b] = dofs;
+    if (batches[b].mult && n) {
+      int32_t* dm = static_cast<int32_t*>(ws_take(c, n * 4));
+      KS_CUDA(c, cudaMemcpyAsync(dm, batches[b].mult, n * 4, cudaMemcpyHostToDevice, c->h2d));
+      dmult[b] = dm;
+    }
     outs[b].lat = static_cast<float*>(ws_take(c, n * (size_t)n_specs * 4));
     dlat[b] = outs[b].lat;
     KS_CUDA(c, cudaEventRecord(c->ev_in[b], c->h2d));
@@ -801,7 +825,7 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
     }
   }
   KS_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_start, 0));     // cfg offsets (and every earlier h2d copy)
-  st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot);
+  st = compose_device(c, dlat, doff, batch_n, n_batches, n_steps, n_specs, params, dcfg, n_cfg, dstep, dtot, dmult);
   if (st != KS_OK) return st;
   if ((size_t)n_steps * n_specs)
     KS_CUDA(c, cudaMemcpyAsync(step_latency, dstep, (size_t)n_steps * n_specs * 4, cudaMemcpyDeviceToHost, c->stream));

@@ -28,6 +28,8 @@ constexpr int kS = 32;                 // steps per chunk (one CTA)
 constexpr int kCapFloats = 12032;      // staged floats per CTA (47 KiB + slack): four CTAs per SM
 constexpr int kSlackFloats = 192;      // readable floats behind the staged data (masked lanes of the last step)
 
+KS_DEV int mA_n(int n, int lane) { return n - lane; }   // elements 32 r < n - lane belong to this lane
+
 // this lane's share of src[0, n) beyond the first 160 elements (rare: very long steps)
 KS_DEV float lane_tail(const float* __restrict__ src, int n, int lane) {
   float a0 = 0.0f, a1 = 0.0f;
@@ -39,7 +41,7 @@ KS_DEV float lane_tail(const float* __restrict__ src, int n, int lane) {
 }
 
 // NB = compile-time bound on the bucket count (1-4: exact, or 8)
-template <int NB>
+template <int NB, bool MULT>
 __global__ void __launch_bounds__(kThreads, 4)
 ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
   extern __shared__ __align__(128) float sdata[];
@@ -140,18 +142,42 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
             x3 = 96 < mA ? sA[96] : 0.0f; y3 = 96 < mB ? sB[96] : 0.0f;
             x4 = 128 < mA ? sA[128] : 0.0f; y4 = 128 < mB ? sB[128] : 0.0f;
           }
-          accA += ((x0 + x1) + (x2 + x3)) + x4;
-          accB += ((y0 + y1) + (y2 + y3)) + y4;
-          if (nA > 160) accA += lane_tail(sA - lane, nA, lane);
-          if (nB > 160) accB += lane_tail(sB - lane, nB, lane);
-          cntA += nA;
-          cntB += nB;
+          if (MULT && p.mult[b] != nullptr) {
+            // layer-homogeneous form: a row stands for m_k identical kernels; the
+            // multiplicities are read from global memory (they are shared by all specs)
+            const int32_t* __restrict__ mA = p.mult[b] + begA + lane;
+            const int32_t* __restrict__ mB = p.mult[b] + begB + lane;
+            int ka = 0, kb = 0;
+            float pa = 0.0f, pb = 0.0f;
+            const float xs[5] = {x0, x1, x2, x3, x4}, ys[5] = {y0, y1, y2, y3, y4};
+#pragma unroll
+            for (int r = 0; r < 5; ++r) {
+              const int ma = 32 * r < mA_n(nA, lane) ? __ldg(mA + 32 * r) : 0;
+              const int mb = 32 * r < mA_n(nB, lane) ? __ldg(mB + 32 * r) : 0;
+              pa = fmaf((float)ma, xs[r], pa); ka += ma;
+              pb = fmaf((float)mb, ys[r], pb); kb += mb;
+            }
+            for (int k = lane + 160; k < nA; k += 32) { const int m = __ldg(p.mult[b] + begA + k); pa = fmaf((float)m, (sA - lane)[k], pa); ka += m; }
+            for (int k = lane + 160; k < nB; k += 32) { const int m = __ldg(p.mult[b] + begB + k); pb = fmaf((float)m, (sB - lane)[k], pb); kb += m; }
+            accA += pa; accB += pb;
+            cntA += ka; cntB += kb;                   // per-lane partial launch counts, summed with the shuffle tree below
+          } else {
+            accA += ((x0 + x1) + (x2 + x3)) + x4;
+            accB += ((y0 + y1) + (y2 + y3)) + y4;
+            if (nA > 160) accA += lane_tail(sA - lane, nA, lane);
+            if (nB > 160) accB += lane_tail(sB - lane, nB, lane);
+            if (!MULT || lane == 0) { cntA += nA; cntB += nB; }
+          }
         }
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
         accA += __shfl_xor_sync(0xffffffffu, accA, o);
         accB += __shfl_xor_sync(0xffffffffu, accB, o);
+        if (MULT) {
+          cntA += __shfl_xor_sync(0xffffffffu, cntA, o);
+          cntB += __shfl_xor_sync(0xffffffffu, cntB, o);
+        }
       }
       if (lane < 2 && (lane == 0 || hasB)) {
         const float t_gpu = p.sp.body_scale * (lane == 0 ? accA : accB);
@@ -198,8 +224,12 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
   if (total > 0) {
     const long long n_chunks = (long long)((p.n_steps + kS - 1) / kS) * p.n_specs;
     if (n_chunks > 0x7fffffffll) return cudaErrorInvalidValue;
-    auto kern = p.n_batches <= 1 ? ks_compose_kernel<1> : p.n_batches == 2 ? ks_compose_kernel<2> :
-                p.n_batches == 3 ? ks_compose_kernel<3> : p.n_batches == 4 ? ks_compose_kernel<4> : ks_compose_kernel<8>;
+    bool weighted = false;
+    for (int b = 0; b < p.n_batches; ++b) weighted = weighted || p.mult[b] != nullptr;
+    auto kern = p.n_batches <= 1 ? ks_compose_kernel<1, false> : p.n_batches == 2 ? ks_compose_kernel<2, false> :
+                p.n_batches == 3 ? ks_compose_kernel<3, false> : p.n_batches == 4 ? ks_compose_kernel<4, false> :
+                                                                                   ks_compose_kernel<8, false>;
+    if (weighted) kern = p.n_batches <= 4 ? ks_compose_kernel<4, true> : ks_compose_kernel<8, true>;
     const size_t smem = (size_t)(kCapFloats + kSlackFloats) * 4;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

@@ -54,6 +54,7 @@ int ks_mlp_k1(int n_in);   // padded K of layer 1 (16 or 32)
 struct KsComposeParams {
   const float* lat[KS_MAX_BATCHES];
   const int32_t* step_off[KS_MAX_BATCHES];
+  const int32_t* mult[KS_MAX_BATCHES];    // optional per-row multiplicities (nullptr = ones)
   int64_t spec_stride[KS_MAX_BATCHES];
   int32_t n_batches, n_steps, n_specs, n_cfg;
   ks_step_params sp;

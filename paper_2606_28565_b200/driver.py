@@ -24,6 +24,7 @@ class DeviceBucket:
     hkv: int
     head_dim: int
     step_off: object = None
+    mult: object = None   # optional int32 per-row multiplicities (layer-homogeneous form)
 
     @property
     def n(self) -> int:
@@ -43,7 +44,8 @@ def to_device(w: Workload, device: str = "cuda:0") -> List[DeviceBucket]:
     for b in w.buckets:
         cols = [torch.from_numpy(np.ascontiguousarray(c)).to(device) for c in b.cols]
         so = torch.from_numpy(np.ascontiguousarray(b.step_off, dtype=np.int32)).to(device) if b.step_off is not None else None
-        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so))
+        mu = torch.from_numpy(np.ascontiguousarray(b.mult, dtype=np.int32)).to(device) if b.mult is not None else None
+        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu))
     return out
 
 
@@ -54,7 +56,8 @@ def to_pinned(w: Workload) -> List[DeviceBucket]:
     for b in w.buckets:
         cols = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in b.cols]
         so = torch.from_numpy(np.ascontiguousarray(b.step_off, dtype=np.int32)).pin_memory() if b.step_off is not None else None
-        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so))
+        mu = torch.from_numpy(np.ascontiguousarray(b.mult, dtype=np.int32)).pin_memory() if b.mult is not None else None
+        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu))
     return out
 
 
@@ -97,6 +100,7 @@ def compose(ctx: B.Context, w: Workload, lat_dev: list, dbuckets: List[DeviceBuc
     step = torch.empty((ns, w.n_steps), dtype=torch.float32, device=device)
     tot = torch.empty((ns, max(n_cfg, 1)), dtype=torch.float32, device=device)
     ctx.compose_steps(lat_dev, [b.step_off for b in dbuckets], [b.n for b in dbuckets], w.n_steps, ns,
-                      params or w.step_params, cfg, n_cfg, step, tot, space=B.KS_MEM_DEVICE)
+                      params or w.step_params, cfg, n_cfg, step, tot, space=B.KS_MEM_DEVICE,
+                      mult=[b.mult for b in dbuckets])
     torch.cuda.synchronize()
     return step.cpu().numpy(), tot.cpu().numpy()[:, :n_cfg]

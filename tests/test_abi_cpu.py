@@ -33,7 +33,7 @@ def test_exports_every_declared_symbol(lib):
 def test_struct_layouts_match_header():
     assert C.sizeof(B.ks_hw_spec) == 44
     assert C.sizeof(B.ks_step_params) == 20
-    assert C.sizeof(B.ks_desc_batch) == 32 + 8 * B.KS_MAX_COLS
+    assert C.sizeof(B.ks_desc_batch) == 32 + 8 * B.KS_MAX_COLS + 8
 
 
 def test_status_strings(lib):

@@ -463,3 +463,39 @@ def test_density_routing_host_space_and_missing_models(ks):
         ctx.close()
     for a, b_ in zip(g, lat_h):
         assert np.array_equal(a["lat"], b_.numpy())                    # host space runs the same kernels
+
+
+# ------------------------------------------------------------------ layer-homogeneous composition
+@pytest.mark.parametrize("tier", [W.TIER_NONE, W.TIER_A])
+def test_layer_homogeneous_steps_match_oracle_and_materialised_steps(ks, tier):
+    B, D = ks
+    import torch
+    full = W.config4(n_steps=61, n_layers=6, tier=tier, tp=2)
+    ded = W.config4(n_steps=61, n_layers=6, tier=tier, tp=2, dedupe=True)
+    assert ded.n_rows * 4 < full.n_rows
+    out = {}
+    ctx = B.Context(0)
+    try:
+        for name, w in (("full", full), ("ded", ded)):
+            D.load_models(ctx, w)
+            db = D.to_device(w)
+            g = D.predict(ctx, w, dbuckets=db)
+            out[name] = (g,) + D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+        # the same through ks_run_steps in host space (multiplicities travel in ks_desc_batch.mult)
+        hb = D.to_pinned(ded)
+        n_cfg = len(ded.cfg_off) - 1
+        step_h = torch.empty((1, ded.n_steps), dtype=torch.float32).pin_memory()
+        tot_h = torch.empty((1, n_cfg), dtype=torch.float32).pin_memory()
+        cfg_h = torch.from_numpy(np.ascontiguousarray(ded.cfg_off, dtype=np.int32)).pin_memory()
+        ctx.run_steps(hb, [b.step_off for b in hb], ded.specs, tier, ded.n_steps, ded.step_params, cfg_h, n_cfg,
+                      step_h, tot_h, space=B.KS_MEM_HOST)
+    finally:
+        ctx.close()
+    g, step, tot = out["ded"]
+    so, to = O.compose([x["lat"][0] for x in g], [b.step_off for b in ded.buckets], ded.n_steps, ded.step_params,
+                       ded.cfg_off, mults=[b.mult for b in ded.buckets])
+    assert rel_err(step[0], so).max() <= TOL_F32 and rel_err(tot[0], to).max() <= TOL_F32
+    assert np.array_equal(step_h.numpy(), step) and np.array_equal(tot_h.numpy(), tot)
+    # L identical kernels summed one by one or taken L times: the same step up to fp32 rounding of the sums
+    assert rel_err(step[0], out["full"][1][0]).max() <= 2 * TOL_F32
+    assert rel_err(tot[0], out["full"][2][0]).max() <= 2 * TOL_F32
