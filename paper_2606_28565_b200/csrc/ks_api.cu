@@ -122,14 +122,13 @@ float bf16_bits_to_f32(uint16_t b) {
 
 KsFastDiv make_fastdiv(uint32_t d) {
   KsFastDiv f;
+  if (d < 1) d = 1;
   f.d = d;
   f.pad = 0;
-  if (d <= 1) { f.mul = 0; f.shr = 0; f.d = 1; return f; }
   uint32_t l = 0;
-  while ((1ull << l) < d) ++l;                       // ceil(log2 d)
-  const uint32_t p = 31 + l;
-  f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
-  f.shr = p - 32;
+  while ((1ull << l) < d) ++l;                       // ceil(log2 d); d = 1 -> l = 0, mul = 2^31
+  f.mul = (uint32_t)(((1ull << (31 + l)) + d - 1) / d);
+  f.shr = l;
   return f;
 }
 

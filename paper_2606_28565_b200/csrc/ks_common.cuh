@@ -15,9 +15,8 @@ struct KsFastDiv {
   uint32_t mul, shr, d, pad;
 };
 
-KS_DEV uint32_t ks_div(uint32_t a, const KsFastDiv& f) {
-  return f.d == 1u ? a : (__umulhi(a, f.mul) >> f.shr);
-}
+// branch-free for every d >= 1: umulhi(2a, ceil(2^(31+l)/d)) >> l with l = ceil(log2 d); 2a fits because a < 2^31
+KS_DEV uint32_t ks_div(uint32_t a, const KsFastDiv& f) { return __umulhi(a << 1, f.mul) >> f.shr; }
 KS_DEV uint32_t ks_ceil_div(uint32_t a, const KsFastDiv& f) {
   uint32_t q = ks_div(a, f);
   return q + (q * f.d != a ? 1u : 0u);
