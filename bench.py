@@ -45,14 +45,19 @@ def load_peaks():
 
 
 def load_traffic():
-    """Per-launch DRAM bytes of the dominant kernel from the committed ncu capture (profiles/), or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu capture (profiles/traffic.txt:
+    lines of "<key> <bytes>"), or an empty dict."""
+    p = os.path.join(ROOT, "profiles", "traffic.txt")
+    out = {}
     if os.path.exists(p):
-        try:
-            return json.load(open(p))
-        except Exception:
-            return {}
-    return {}
+        for line in open(p):
+            parts = line.split()
+            if len(parts) == 2 and not line.startswith("#"):
+                try:
+                    out[parts[0]] = int(parts[1])
+                except ValueError:
+                    pass
+    return out
 
 
 class ClockSampler:
