@@ -333,6 +333,51 @@ int kso_predict_batch_bounded(int family, int64_t n, const double *const *cols, 
   return 0;
 }
 
+/* PAPER.md:201 (pool member "small MLP ensemble"); Q17: mean of the members' efficiencies */
+double kso_ensemble_e(const kso_head *members, int k, const double *x) {
+  double sum = 0.0;
+  for (int m = 0; m < k; ++m) sum += kso_sigmoid(kso_mlp_z(&members[m], x));
+  return sum / (double)k;
+}
+
+double kso_predict_one_ensemble(const kso_desc *d, const kso_spec *hw, const kso_head *members, int k,
+                                kso_roof *rout, double *e_out) {
+  if (d->family == KSO_ALLREDUCE) return kso_predict_one(d, hw, KSO_TIER_NONE, NULL, NULL, rout, e_out);
+  kso_roof r;
+  kso_roofline(d, hw, &r);
+  double x[32];
+  kso_features(d, hw, &r, members[0].n_in, x);
+  for (int i = 0; i < members[0].n_in; ++i) x[i] = kso_bf16(x[i]);   /* bf16 inputs, Q11 */
+  double e = kso_ensemble_e(members, k, x);
+  e = dmax(e, ldexp(1.0, -10));                                      /* guard, Q3 */
+  if (rout) *rout = r;
+  if (e_out) *e_out = e;
+  return dmax(r.t_roof / e, hw->t0);
+}
+
+int kso_predict_batch_ensemble(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
+                               int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
+                               const kso_head *members, int k, double *lat, int64_t *tiles, int64_t *waves,
+                               double *troof) {
+  if (n < 0 || n_cols < 0 || n_cols > KSO_MAX_COLS || !members || k < 1) return -1;
+  for (int m = 1; m < k; ++m) if (members[m].n_in != members[0].n_in) return -1;
+  for (int sp = 0; sp < n_specs; ++sp) {
+    for (int64_t i = 0; i < n; ++i) {
+      kso_desc d;
+      d.family = family; d.s = s; d.hq = hq; d.hkv = hkv; d.d = dh;
+      for (int c = 0; c < KSO_MAX_COLS; ++c) d.v[c] = (c < n_cols) ? (int64_t)llround(cols[c][i]) : 0;
+      kso_roof r;
+      const double t = kso_predict_one_ensemble(&d, &specs[sp], members, k, &r, NULL);
+      const size_t o = (size_t)sp * (size_t)n + (size_t)i;
+      lat[o] = t;
+      if (tiles) tiles[o] = r.B;
+      if (waves) waves[o] = r.W;
+      if (troof) troof[o] = r.t_roof;
+    }
+  }
+  return 0;
+}
+
 /* PAPER.md:211 density routing; Q16 */
 int kso_in_hull(const kso_grid *g, const kso_desc *d) {
   double v[3];

@@ -114,6 +114,17 @@ double kso_predict_one_bounded(const kso_desc *d, const kso_spec *hw, const kso_
 int kso_predict_batch_bounded(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
                               int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
                               const kso_bounded *bh, double *lat, int64_t *tiles, int64_t *waves, double *troof);
+/* MLP ensemble ("small MLP ensemble"; Q17): k members of the same shape, each the
+ * MLP of kso_mlp_z; the ensemble's efficiency is the arithmetic mean of the members' outputs,
+ * e = (1/k) sum_m sigmoid(z_m(x)), taken before the guard and the inversion eta = 1/e. */
+double kso_ensemble_e(const kso_head *members, int k, const double *x);
+/* One full prediction with an ensemble head: bf16 inputs as for a single MLP head (Q11). */
+double kso_predict_one_ensemble(const kso_desc *d, const kso_spec *hw, const kso_head *members, int k,
+                                kso_roof *r, double *e_out);
+int kso_predict_batch_ensemble(int family, int64_t n, const double *const *cols, int n_cols, int64_t s,
+                               int64_t hq, int64_t hkv, int64_t dh, const kso_spec *specs, int n_specs,
+                               const kso_head *members, int k, double *lat, int64_t *tiles, int64_t *waves,
+                               double *troof);
 /* Density routing: 1 iff the query lies inside the measured hull, here the grid's box:
  * lo_a <= log2 v_a <= hi_a on every axis with more than one node, decided on integers as
  * ceil(2^lo_a) <= v_a <= floor(2^hi_a) (Q16); a non-positive axis value is outside. */

@@ -85,6 +85,13 @@ def lib():
                                                 C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.POINTER(Spec), C.c_int,
                                                 C.POINTER(BoundedC), C.POINTER(C.c_double), C.POINTER(C.c_int64),
                                                 C.POINTER(C.c_int64), C.POINTER(C.c_double)]
+        L.kso_ensemble_e.restype = C.c_double
+        L.kso_ensemble_e.argtypes = [C.POINTER(HeadC), C.c_int, C.POINTER(C.c_double)]
+        L.kso_predict_batch_ensemble.restype = C.c_int
+        L.kso_predict_batch_ensemble.argtypes = [C.c_int, C.c_int64, C.POINTER(C.POINTER(C.c_double)), C.c_int,
+                                                 C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.POINTER(Spec), C.c_int,
+                                                 C.POINTER(HeadC), C.c_int, C.POINTER(C.c_double),
+                                                 C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_double)]
         L.kso_predict_batch_routed.restype = C.c_int
         L.kso_predict_batch_routed.argtypes = [C.c_int, C.c_int64, C.POINTER(C.POINTER(C.c_double)), C.c_int,
                                                C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.POINTER(Spec), C.c_int,
@@ -170,6 +177,15 @@ class Head:
                        _dp(self.b2), _dp(self.w3), float(h.b3))
 
 
+class Ensemble:
+    """k MLP members of one shape ("small MLP ensemble"; Q17): e = mean of sigmoid(z_m)."""
+
+    def __init__(self, members, round_weights: bool = True):
+        self.heads = [Head(m, round_weights) for m in members]
+        self.k = len(self.heads)
+        self.c = (HeadC * self.k)(*[h.c for h in self.heads])
+
+
 class BoundedC(C.Structure):
     _fields_ = [("n_in", C.c_int), ("w_gamma", C.POINTER(C.c_double)), ("w_alpha", C.POINTER(C.c_double)),
                 ("b_gamma", C.c_double), ("b_alpha", C.c_double)]
@@ -237,9 +253,14 @@ def bounded_e(bh: "Bounded", x, W: int) -> float:
     return float(lib().kso_bounded_e(C.byref(bh.c), _dp(xa), int(W)))
 
 
+def ensemble_e(ens: "Ensemble", x) -> float:
+    xa = np.ascontiguousarray(x, dtype=np.float64)
+    return float(lib().kso_ensemble_e(ens.c, ens.k, _dp(xa)))
+
+
 def predict_bucket(bucket, specs: Sequence[dict], tier: int, head: Optional[Head] = None,
                    grid: Optional[Grid] = None, rows: Optional[np.ndarray] = None,
-                   bounded: Optional["Bounded"] = None):
+                   bounded: Optional["Bounded"] = None, ensemble: Optional["Ensemble"] = None):
     """Run the oracle over one workloads.Bucket (optionally only ``rows``) for every spec.
 
     Returns dict(lat [n_specs,n] f64, tiles i64, waves i64, troof f64).
@@ -263,6 +284,13 @@ def predict_bucket(bucket, specs: Sequence[dict], tier: int, head: Optional[Head
         if rc != 0:
             raise ValueError("kso_predict_batch_routed: bad arguments")
         return dict(lat=lat, tiles=tiles, waves=waves, troof=troof, routed=routed)
+    if ensemble is not None and tier == 1:     # Tier A with an MLP ensemble for this family
+        rc = lib().kso_predict_batch_ensemble(int(bucket.family), n, colp, len(cols), int(bucket.dtype_bytes),
+                                              int(bucket.hq), int(bucket.hkv), int(bucket.head_dim), sp, ns,
+                                              ensemble.c, ensemble.k, _dp(lat), _ip(tiles), _ip(waves), _dp(troof))
+        if rc != 0:
+            raise ValueError("kso_predict_batch_ensemble: bad arguments")
+        return dict(lat=lat, tiles=tiles, waves=waves, troof=troof)
     if bounded is not None and tier == 1:      # Tier A with the bounded analytical head for this family
         rc = lib().kso_predict_batch_bounded(int(bucket.family), n, colp, len(cols), int(bucket.dtype_bytes),
                                              int(bucket.hq), int(bucket.hkv), int(bucket.head_dim), sp, ns,

@@ -88,6 +88,7 @@ class Workload:
     heads: Dict[int, Head] = field(default_factory=dict)
     grids: Dict[int, Grid] = field(default_factory=dict)
     bounded: Dict[int, BoundedHead] = field(default_factory=dict)   # families whose Tier-A head is the bounded form
+    ensembles: Dict[int, List[Head]] = field(default_factory=dict)  # families whose Tier-A head is an MLP ensemble
     n_steps: int = 0
     cfg_off: Optional[np.ndarray] = None  # CSR [n_cfg+1] int32 over steps
     step_params: Optional[dict] = None
@@ -135,6 +136,11 @@ def make_head(rng, n_in: int, h: int, bias_std: float = 0.1, w_std: float = 0.1)
         b2 = np.zeros(h, np.float32)
         b3 = 0.0
     return Head(n_in, h, h, W1, b1, W2, b2, w3, b3)
+
+
+def make_ensemble(rng, n_in: int, h_member: int, k: int, bias_std: float = 0.1, w_std: float = 0.1) -> List[Head]:
+    """k independently drawn MLP members of one shape ("small MLP ensemble"; Q17)."""
+    return [make_head(rng, n_in, h_member, bias_std, w_std) for _ in range(k)]
 
 
 def make_bounded_head(rng, n_in: int) -> BoundedHead:
