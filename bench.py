@@ -362,6 +362,17 @@ def run_extras(h: Harness, peaks):
                                    launches=3, note="streaming kernel, ~300 instructions per row: issue-bound")
     del st
     torch.cuda.empty_cache()
+    # NEXT-2: MLP ensembles (Q17), 4 members of width 32 per family of cfg2, packed into one pass of the Tier-A kernel
+    we = W.config2()
+    rng = np.random.Generator(np.random.PCG64(13))
+    we.ensembles = {f: W.make_ensemble(rng, 12, 32, 4) for f in list(we.heads)}
+    we.heads = {}
+    st = h.prepare(we)
+    ms = h.timed([lambda: h.predict(st)], EX_ITERS, EX_WARM)[:, 0]
+    ex["cfg2_ensemble_4x32"] = dict(ms=float(ms.mean()), predictions_per_s=float(we.n_rows / (ms.mean() * 1e-3)),
+                                    launches=1, note="same kernel and tile shape as cfg2's single heads (H = 128)")
+    del st
+    torch.cuda.empty_cache()
     # config 3: Tier B, 4M queries
     st = h.prepare(W.config3())
     sets = None if PROFILE else clone_sets(st, 8)

@@ -114,6 +114,19 @@ KS_API ks_status ks_create(ks_ctx **out, int device, void *cuda_stream);
 KS_API ks_status ks_load_heads(ks_ctx *ctx, ks_family family, int n_in, int h1, int h2, const float *W1,
                         const float *b1, const float *W2, const float *b2, const float *w3, float b3);
 
+/* Load (or replace) the Tier-A head of `family` with an MLP ENSEMBLE ("small MLP ensemble";
+ * DESIGN.md Q17): n_members MLPs n_in -> h -> h -> 1 of one shape, each as in ks_load_heads; the efficiency is
+ * the arithmetic mean of the members' sigmoid outputs, e = (1/k) sum_m sigmoid(z_m(x)), then the guard and
+ * eta = 1/e.  Arrays are HOST fp32 with the member index leading, copied: W1[k][n_in][h], b1[k][h],
+ * W2[k][h][h], b2[k][h], w3[k][h], b3[k].  The members run side by side in ONE pass of the Tier-A kernel
+ * (layer 1 concatenated, layer 2 block-diagonal), so k * h must be a supported hidden size:
+ * h in {32, 64, 128}, k <= KS_MAX_ENSEMBLE, k * h in {64, 128, 256}; anything else KS_EUNSUPPORTED.
+ * Replaces any head the family held. */
+#define KS_MAX_ENSEMBLE 8
+KS_API ks_status ks_load_head_ensemble(ks_ctx *ctx, ks_family family, int n_in, int h, int n_members,
+                                const float *W1, const float *b1, const float *W2, const float *b2,
+                                const float *w3, const float *b3);
+
 /* Load (or replace) the Tier-A head of `family` with the BOUNDED ANALYTICAL form (PAPER.md:197 Fig. 6, :201;
  * DESIGN.md Q15): utilisation e = gamma(x) - alpha(x) / W with W the kernel's wave count,
  * gamma(x) = sigmoid(w_gamma . x + b_gamma), alpha(x) = max(0, w_alpha . x + b_alpha), e clamped to

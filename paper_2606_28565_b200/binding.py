@@ -21,7 +21,7 @@ KS_TIER_NONE, KS_TIER_A, KS_TIER_B = range(3)
 KS_COL_I32, KS_COL_F32 = 0, 1
 KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
-EXPORTS = ["ks_create", "ks_load_heads", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
+EXPORTS = ["ks_create", "ks_load_heads", "ks_load_head_ensemble", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
            "ks_compose_steps_weighted",
            "ks_run_steps", "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
 
@@ -65,6 +65,7 @@ def load() -> C.CDLL:
     vp, i32, fp = C.c_void_p, C.c_int, C.POINTER(C.c_float)
     L.ks_create.argtypes = [C.POINTER(vp), i32, vp]
     L.ks_load_heads.argtypes = [vp, i32, i32, i32, i32, fp, fp, fp, fp, fp, C.c_float]
+    L.ks_load_head_ensemble.argtypes = [vp, i32, i32, i32, i32, fp, fp, fp, fp, fp, fp]
     L.ks_load_bounded_head.argtypes = [vp, i32, i32, fp, C.c_float, fp, C.c_float]
     L.ks_load_grid.argtypes = [vp, i32, C.POINTER(C.c_int32), fp, fp, fp]
     L.ks_predict_kernels.argtypes = [vp, C.POINTER(ks_desc_batch), i32, C.POINTER(ks_hw_spec), i32, i32, i32,
@@ -175,6 +176,18 @@ class Context:
         fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
         _check(self._lib.ks_load_heads(self._h, int(family), int(head.n_in), int(head.h1), int(head.h2), fp(W1),
                                        fp(b1), fp(W2), fp(b2), fp(w3), float(head.b3)), "ks_load_heads")
+
+    def load_head_ensemble(self, family: int, members) -> None:
+        """members: workloads.Head objects of one shape (n_in -> h -> h -> 1)."""
+        m0 = members[0]
+        if any((m.n_in, m.h1, m.h2) != (m0.n_in, m0.h1, m0.h1) for m in members):
+            raise ValueError("ensemble members must share one shape n_in -> h -> h -> 1")
+        st = lambda name: np.ascontiguousarray(np.stack([np.asarray(getattr(m, name), np.float32) for m in members]))
+        W1, b1, W2, b2, w3 = st("W1"), st("b1"), st("W2"), st("b2"), st("w3")
+        b3 = np.array([m.b3 for m in members], np.float32)
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        _check(self._lib.ks_load_head_ensemble(self._h, int(family), int(m0.n_in), int(m0.h1), len(members), fp(W1),
+                                               fp(b1), fp(W2), fp(b2), fp(w3), fp(b3)), "ks_load_head_ensemble")
 
     def load_bounded_head(self, family: int, head) -> None:
         wg = np.ascontiguousarray(head.w_gamma, dtype=np.float32)

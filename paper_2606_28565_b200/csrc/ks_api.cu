@@ -24,6 +24,8 @@ struct HeadState {
   float* w3 = nullptr;
   float* b2 = nullptr;
   float b3 = 0.0f;
+  int members = 1;           // > 1: MLP ensemble packed as one head of width h (Q17)
+  float b3m[KS_MAX_ENSEMBLE] = {};
 };
 
 struct GridState {
@@ -302,6 +304,9 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
           p.head[nb].w3 = hq.w3;
           p.head[nb].b2 = hq.b2;
           p.head[nb].b3 = hq.b3;
+          p.head[nb].members = hq.members;
+          if (hq.members > 1) p.any_ens = 1;
+          for (int m = 0; m < KS_MAX_ENSEMBLE; ++m) p.head[nb].b3m[m] = hq.b3m[m];
           p.tile_begin[nb] = tiles;
           tiles += (batches[q].n + 127) / 128;
           done[q] = true;
@@ -392,13 +397,13 @@ ks_status ks_set_gelu_mode(ks_ctx* c, int mode) {
   return KS_OK;
 }
 
-ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, const float* W1, const float* b1,
-                        const float* W2, const float* b2, const float* w3, float b3) {
-  if (!c || family < 0 || family >= KS_FAM_COUNT || !W1 || !b1 || !W2 || !b2 || !w3) return KS_EINVAL;
-  if (n_in <= 0 || h1 <= 0 || h2 <= 0) return KS_EINVAL;
-  if (c->sticky) return KS_ECUDA;
-  if ((n_in != 8 && n_in != 12 && n_in != 32) || h1 != h2 || (h1 != 64 && h1 != 128 && h1 != 256)) return KS_EUNSUPPORTED;
-  const int H = h1, K1 = ks_mlp_k1(n_in);
+namespace {
+
+// Builds the operand images of a dense head n_in -> H -> H and installs it for `family`.  members > 1:
+// the arrays hold an ensemble packed by ks_load_head_ensemble and b3m its per-member output biases.
+ks_status install_head(ks_ctx* c, ks_family family, int n_in, int H, const float* W1, const float* b1,
+                       const float* W2, const float* b2, const float* w3, float b3, int members, const float* b3m) {
+  const int K1 = ks_mlp_k1(n_in);
   const int n_real = n_in == 32 ? 22 : n_in;          // features 22..31 are identically zero (Q2)
   const int bias_row = n_real;
   // UMMA operand images, K-major no-swizzle: element (n, k) at ((k/8) * H + n) * 8 + k % 8
@@ -444,7 +449,52 @@ ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, c
   hs.w3 = static_cast<float*>(d3);
   hs.b2 = static_cast<float*>(d4);
   hs.b3 = b3;
+  hs.members = members;
+  for (int m = 0; m < members && m < KS_MAX_ENSEMBLE && b3m; ++m) hs.b3m[m] = b3m[m];
   return KS_OK;
+}
+
+}  // namespace
+
+ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, const float* W1, const float* b1,
+                        const float* W2, const float* b2, const float* w3, float b3) {
+  if (!c || family < 0 || family >= KS_FAM_COUNT || !W1 || !b1 || !W2 || !b2 || !w3) return KS_EINVAL;
+  if (n_in <= 0 || h1 <= 0 || h2 <= 0) return KS_EINVAL;
+  if (c->sticky) return KS_ECUDA;
+  if ((n_in != 8 && n_in != 12 && n_in != 32) || h1 != h2 || (h1 != 64 && h1 != 128 && h1 != 256)) return KS_EUNSUPPORTED;
+  return install_head(c, family, n_in, h1, W1, b1, W2, b2, w3, b3, 1, nullptr);
+}
+
+ks_status ks_load_head_ensemble(ks_ctx* c, ks_family family, int n_in, int h, int n_members, const float* W1,
+                                const float* b1, const float* W2, const float* b2, const float* w3, const float* b3) {
+  if (!c || family < 0 || family >= KS_FAM_COUNT || family == KS_FAM_ALLREDUCE || !W1 || !b1 || !W2 || !b2 || !w3 || !b3)
+    return KS_EINVAL;
+  if (n_in <= 0 || h <= 0 || n_members <= 0) return KS_EINVAL;
+  if (c->sticky) return KS_ECUDA;
+  const int H = h * n_members;
+  if ((n_in != 8 && n_in != 12 && n_in != 32) || n_members > KS_MAX_ENSEMBLE || (h != 32 && h != 64 && h != 128) ||
+      (H != 64 && H != 128 && H != 256))
+    return KS_EUNSUPPORTED;
+  if (n_members == 1) return install_head(c, family, n_in, h, W1, b1, W2, b2, w3, b3[0], 1, nullptr);
+  // Pack the members side by side into one head of width H = k h: layer 1 concatenated along its outputs,
+  // layer 2 block-diagonal (the zero blocks contribute exact zeros to the fp32 accumulators), layer 3
+  // concatenated; the kernels close one dot product + sigmoid per member and average (Q17).
+  std::vector<float> pW1((size_t)n_in * H), pb1(H), pW2((size_t)H * H, 0.0f), pb2(H), pw3(H);
+  for (int m = 0; m < n_members; ++m) {
+    const float* mW1 = W1 + (size_t)m * n_in * h;
+    const float* mW2 = W2 + (size_t)m * h * h;
+    for (int i = 0; i < n_in; ++i)
+      for (int j = 0; j < h; ++j) pW1[(size_t)i * H + m * h + j] = mW1[(size_t)i * h + j];
+    for (int i = 0; i < h; ++i)
+      for (int j = 0; j < h; ++j) pW2[(size_t)(m * h + i) * H + m * h + j] = mW2[(size_t)i * h + j];
+    for (int j = 0; j < h; ++j) {
+      pb1[m * h + j] = b1[(size_t)m * h + j];
+      pb2[m * h + j] = b2[(size_t)m * h + j];
+      pw3[m * h + j] = w3[(size_t)m * h + j];
+    }
+  }
+  return install_head(c, family, n_in, H, pW1.data(), pb1.data(), pW2.data(), pb2.data(), pw3.data(), 0.0f,
+                      n_members, b3);
 }
 
 ks_status ks_load_bounded_head(ks_ctx* c, ks_family family, int n_in, const float* w_gamma, float b_gamma,

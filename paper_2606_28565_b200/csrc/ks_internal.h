@@ -32,13 +32,15 @@ struct KsHeadDev {
   const float* w3;         // fp32 [H], holds w3 / 2
   const float* b2;         // fp32 [H] (the H = 256 kernel adds b2 in its fp32 epilogue)
   float b3;
-  int32_t pad;
+  int32_t members;         // > 1: MLP ensemble (Q17) of `members` heads, H / members columns each:
+                           // W1/b1/b2/w3 concatenated, W2 block-diagonal, one output bias per member
+  float b3m[KS_MAX_ENSEMBLE];
 };
 struct KsMlpParams {
   KsBucketDev bk[KS_MLP_MAX_BUCKETS];
   KsHeadDev head[KS_MLP_MAX_BUCKETS];
   int32_t tile_begin[KS_MLP_MAX_BUCKETS + 1];   // prefix of 128-row tiles per bucket
-  int32_t n_buckets, n_specs, gelu_mode, pad;
+  int32_t n_buckets, n_specs, gelu_mode, any_ens;   // any_ens: some head of the launch is an ensemble
   KsSpecTable specs;
 };
 // n_in in {8,12,32}; h in {64,128,256}; all buckets of one launch share (n_in, h)

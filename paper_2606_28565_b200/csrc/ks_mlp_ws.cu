@@ -25,6 +25,7 @@
 // on the waiter's own progress), so single-bit phase parity is sufficient.
 // The t_roof ring has 8 entries: the producer can be at most 7 items ahead of EPI2 (item q+8 needs
 // mma1_done(q+6); MMA1(q+6) is issued after MMA2(q+3), which waits for d2_free(q+1) >= d2_free(q)).
+#include <type_traits>
 #include "ks_mlp_common.cuh"
 
 namespace {
@@ -184,7 +185,7 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
 }
 
 // ------------------------------------------------------------------ EPI2 (warps 12-19): D2 -> 2 GELU . w3/2 -> latency
-template <int NIN, int H, int GM>
+template <int NIN, int H, int GM, bool ENS>
 KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
                      uint64_t* bars, const uint32_t tmem_base) {
   using C = WsCfg<NIN, H>;
@@ -198,7 +199,10 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     const Range tr = bucket_range(tm, b, t_lo, t_hi);
     const KsBucketDev& bk = p.bk[b];
     const float* sw3 = reinterpret_cast<const float*>(smem + C::OFF_W3) + b * H;
-    const float b3 = p.head[b].b3;
+    const KsHeadDev& hd = p.head[b];
+    const float b3 = hd.b3;
+    const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble, members of H / members columns
+    const int ens_mask = members > 1 ? H / 16 / members - 1 : 0;     // member width is 32 or 64: a power-of-two chunk count
     const int tile0 = tm.tb[b], ne = tm.ne[b];
     for (int t = tr.lo; t < tr.hi; ++t) {
       const int pos = (t - tile0) * kRows + r;
@@ -237,21 +241,37 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
             }
           }
         };
+        float esum = 0.0f;                         // ensemble: sum of the members' efficiencies so far
+        auto sweep = [&](auto ens) {
+          int m = 0;
 #pragma unroll 1
-        for (int c = 0; c < H / 16; c += 2) {
-          ks_tmem_ld_wait();
-          ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
-          act_dot(accA, c);
-          ks_tmem_ld_wait();
-          if (c + 2 < H / 16) ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
-          act_dot(accB, c + 1);
-        }
+          for (int c = 0; c < H / 16; c += 2) {
+            ks_tmem_ld_wait();
+            ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
+            act_dot(accA, c);
+            ks_tmem_ld_wait();
+            if (c + 2 < H / 16) ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
+            act_dot(accB, c + 1);
+            if (decltype(ens)::value && ((c + 2) & ens_mask) == 0) {   // last column of member m (Q17)
+              const float z = ((z0 + z1) + (z2 + z3)) + hd.b3m[m++];
+              esum += __fdividef(1.0f, 1.0f + __expf(-z));
+              z0 = z1 = z2 = z3 = 0.0f;
+            }
+          }
+        };
+        if (members > 1) sweep(std::true_type{}); else sweep(std::false_type{});
         ks_tc_fence_before();                      // orders this thread's tcgen05.ld before MMA2(q+2)
         ks_mbar_arrive(bars + BAR_D2_FREE + buf);
         if (valid) {
-          const float z = ((z0 + z1) + (z2 + z3)) + b3;
-          // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
-          const float eta = fminf(1.0f + __expf(-z), 1024.0f);
+          float eta;
+          if (members > 1) {
+            // e = mean of the members' sigmoids; eta = 1/e with the same guard e >= 2^-10
+            eta = fminf(__fdividef((float)members, esum), 1024.0f);
+          } else {
+            const float z = ((z0 + z1) + (z2 + z3)) + b3;
+            // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
+            eta = fminf(1.0f + __expf(-z), 1024.0f);
+          }
           bk.lat[(long long)s * bk.n + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
         }
       }
@@ -397,8 +417,14 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
     if (p.gelu_mode == 0) epi1_items<NIN, H, 0>(p, (uint32_t)(t_hi - t_lo) * (uint32_t)p.n_specs, smem, bars, tmem_base);
     else epi1_items<NIN, H, 1>(p, (uint32_t)(t_hi - t_lo) * (uint32_t)p.n_specs, smem, bars, tmem_base);
   } else if (warp < kMmaWarp) {
-    if (p.gelu_mode == 0) epi2_all<NIN, H, 0>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
-    else epi2_all<NIN, H, 1>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    // four copies of the role, one runs: the ensemble bookkeeping stays out of the single-head loop
+    if (p.any_ens) {
+      if (p.gelu_mode == 0) epi2_all<NIN, H, 0, true>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+      else epi2_all<NIN, H, 1, true>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    } else {
+      if (p.gelu_mode == 0) epi2_all<NIN, H, 0, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+      else epi2_all<NIN, H, 1, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    }
   } else if (tid == kMmaWarp * 32) {
     mma_all<NIN, H>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   }

@@ -22,6 +22,7 @@
 // as one more K step): dropping the bias rows of W2 and the ones-block is what makes 225 KB fit.
 // Every mbarrier completes exactly once per item, so its phase parity is q & 1; a waiter for item q
 // always runs before the completion for item q+1 can happen (that one depends on the waiter).
+#include <type_traits>
 #include "ks_mlp_common.cuh"
 
 namespace {
@@ -177,7 +178,7 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
 }
 
 // ------------------------------------------------------------------ EPI2 (warps 12-19)
-template <int NIN, int GM>
+template <int NIN, int GM, bool ENS>
 KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
                      uint64_t* bars, const uint32_t tmem_base) {
   using C = Cfg256<NIN>;
@@ -200,7 +201,10 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     sw3[e] = __ldg(p.head[b].w3 + e);
     sb2[e] = __ldg(p.head[b].b2 + e);
     ks_bar_sync(2, 2 * 128);
-    const float b3 = p.head[b].b3;
+    const KsHeadDev& hd = p.head[b];
+    const float b3 = hd.b3;
+    const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble (2, 4 or 8 members here)
+    const int ens_mask = members > 1 ? H / 16 / members - 1 : 0;     // chunks per member - 1 (member width 32 .. 128)
     const int tile0 = tm.tb[b], ne = tm.ne[b];
     for (int t = tr.lo; t < tr.hi; ++t) {
       const int pos = (t - tile0) * kRows + r;
@@ -235,28 +239,40 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
             }
           }
         };
+        float esum = 0.0f;                         // ensemble: sum of this half's members' efficiencies
+        auto sweep = [&](auto ens) {
+          int m = wg * (members >> 1);             // first member of this warpgroup's 128 columns
 #pragma unroll 1
-        for (int c = 0; c < 8; c += 2) {
-          ks_tmem_ld_wait();
-          ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
-          act_dot(accA, c);
-          ks_tmem_ld_wait();
-          if (c + 2 < 8) {
-            ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
-          } else {                                                  // D2 is drained: MMA2(q+1) may overwrite it
-            ks_tc_fence_before();
-            ks_mbar_arrive(bars + BAR_D2_FREE);
+          for (int c = 0; c < 8; c += 2) {
+            ks_tmem_ld_wait();
+            ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
+            act_dot(accA, c);
+            ks_tmem_ld_wait();
+            if (c + 2 < 8) {
+              ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
+            } else {                                                  // D2 is drained: MMA2(q+1) may overwrite it
+              ks_tc_fence_before();
+              ks_mbar_arrive(bars + BAR_D2_FREE);
+            }
+            act_dot(accB, c + 1);
+            if (decltype(ens)::value && ((c + 2) & ens_mask) == 0) {  // last column of member m (Q17)
+              const float zm = ((z0 + z1) + (z2 + z3)) + hd.b3m[m++];
+              esum += __fdividef(1.0f, 1.0f + __expf(-zm));
+              z0 = z1 = z2 = z3 = 0.0f;
+            }
           }
-          act_dot(accB, c + 1);
-        }
-        float z = (z0 + z1) + (z2 + z3);
+        };
+        if (members > 1) sweep(std::true_type{}); else sweep(std::false_type{});
+        // single head: partial logit of this half; ensemble: partial sum of efficiencies
+        float z = members > 1 ? esum : (z0 + z1) + (z2 + z3);
         // the two column halves meet in shared memory (double-buffered by item parity)
         if (wg == 1) zpart[(q & 1u) * kRows + r] = z;
         ks_bar_sync(2, 2 * 128);
         if (wg == 0 && valid) {
-          z += zpart[(q & 1u) * kRows + r] + b3;
-          // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
-          const float eta = fminf(1.0f + __expf(-z), 1024.0f);
+          z += zpart[(q & 1u) * kRows + r];
+          // eta = 1/e, guarded at e >= 2^-10 (Q3): 1 + exp(-z) for one head, k / sum of the members'
+          // sigmoids for an ensemble; Eq. 2 floor after eta
+          const float eta = fminf(members > 1 ? __fdividef((float)members, z) : 1.0f + __expf(-(z + b3)), 1024.0f);
           bk.lat[(long long)s * bk.n + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
         }
       }
@@ -387,8 +403,13 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
     if (p.gelu_mode == 0) epi1_items<NIN, 0>(p, n_items, smem, bars, tmem_base);
     else epi1_items<NIN, 1>(p, n_items, smem, bars, tmem_base);
   } else if (warp < kMmaWarp) {
-    if (p.gelu_mode == 0) epi2_all<NIN, 0>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
-    else epi2_all<NIN, 1>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    if (p.any_ens) {
+      if (p.gelu_mode == 0) epi2_all<NIN, 0, true>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+      else epi2_all<NIN, 1, true>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    } else {
+      if (p.gelu_mode == 0) epi2_all<NIN, 0, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+      else epi2_all<NIN, 1, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+    }
   } else if (tid == kMmaWarp * 32) {
     mma_all<NIN>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   }

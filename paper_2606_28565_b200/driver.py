@@ -64,6 +64,8 @@ def to_pinned(w: Workload) -> List[DeviceBucket]:
 def load_models(ctx: B.Context, w: Workload) -> None:
     for fam, h in w.heads.items():
         ctx.load_heads(fam, h)
+    for fam, members in getattr(w, "ensembles", {}).items():  # families whose Tier-A head is an MLP ensemble
+        ctx.load_head_ensemble(fam, members)
     for fam, bh in getattr(w, "bounded", {}).items():      # families whose Tier-A head is the bounded analytical form
         ctx.load_bounded_head(fam, bh)
     for fam, g in w.grids.items():

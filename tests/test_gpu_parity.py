@@ -39,8 +39,9 @@ def oracle_all(w, tier=None, rows=None):
     for i, b in enumerate(w.buckets):
         r = None if rows is None else rows[i]
         bnd = O.Bounded(w.bounded[b.family]) if (tier == W.TIER_A and b.family in getattr(w, "bounded", {})) else None
+        ens = O.Ensemble(w.ensembles[b.family]) if (tier == W.TIER_A and b.family in getattr(w, "ensembles", {})) else None
         out.append(O.predict_bucket(b, w.specs, tier, head=heads.get(b.family), grid=grids.get(b.family), rows=r,
-                                    bounded=bnd))
+                                    bounded=bnd, ensemble=ens))
     return out
 
 
@@ -377,6 +378,63 @@ def test_bounded_head_closed_forms_and_replacement(ks):
             c2.load_bounded_head(fam, W.BoundedHead(9, np.zeros(9, np.float32), 0.0, np.zeros(9, np.float32), 0.0))
         finally:
             c2.close()
+
+
+# ------------------------------------------------------------------ MLP ensembles (NEXT-2, Q17)
+@pytest.mark.parametrize("n_in,h,k", [(12, 32, 4), (12, 64, 2), (8, 32, 2), (32, 64, 4), (32, 128, 2), (12, 32, 8)])
+def test_ensemble_parity(ks, n_in, h, k):
+    B, D = ks
+    w = W.config2(n=20011, n_in=n_in, h=h * k) if n_in != 32 else W.config5(n_rows=12007, n_specs=3, n_layers=4, h=h * k)
+    rng = np.random.Generator(np.random.PCG64(1000 + n_in + h + k))
+    fams = [b.family for b in w.buckets]
+    # every other family gets an ensemble of k members of width h, the rest keep a single head of width k h:
+    # both kinds share the kernel launch
+    w.ensembles = {f: W.make_ensemble(rng, n_in, h, k, bias_std=0.2, w_std=0.2) for f in fams[::2]}
+    w.heads = {f: hd for f, hd in w.heads.items() if f not in w.ensembles}
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        g = D.predict(ctx, w)
+    finally:
+        ctx.close()
+    o = oracle_all(w, W.TIER_A)
+    errs = [check_bucket(gi, oi, TOL_MLP, what=f"{w.name}/bucket{i}") for i, (gi, oi) in enumerate(zip(g, o))]
+    print("ensemble", (n_in, h, k), "max rel err per bucket", errs, "ensemble families", sorted(w.ensembles))
+
+
+def test_ensemble_closed_forms_reductions_and_shapes(ks):
+    B, D = ks
+    w = W.config1()
+    fam = w.buckets[0].family
+    z = np.zeros
+
+    def const_member(h, b3):
+        return W.Head(8, h, h, z((8, h), np.float32), z(h, np.float32), z((h, h), np.float32), z(h, np.float32),
+                      z(h, np.float32), float(b3))
+
+    rng = np.random.Generator(np.random.PCG64(5))
+    one = W.make_head(rng, 8, 64, bias_std=0.2, w_std=0.2)
+    ctx = B.Context(0)
+    try:
+        # members with constant outputs 0.8 and 0.5: e = 0.65 (the mean of the efficiencies, Q17)
+        ctx.load_head_ensemble(fam, [const_member(32, np.log(4.0)), const_member(32, 0.0)])
+        g = D.predict(ctx, w)
+        want = np.maximum(g[0]["troof"].astype(np.float64) / 0.65, w.specs[0]["t0"])
+        assert rel_err(g[0]["lat"], want).max() <= 2e-6
+        # two copies of one member = that member alone (different kernel shape, same arithmetic up to rounding)
+        ctx.load_heads(fam, one)
+        single = D.predict(ctx, w)[0]["lat"].copy()
+        ctx.load_head_ensemble(fam, [one, one])
+        twice = D.predict(ctx, w)[0]["lat"]
+        assert rel_err(twice, single).max() <= 2e-6
+        ctx.load_head_ensemble(fam, [one])                        # k = 1 is the plain head, bit for bit
+        assert np.array_equal(D.predict(ctx, w)[0]["lat"], single)
+        for h, k in ((16, 4), (32, 3), (64, 8), (128, 4), (32, 9)):
+            with pytest.raises(B.KsError) as ei:
+                ctx.load_head_ensemble(fam, [const_member(h, 0.0)] * k)
+            assert ei.value.status == B.KS_EUNSUPPORTED
+    finally:
+        ctx.close()
 
 
 # ------------------------------------------------------------------ density-routed Tier B (NEXT-1)
