@@ -1,0 +1,176 @@
+"""Pins for the oracle scheduler (oracle/sched.py; Q18): hand-worked schedules,
+closed forms for the uncontended regime, conservation laws and per-step invariants under KV pressure."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import sched as S
+
+BIG = S.SchedConfig(max_num_batched_tokens=8192, max_num_seqs=256, block_size=16, num_blocks=1 << 20)
+
+
+def run(cfg, arrival, P, O, dt=1.0):
+    s = S.Scheduler(cfg, arrival, P, O)
+    end, priced, batches = S.simulate(s, lambda b: dt)
+    return s, end, batches
+
+
+def test_single_request_prefill_then_decodes():
+    # P = 10, 3 output tokens: the prefill step emits token 1, two decode steps emit tokens 2 and 3
+    s, end, batches = run(BIG, [0.0], [10], [3])
+    assert batches == [[(0, 10, 0)], [(0, 1, 10)], [(0, 1, 11)]]
+    assert s.first_token == [1.0] and s.finish == [3.0] and end == 3.0
+
+
+def test_chunked_prefill_splits_a_prompt_over_the_token_budget():
+    cfg = S.SchedConfig(256, 8, 16, 4096)
+    s, end, batches = run(cfg, [0.0], [1000], [2])
+    assert [b[0][1:] for b in batches] == [(256, 0), (256, 256), (256, 512), (232, 768), (1, 1000)]
+    assert s.first_token == [4.0] and s.finish == [5.0]
+
+
+def test_running_requests_come_first_and_prefill_takes_the_leftover_budget():
+    # three decoding requests + a 1000-token prompt arriving later, budget 256: chunk = 256 - 3 = 253
+    cfg = S.SchedConfig(256, 8, 16, 4096)
+    s = S.Scheduler(cfg, [0.0, 0.0, 0.0, 1.5], [4, 5, 6, 1000], [50, 50, 50, 1])
+    assert s.step(0.0) == [(0, 4, 0), (1, 5, 0), (2, 6, 0)]
+    s.commit(1.0)
+    assert s.step(1.0) == [(0, 1, 4), (1, 1, 5), (2, 1, 6)]      # request 3 has not arrived yet
+    s.commit(2.0)
+    assert s.step(2.0) == [(0, 1, 5), (1, 1, 6), (2, 1, 7), (3, 253, 0)]
+    s.commit(3.0)
+    assert s.step(3.0)[-1] == (3, 253, 253)
+
+
+def test_fcfs_by_arrival_then_index_and_max_num_seqs():
+    cfg = S.SchedConfig(8192, 2, 16, 4096)
+    s = S.Scheduler(cfg, [0.3, 0.1, 0.1, 0.2], [8, 8, 8, 8], [2, 2, 2, 2])
+    assert [r for r, _, _ in s.step(0.5)] == [1, 2]                # earliest arrivals, tie by index; cap S = 2
+    s.commit(1.0)
+    assert [r for r, _, _ in s.step(1.0)] == [1, 2]
+    s.commit(2.0)                                                  # both finish
+    assert [r for r, _, _ in s.step(2.0)] == [3, 0]
+
+
+def test_uncontended_closed_form():
+    # all requests at t = 0, budget and cache ample: every prompt is prefilled in step 1 and request i
+    # finishes at step O_i; with a constant step time dt: first token at dt, finish at O_i dt
+    rng = np.random.Generator(np.random.PCG64(3))
+    P = rng.integers(1, 60, 40).tolist()
+    O = rng.integers(1, 30, 40).tolist()
+    s, end, batches = run(BIG, [0.0] * 40, P, O, dt=0.5)
+    assert s.first_token == [0.5] * 40
+    assert s.finish == [0.5 * o for o in O]
+    assert end == 0.5 * max(O) and s.n_steps == max(O)
+    assert [len(b) for b in batches] == [sum(1 for o in O if o > k) for k in range(max(O))]
+
+
+def test_idle_gaps_jump_to_the_next_arrival():
+    s, end, _ = run(BIG, [0.0, 10.0], [5, 5], [2, 2], dt=1.0)
+    assert s.finish == [2.0, 12.0] and s.first_token == [1.0, 11.0]
+
+
+def test_preemption_recomputes_the_newest_request():
+    # 6 blocks of 4 tokens.  Two requests of 8 prompt tokens: 2 blocks each.  Decoding grows both until the
+    # cache is full; the request at the back of the running queue (1) is preempted and recomputed later.
+    cfg = S.SchedConfig(64, 4, 4, 6)
+    s = S.Scheduler(cfg, [0.0, 0.0], [8, 8], [8, 6])
+    log = []
+    now = 0.0
+    while not s.done():
+        b = s.step(now)
+        log.append(b)
+        now += 1.0
+        s.commit(now)
+        assert s.free_blocks >= 0 and sum(s.blocks) + s.free_blocks == 6
+    # step 1: both prefill (2 + 2 blocks).  steps 2-5: decode at hist 8..11, a third block each at step 2
+    # (tokens 9..12 fit in 3 blocks).  step 6: hist 12 needs a 4th block for request 0 (free = 0):
+    # request 1 is preempted (its 5 generated tokens are kept, to be recomputed), request 0 runs alone.
+    assert log[0] == [(0, 8, 0), (1, 8, 0)]
+    assert log[1] == [(0, 1, 8), (1, 1, 9 - 1)]
+    assert log[5] == [(0, 1, 12)]
+    assert s.n_preempt == [0, 1]
+    # request 0 needs 8 + 8 - 1 = 15 computed tokens -> 4 blocks until it finishes (step 8); request 1
+    # cannot be re-admitted while a preemption happened in the step, then needs ceil(13/4) = 4 blocks
+    # with only 2 free, so it waits for request 0 to finish, then recomputes 8 + 5 = 13 tokens in one
+    # step (emitting token 6 = its last)
+    assert s.finish[0] == 8.0
+    assert log[8] == [(1, 13, 0)] and s.finish[1] == 9.0
+    assert s.tokens_scheduled == (8 + 7) + (8 + 4) + 13        # request 0; request 1 before and after its preemption
+    assert s.tokens_scheduled == sum(n for b in log for _, n, _ in b)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_invariants_and_conservation_under_pressure(seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n = 60
+    cfg = S.SchedConfig(int(rng.integers(64, 512)), int(rng.integers(4, 32)), 16, int(rng.integers(40, 120)))
+    arrival = np.sort(rng.uniform(0, 30, n)).tolist()
+    P = rng.integers(1, 400, n).tolist()
+    O = rng.integers(1, 80, n).tolist()
+    s = S.Scheduler(cfg, arrival, P, O)
+    now, steps = 0.0, 0
+    emitted = [0] * n
+    while not s.done():
+        b = s.step(now)
+        if not b:
+            assert not s.running and not s.waiting                # idle only when nothing is queued
+            now = max(now, s.next_arrival())
+            continue
+        assert 0 < sum(x[1] for x in b) <= cfg.max_num_batched_tokens          # token budget
+        assert len(s.running) <= cfg.max_num_seqs and len({x[0] for x in b}) == len(b)
+        assert [x[0] for x in b] == s.running[:len(b)]            # the batch is a prefix of the running queue
+        assert sum(s.blocks) + s.free_blocks == cfg.num_blocks and s.free_blocks >= 0
+        for r, n_new, hist in b:
+            assert arrival[r] <= now and hist == s.c[r] and n_new >= 1
+            assert s.blocks[r] * cfg.block_size >= hist + n_new   # KV blocks cover every scheduled token
+            if hist + n_new == s.n_tok[r]:
+                emitted[r] += 1
+        now += 0.01 + 1e-5 * sum(x[1] for x in b)
+        s.commit(now)
+        steps += 1
+        assert steps < 100000
+    assert emitted == O                                           # every request emits exactly max_new tokens
+    assert all(math.isfinite(f) and f >= ft > a for f, ft, a in zip(s.finish, s.first_token, arrival))
+    assert s.free_blocks == cfg.num_blocks and not s.running and not s.waiting
+    # conservation: tokens computed = prompt + generated - 1 per request, plus what preemptions threw away
+    assert s.tokens_scheduled >= sum(p + o - 1 for p, o in zip(P, O))
+    assert (s.tokens_scheduled == sum(p + o - 1 for p, o in zip(P, O))) == (sum(s.n_preempt) == 0)
+
+
+def test_rejects_a_request_that_can_never_fit():
+    with pytest.raises(ValueError):
+        S.Scheduler(S.SchedConfig(64, 4, 16, 4), [0.0], [60], [10])
+
+
+def test_step_rows_follow_the_mixed_step_pricing_rule():
+    # two decodes (cached context 100 and 7) + one 32-token prefill chunk with 64 tokens of history
+    m = S.Model(n_layers=4, hidden=64, ffn=128, vocab=1000, hq=4, hkv=2, head_dim=16, tp=2)
+    rows = S.step_rows([(5, 1, 100), (9, 1, 7), (2, 32, 64)], m)
+    T = 34
+    assert rows[0] == ([[T, 128, 64], [T, 64, 64], [T, 256, 64], [T, 64, 128], [3, 1000, 64]], [4, 4, 4, 4, 1])
+    assert rows[2] == ([[1, 1, 101], [1, 1, 8], [1, 32, 96]], [4, 4, 4])      # per request: (B, q, kv = hist + q)
+    assert rows[3] == ([[T * 64, 4], [T * 64, 0], [T * 96, 2], [T * 64, 3], [T * 128, 1], [T * 64, 0]], [1, 4, 4, 4, 4, 1])
+    assert rows[4] == ([[T * 64 * 2, 2]], [8])                                # two all-reduces per layer
+    # kernel launches of the step: n = L (4 GEMM + 3 attention + 4 elementwise + 2 all-reduce) + lm_head + embed + final norm
+    assert sum(sum(mm) for _, mm in rows.values()) == 4 * (4 + 3 + 4 + 2) + 3
+
+
+def test_price_steps_equals_hand_composition():
+    from oracle import oracle as O
+    from paper_2606_28565_b200 import workloads as W
+    m = S.Model()
+    spec = W.spec_gb200()
+    batch = [(0, 1, 500), (1, 1, 2000), (2, 512, 1024)]
+    t = S.price_steps([batch], m, spec, 0, W.STEP_PARAMS_CFG4)[0]
+    # by hand: L x (4 GEMMs + attention rows + 4 elementwise) + lm_head + embed + final norm, Eq. 4 GPU-bound
+    def one(f, v, **kw):
+        return O.predict_one(O.make_desc(f, v, **kw), O.make_spec(spec), 0)[0]
+    T = 514
+    layer = (one(0, [T, 6144, 4096]) + one(0, [T, 4096, 4096]) + one(0, [T, 28672, 4096]) + one(0, [T, 4096, 14336])
+             + sum(one(2, [1, q, h + q], hq=32, hkv=8, d=128) for _, q, h in batch)
+             + one(3, [T * 4096, 0]) + one(3, [T * 40 * 128, 2]) + one(3, [T * 16 * 128, 3]) + one(3, [T * 14336, 1]))
+    body = 32 * layer + one(0, [3, 131072, 4096]) + one(3, [T * 4096, 4]) + one(3, [T * 4096, 0])
+    n = 32 * (4 + 3 + 4) + 3
+    assert abs(t - (body + n * 4e-6)) < 1e-12
