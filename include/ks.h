@@ -192,6 +192,81 @@ KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const i
                        const ks_step_params *params, const int32_t *cfg_off, int n_cfg,
                        ks_mem_space space, float *const *latency, float *step_latency, float *cfg_latency);
 
+/* ------------------------------------------------------------------------------------------------
+ * Serving scheduler and the closed simulation loop.
+ *
+ * ks_sched is one replica's scheduler, HOST logic (the paper's scheduler is host code too): "a single
+ * token-budget loop advances every request's computed-token count toward its target", with continuous
+ * batching, chunked prefill, FCFS queuing and preemption/recompute under KV pressure (
+ * the exact rules are DESIGN.md Q18; prefix caching is not modelled).  It needs no GPU and no ks_ctx.
+ * ks_sim_run closes the loop for many replicas at once: every iteration each unfinished replica forms
+ * the batch of its next step, the batches' kernel rows (layer-homogeneous form :231) are
+ * priced by ONE pass of the GPU path (ks_run_steps), and each replica's clock advances by its own
+ * step time.  All pointers below are HOST pointers. */
+typedef struct ks_sched ks_sched;
+
+typedef struct {
+  int32_t max_num_batched_tokens;  /* T: token budget of one step, >= 1 */
+  int32_t max_num_seqs;            /* most requests running at once, >= 1 */
+  int32_t block_size;              /* tokens per KV-cache block, >= 1 */
+  int32_t num_blocks;              /* KV-cache blocks, >= 1 */
+} ks_sched_config;
+
+/* Dense decoder the steps are priced for. */
+typedef struct {
+  int32_t n_layers, hidden, ffn, vocab, hq, hkv, head_dim;
+  int32_t dtype_bytes;             /* bytes per tensor element (1, 2 or 4) */
+  int32_t tp;                      /* tensor-parallel degree; > 1 adds two all-reduces per layer */
+} ks_model_desc;
+
+typedef struct {
+  int64_t n_steps, tokens_scheduled, n_preemptions;
+  int32_t n_requests, n_finished, n_running, n_waiting, free_blocks, pad;
+} ks_sched_stats;
+
+KS_API ks_status ks_sched_create(ks_sched **out, const ks_sched_config *cfg);
+/* Append n requests (arrival time in seconds, prompt tokens >= 1, tokens to emit >= 1).  Queue order is
+ * FCFS by (arrival, order of insertion).  KS_EINVAL if a request alone can never fit the KV cache
+ * (ceil((prompt + max_new) / block_size) > num_blocks) or a value is not finite / not positive;
+ * KS_ESTATE once the first step has been formed. */
+KS_API ks_status ks_sched_add_requests(ks_sched *s, int n, const double *arrival, const int32_t *prompt_len,
+                                const int32_t *max_new);
+/* Form the batch of the step that starts at `now`.  Writes up to cap entries (request index, new tokens
+ * n_new >= 1, cached history hist = computed tokens before the step) in queue order and their number
+ * to *n_sched; KS_EINVAL if cap is too small (max_num_seqs always suffices).  *n_sched == 0 means the
+ * replica is idle: *next_arrival then holds the arrival time of the next request, or +inf when every
+ * request has finished.  KS_ESTATE if the previous batch has not been committed. */
+KS_API ks_status ks_sched_step(ks_sched *s, double now, int32_t cap, int32_t *n_sched, int32_t *req,
+                        int32_t *n_new, int32_t *hist, double *next_arrival);
+/* The step formed last completes at t_end: computed-token counts advance, requests whose known tokens are
+ * all computed emit one token (the first one fixes first_token, the max_new-th finish; the request then
+ * leaves and frees its blocks). */
+KS_API ks_status ks_sched_commit(ks_sched *s, double t_end);
+/* Per-request results, each [n_requests] in insertion order (any pointer may be NULL): time of the first
+ * and of the last emitted token (NaN while not reached), number of preemptions. */
+KS_API ks_status ks_sched_results(ks_sched *s, double *first_token, double *finish, int32_t *n_preempt);
+KS_API ks_status ks_sched_get_stats(ks_sched *s, ks_sched_stats *out);
+KS_API ks_status ks_sched_destroy(ks_sched *s);
+
+typedef struct {
+  int64_t iterations;              /* passes of the GPU path */
+  int64_t steps;                   /* serving steps priced, all replicas */
+  int64_t rows;                    /* kernel rows priced */
+  int64_t kernel_instances;        /* sum of multiplicities = kernel launches those steps stand for */
+} ks_sim_stats;
+
+/* Run n_replicas schedulers in lock step until all have finished or max_iters iterations have run
+ * (max_iters <= 0: no limit).  clock[r] (in/out) is replica r's simulated time.  Step times are
+ * Eq. 4 wall times in fp32 from the GPU path for `spec`, `tier` (heads/grids as loaded in ctx) and
+ * `params`; clocks accumulate in double.  Optional log (may be NULL with log_cap 0): step_replica[i],
+ * step_time[i] for the i-th priced step in the order they were committed (iteration-major, replica
+ * order within an iteration); *n_logged receives the count (steps beyond log_cap are not logged).
+ * Blocking; uses the context's stream. */
+KS_API ks_status ks_sim_run(ks_ctx *ctx, ks_sched *const *scheds, double *clock, int n_replicas,
+                     const ks_model_desc *model, const ks_hw_spec *spec, ks_tier tier,
+                     const ks_step_params *params, int64_t max_iters, int32_t *step_replica, float *step_time,
+                     int64_t log_cap, int64_t *n_logged, ks_sim_stats *stats);
+
 /* Counters: number of kernel launches this context has enqueued so far (for gpu_launches). */
 KS_API ks_status ks_get_launch_count(ks_ctx *ctx, int64_t *out);
 

@@ -23,7 +23,9 @@ KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
 EXPORTS = ["ks_create", "ks_load_heads", "ks_load_head_ensemble", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
            "ks_compose_steps_weighted",
-           "ks_run_steps", "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
+           "ks_run_steps", "ks_sched_create", "ks_sched_add_requests", "ks_sched_step", "ks_sched_commit",
+           "ks_sched_results", "ks_sched_get_stats", "ks_sched_destroy", "ks_sim_run",
+           "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
 
 
 class KsError(RuntimeError):
@@ -48,6 +50,26 @@ class ks_desc_batch(C.Structure):
 class ks_step_params(C.Structure):
     _fields_ = [("c_disp", C.c_float), ("floor_l", C.c_float), ("c_ovl", C.c_float), ("c_tail", C.c_float),
                 ("body_scale", C.c_float)]
+
+
+class ks_sched_config(C.Structure):
+    _fields_ = [("max_num_batched_tokens", C.c_int32), ("max_num_seqs", C.c_int32), ("block_size", C.c_int32),
+                ("num_blocks", C.c_int32)]
+
+
+class ks_model_desc(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in ("n_layers", "hidden", "ffn", "vocab", "hq", "hkv", "head_dim",
+                                         "dtype_bytes", "tp")]
+
+
+class ks_sched_stats(C.Structure):
+    _fields_ = [("n_steps", C.c_int64), ("tokens_scheduled", C.c_int64), ("n_preemptions", C.c_int64),
+                ("n_requests", C.c_int32), ("n_finished", C.c_int32), ("n_running", C.c_int32),
+                ("n_waiting", C.c_int32), ("free_blocks", C.c_int32), ("pad", C.c_int32)]
+
+
+class ks_sim_stats(C.Structure):
+    _fields_ = [("iterations", C.c_int64), ("steps", C.c_int64), ("rows", C.c_int64), ("kernel_instances", C.c_int64)]
 
 
 _lib = None
@@ -76,6 +98,17 @@ def load() -> C.CDLL:
                                             i32, i32, C.POINTER(ks_step_params), vp, i32, i32, vp, vp]
     L.ks_run_steps.argtypes = [vp, C.POINTER(ks_desc_batch), C.POINTER(vp), i32, C.POINTER(ks_hw_spec), i32, i32,
                                i32, C.POINTER(ks_step_params), vp, i32, i32, C.POINTER(vp), vp, vp]
+    dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int32)
+    L.ks_sched_create.argtypes = [C.POINTER(vp), C.POINTER(ks_sched_config)]
+    L.ks_sched_add_requests.argtypes = [vp, i32, dp, ip, ip]
+    L.ks_sched_step.argtypes = [vp, C.c_double, C.c_int32, ip, ip, ip, ip, dp]
+    L.ks_sched_commit.argtypes = [vp, C.c_double]
+    L.ks_sched_results.argtypes = [vp, dp, dp, ip]
+    L.ks_sched_get_stats.argtypes = [vp, C.POINTER(ks_sched_stats)]
+    L.ks_sched_destroy.argtypes = [vp]
+    L.ks_sim_run.argtypes = [vp, C.POINTER(vp), dp, i32, C.POINTER(ks_model_desc), C.POINTER(ks_hw_spec), i32,
+                             C.POINTER(ks_step_params), C.c_int64, ip, fp, C.c_int64, C.POINTER(C.c_int64),
+                             C.POINTER(ks_sim_stats)]
     L.ks_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.ks_set_gelu_mode.argtypes = [vp, i32]
     L.ks_destroy.argtypes = [vp]
@@ -259,3 +292,93 @@ class Context:
                                       int(n_steps), C.byref(p), _ptr(cfg_off), int(n_cfg), int(space),
                                       _ptr_array(latency) if latency is not None else None, _ptr(step_latency),
                                       _ptr(cfg_latency)), "ks_run_steps")
+
+
+class Scheduler:
+    """One replica's serving scheduler (ks_sched_*): host logic, needs no GPU.  Marshalling only."""
+
+    def __init__(self, max_num_batched_tokens: int, max_num_seqs: int, block_size: int, num_blocks: int):
+        self._lib = load()
+        self._h = C.c_void_p()
+        cfg = ks_sched_config(int(max_num_batched_tokens), int(max_num_seqs), int(block_size), int(num_blocks))
+        _check(self._lib.ks_sched_create(C.byref(self._h), C.byref(cfg)), "ks_sched_create")
+        self.cap = int(max_num_seqs)
+        self.n_requests = 0
+        self._req = np.zeros(self.cap, np.int32)
+        self._new = np.zeros(self.cap, np.int32)
+        self._hist = np.zeros(self.cap, np.int32)
+
+    def add_requests(self, arrival, prompt_len, max_new) -> None:
+        a = np.ascontiguousarray(arrival, dtype=np.float64)
+        p = np.ascontiguousarray(prompt_len, dtype=np.int32)
+        o = np.ascontiguousarray(max_new, dtype=np.int32)
+        if not (a.shape == p.shape == o.shape and a.ndim == 1):
+            raise ValueError("arrival, prompt_len, max_new: 1-D arrays of one length")
+        ip = C.POINTER(C.c_int32)
+        _check(self._lib.ks_sched_add_requests(self._h, a.shape[0], a.ctypes.data_as(C.POINTER(C.c_double)),
+                                               p.ctypes.data_as(ip), o.ctypes.data_as(ip)), "ks_sched_add_requests")
+        self.n_requests += int(a.shape[0])
+
+    def step(self, now: float):
+        """-> (list of (request, n_new, hist), next_arrival)"""
+        n = C.c_int32()
+        nxt = C.c_double()
+        ip = C.POINTER(C.c_int32)
+        _check(self._lib.ks_sched_step(self._h, float(now), self.cap, C.byref(n), self._req.ctypes.data_as(ip),
+                                       self._new.ctypes.data_as(ip), self._hist.ctypes.data_as(ip), C.byref(nxt)),
+               "ks_sched_step")
+        k = n.value
+        return list(zip(self._req[:k].tolist(), self._new[:k].tolist(), self._hist[:k].tolist())), nxt.value
+
+    def commit(self, t_end: float) -> None:
+        _check(self._lib.ks_sched_commit(self._h, float(t_end)), "ks_sched_commit")
+
+    def results(self):
+        ft = np.zeros(self.n_requests, np.float64)
+        fin = np.zeros(self.n_requests, np.float64)
+        npre = np.zeros(self.n_requests, np.int32)
+        dp = C.POINTER(C.c_double)
+        _check(self._lib.ks_sched_results(self._h, ft.ctypes.data_as(dp), fin.ctypes.data_as(dp),
+                                          npre.ctypes.data_as(C.POINTER(C.c_int32))), "ks_sched_results")
+        return dict(first_token=ft, finish=fin, n_preempt=npre)
+
+    def stats(self) -> dict:
+        st = ks_sched_stats()
+        _check(self._lib.ks_sched_get_stats(self._h, C.byref(st)), "ks_sched_get_stats")
+        return {k: getattr(st, k) for k, _ in ks_sched_stats._fields_ if k != "pad"}
+
+    def close(self) -> None:
+        if self._h:
+            self._lib.ks_sched_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def make_model_desc(m) -> ks_model_desc:
+    """m: any object with n_layers, hidden, ffn, vocab, hq, hkv, head_dim, dtype_bytes, tp."""
+    return ks_model_desc(*[int(getattr(m, k)) for k, _ in ks_model_desc._fields_])
+
+
+def sim_run(ctx: "Context", scheds: Sequence[Scheduler], clock: np.ndarray, model, spec: dict, tier: int, params: dict,
+            max_iters: int = 0, log_cap: int = 0):
+    """ks_sim_run: clock is a float64 array [n_replicas], updated in place.  Returns (stats dict, step_replica, step_time)."""
+    n = len(scheds)
+    if not (isinstance(clock, np.ndarray) and clock.dtype == np.float64 and clock.shape == (n,) and clock.flags.c_contiguous):
+        raise ValueError("clock: contiguous float64 array [n_replicas]")
+    hs = (C.c_void_p * max(n, 1))(*[s._h.value for s in scheds])
+    md, sp, pp = make_model_desc(model), make_spec(spec), make_step_params(params)
+    rep = np.zeros(max(log_cap, 1), np.int32)
+    tim = np.zeros(max(log_cap, 1), np.float32)
+    nlog = C.c_int64()
+    st = ks_sim_stats()
+    _check(ctx._lib.ks_sim_run(ctx._h, hs, clock.ctypes.data_as(C.POINTER(C.c_double)), n, C.byref(md), C.byref(sp),
+                               int(tier), C.byref(pp), int(max_iters), rep.ctypes.data_as(C.POINTER(C.c_int32)),
+                               tim.ctypes.data_as(C.POINTER(C.c_float)), int(log_cap), C.byref(nlog), C.byref(st)),
+           "ks_sim_run")
+    k = nlog.value
+    return {f: getattr(st, f) for f, _ in ks_sim_stats._fields_}, rep[:k].copy(), tim[:k].copy()

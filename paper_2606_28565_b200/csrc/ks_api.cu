@@ -54,6 +54,9 @@ struct ks_ctx {
   cudaEvent_t ev_in[KS_MAX_BATCHES] = {}, ev_out[KS_MAX_BATCHES] = {}, ev_start = nullptr;
 };
 
+cudaStream_t ks_internal_stream(ks_ctx* c) { return c->stream; }
+cudaError_t ks_internal_set_device(ks_ctx* c) { return cudaSetDevice(c->device); }
+
 namespace {
 
 const int kFamCols[KS_FAM_COUNT] = {3, 10, 3, 2, 2};

@@ -64,4 +64,7 @@ struct KsComposeParams {
   float* step_lat;   // [n_specs][n_steps]
   float* cfg_lat;    // [n_specs][n_cfg]
 };
+// for ks_sched.cu (the simulation loop lives outside ks_api.cu): the context's stream and device
+cudaStream_t ks_internal_stream(ks_ctx* c);
+cudaError_t ks_internal_set_device(ks_ctx* c);
 cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_t st, int* launches);

@@ -1,0 +1,409 @@
+// ks_sched.cu — the serving scheduler (host logic) and the closed simulation loop over the GPU path.
+// SURVEY.md §8(f) NEXT-4; PAPER.md:241-249 (scheduler, mixed-step pricing), :231 (layer-homogeneous
+// step body), :159 (a step completes at now + t_step).  Rules: DESIGN.md Q18.
+//
+// The scheduler is plain C++ with no device code.  ks_sim_run drives many of them in lock step and
+// prices every iteration's batches with ONE pass of the library's own GPU path: rows are packed into
+// one pinned arena, moved with one H2D copy, run through ks_run_steps on device pointers, and the step
+// times come back with one D2H copy.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <deque>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "ks_internal.h"
+
+struct ks_sched {
+  ks_sched_config cfg{};
+  // per request, insertion order
+  std::vector<double> arrival, first_token, finish;
+  std::vector<int32_t> prompt, max_new, n_tok, computed, generated, blocks, n_preempt;
+  std::vector<int32_t> order;          // FCFS order: (arrival, insertion index)
+  size_t next_pos = 0;                 // first entry of `order` that has not arrived yet
+  bool started = false;
+  std::deque<int32_t> waiting;
+  std::vector<int32_t> running;
+  // the batch being executed
+  std::vector<int32_t> b_req, b_new, b_hist;
+  bool pending = false;
+  int32_t free_blocks = 0;
+  int64_t n_steps = 0, tokens = 0, preemptions = 0;
+  int32_t n_finished = 0;
+
+  int32_t blocks_for(int64_t tokens_) const { return (int32_t)((tokens_ + cfg.block_size - 1) / cfg.block_size); }
+};
+
+namespace {
+
+void sched_start(ks_sched* s) {
+  const int n = (int)s->arrival.size();
+  s->order.resize(n);
+  for (int i = 0; i < n; ++i) s->order[i] = i;
+  std::stable_sort(s->order.begin(), s->order.end(),
+                   [s](int32_t a, int32_t b) { return s->arrival[a] < s->arrival[b]; });
+  s->started = true;
+}
+
+// The token-budget loop.  Fills s->b_* with the batch of the step that starts at `now`.
+void sched_form_batch(ks_sched* s, double now) {
+  if (!s->started) sched_start(s);
+  while (s->next_pos < s->order.size() && s->arrival[s->order[s->next_pos]] <= now) s->waiting.push_back(s->order[s->next_pos++]);
+  s->b_req.clear(); s->b_new.clear(); s->b_hist.clear();
+  int32_t budget = s->cfg.max_num_batched_tokens;
+  bool preempted = false;
+  auto take = [s, &budget](int32_t r, int32_t n_new, int32_t need) {
+    s->free_blocks -= need;
+    s->blocks[r] += need;
+    s->b_req.push_back(r); s->b_new.push_back(n_new); s->b_hist.push_back(s->computed[r]);
+    budget -= n_new;
+  };
+  // running requests first, in queue order
+  for (size_t i = 0; i < s->running.size() && budget > 0;) {
+    const int32_t r = s->running[i];
+    const int32_t n_new = std::min(s->n_tok[r] - s->computed[r], budget);
+    const int32_t need = s->blocks_for((int64_t)s->computed[r] + n_new) - s->blocks[r];
+    bool self = false;
+    while (need > s->free_blocks) {        // KV pressure: the back of the running queue is recomputed later
+      const int32_t v = s->running.back();
+      s->running.pop_back();
+      s->free_blocks += s->blocks[v];
+      s->blocks[v] = 0;
+      s->computed[v] = 0;
+      ++s->n_preempt[v];
+      ++s->preemptions;
+      s->waiting.push_front(v);
+      preempted = true;
+      if (v == r) { self = true; break; }
+    }
+    if (self) break;
+    take(r, n_new, need);
+    ++i;
+  }
+  // FCFS admission (a partial chunk of a prompt is admitted with the budget that is left)
+  if (!preempted) {
+    while (!s->waiting.empty() && budget > 0 && (int32_t)s->running.size() < s->cfg.max_num_seqs) {
+      const int32_t r = s->waiting.front();
+      const int32_t n_new = std::min(s->n_tok[r] - s->computed[r], budget);
+      const int32_t need = s->blocks_for((int64_t)s->computed[r] + n_new) - s->blocks[r];
+      if (need > s->free_blocks) break;
+      s->waiting.pop_front();
+      s->running.push_back(r);
+      take(r, n_new, need);
+    }
+  }
+  s->pending = !s->b_req.empty();
+}
+
+double sched_next_arrival(const ks_sched* s) {
+  return s->next_pos < s->order.size() ? s->arrival[s->order[s->next_pos]] : std::numeric_limits<double>::infinity();
+}
+
+void sched_commit(ks_sched* s, double t_end) {
+  for (size_t k = 0; k < s->b_req.size(); ++k) {
+    const int32_t r = s->b_req[k];
+    s->computed[r] += s->b_new[k];
+    s->tokens += s->b_new[k];
+    if (s->computed[r] != s->n_tok[r]) continue;
+    if (++s->generated[r] == 1) s->first_token[r] = t_end;
+    if (s->generated[r] == s->max_new[r]) {
+      s->finish[r] = t_end;
+      s->free_blocks += s->blocks[r];
+      s->blocks[r] = 0;
+      s->running.erase(std::find(s->running.begin(), s->running.end(), r));
+      ++s->n_finished;
+    } else {
+      ++s->n_tok[r];
+    }
+  }
+  if (!s->b_req.empty()) ++s->n_steps;
+  s->b_req.clear(); s->b_new.clear(); s->b_hist.clear();
+  s->pending = false;
+}
+
+bool sched_done(const ks_sched* s) { return s->n_finished == (int32_t)s->arrival.size(); }
+
+}  // namespace
+
+extern "C" {
+
+ks_status ks_sched_create(ks_sched** out, const ks_sched_config* cfg) {
+  if (!out) return KS_EINVAL;
+  *out = nullptr;
+  if (!cfg || cfg->max_num_batched_tokens < 1 || cfg->max_num_seqs < 1 || cfg->block_size < 1 || cfg->num_blocks < 1)
+    return KS_EINVAL;
+  ks_sched* s = new (std::nothrow) ks_sched();
+  if (!s) return KS_ENOMEM;
+  s->cfg = *cfg;
+  s->free_blocks = cfg->num_blocks;
+  *out = s;
+  return KS_OK;
+}
+
+ks_status ks_sched_add_requests(ks_sched* s, int n, const double* arrival, const int32_t* prompt_len, const int32_t* max_new) {
+  if (!s || n < 0 || (n > 0 && (!arrival || !prompt_len || !max_new))) return KS_EINVAL;
+  if (s->started) return KS_ESTATE;
+  for (int i = 0; i < n; ++i) {
+    if (!std::isfinite(arrival[i]) || prompt_len[i] < 1 || max_new[i] < 1) return KS_EINVAL;
+    if (s->blocks_for((int64_t)prompt_len[i] + max_new[i]) > s->cfg.num_blocks) return KS_EINVAL;
+  }
+  if ((int64_t)s->arrival.size() + n > (int64_t)std::numeric_limits<int32_t>::max()) return KS_EINVAL;
+  try {
+    for (int i = 0; i < n; ++i) {
+      s->arrival.push_back(arrival[i]);
+      s->prompt.push_back(prompt_len[i]);
+      s->max_new.push_back(max_new[i]);
+      s->n_tok.push_back(prompt_len[i]);
+      s->computed.push_back(0);
+      s->generated.push_back(0);
+      s->blocks.push_back(0);
+      s->n_preempt.push_back(0);
+      s->first_token.push_back(std::numeric_limits<double>::quiet_NaN());
+      s->finish.push_back(std::numeric_limits<double>::quiet_NaN());
+    }
+  } catch (const std::bad_alloc&) {
+    return KS_ENOMEM;
+  }
+  return KS_OK;
+}
+
+ks_status ks_sched_step(ks_sched* s, double now, int32_t cap, int32_t* n_sched, int32_t* req, int32_t* n_new,
+                        int32_t* hist, double* next_arrival) {
+  if (!s || !n_sched || cap < 0 || std::isnan(now)) return KS_EINVAL;
+  if (s->pending) return KS_ESTATE;
+  if ((int64_t)cap < std::min<int64_t>(s->cfg.max_num_seqs, (int64_t)s->arrival.size()))
+    return KS_EINVAL;                  // the caller's arrays might not hold the batch
+  sched_form_batch(s, now);
+  const int32_t n = (int32_t)s->b_req.size();
+  *n_sched = n;
+  for (int32_t k = 0; k < n; ++k) {
+    if (req) req[k] = s->b_req[k];
+    if (n_new) n_new[k] = s->b_new[k];
+    if (hist) hist[k] = s->b_hist[k];
+  }
+  if (next_arrival) *next_arrival = sched_next_arrival(s);
+  return KS_OK;
+}
+
+ks_status ks_sched_commit(ks_sched* s, double t_end) {
+  if (!s || std::isnan(t_end)) return KS_EINVAL;
+  if (!s->pending) return KS_ESTATE;
+  sched_commit(s, t_end);
+  return KS_OK;
+}
+
+ks_status ks_sched_results(ks_sched* s, double* first_token, double* finish, int32_t* n_preempt) {
+  if (!s) return KS_EINVAL;
+  const size_t n = s->arrival.size();
+  if (first_token && n) memcpy(first_token, s->first_token.data(), n * sizeof(double));
+  if (finish && n) memcpy(finish, s->finish.data(), n * sizeof(double));
+  if (n_preempt && n) memcpy(n_preempt, s->n_preempt.data(), n * sizeof(int32_t));
+  return KS_OK;
+}
+
+ks_status ks_sched_get_stats(ks_sched* s, ks_sched_stats* out) {
+  if (!s || !out) return KS_EINVAL;
+  memset(out, 0, sizeof(*out));
+  out->n_steps = s->n_steps;
+  out->tokens_scheduled = s->tokens;
+  out->n_preemptions = s->preemptions;
+  out->n_requests = (int32_t)s->arrival.size();
+  out->n_finished = s->n_finished;
+  out->n_running = (int32_t)s->running.size();
+  out->n_waiting = (int32_t)s->waiting.size();
+  out->free_blocks = s->free_blocks;
+  return KS_OK;
+}
+
+ks_status ks_sched_destroy(ks_sched* s) {
+  delete s;
+  return KS_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// The closed loop.
+namespace {
+
+// One iteration's rows, packed for a single H2D copy.  Every array starts on a 16-byte boundary (the
+// alignment KS_MEM_DEVICE asks for).  Families in bucket order: GEMM, attention, elementwise[, all-reduce].
+struct Arena {
+  char* host = nullptr;
+  char* dev = nullptr;
+  size_t bytes = 0;
+  // offsets into the arena
+  size_t col[4][3] = {}, mult[4] = {}, off[4] = {}, out = 0;
+  int cap_rows[4] = {};
+  int n_fam = 3;
+};
+
+size_t a16(size_t x) { return (x + 15) & ~(size_t)15; }
+
+}  // namespace
+
+extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* clock, int n_replicas,
+                                const ks_model_desc* model, const ks_hw_spec* spec, ks_tier tier,
+                                const ks_step_params* params, int64_t max_iters, int32_t* step_replica,
+                                float* step_time, int64_t log_cap, int64_t* n_logged, ks_sim_stats* stats) {
+  if (n_logged) *n_logged = 0;
+  if (stats) memset(stats, 0, sizeof(*stats));
+  if (!ctx || !scheds || !clock || n_replicas < 0 || !model || !spec || !params || log_cap < 0) return KS_EINVAL;
+  if (log_cap > 0 && (!step_replica || !step_time)) return KS_EINVAL;
+  const ks_model_desc& m = *model;
+  if (m.n_layers < 1 || m.hidden < 1 || m.ffn < 1 || m.vocab < 1 || m.hq < 1 || m.hkv < 1 || m.head_dim < 1 || m.tp < 1 ||
+      (m.dtype_bytes != 1 && m.dtype_bytes != 2 && m.dtype_bytes != 4))
+    return KS_EINVAL;
+  for (int r = 0; r < n_replicas; ++r) {
+    if (!scheds[r] || std::isnan(clock[r])) return KS_EINVAL;
+    if (scheds[r]->pending) return KS_ESTATE;
+    // int32 row columns: the largest value is tokens x max(2 ffn, hidden x dtype_bytes, ...)
+    const int64_t T = scheds[r]->cfg.max_num_batched_tokens;
+    const int64_t widest = std::max<int64_t>({(int64_t)m.ffn, (int64_t)m.hidden * m.dtype_bytes,
+                                              (int64_t)(m.hq + m.hkv) * m.head_dim, (int64_t)2 * m.hkv * m.head_dim});
+    if (T * widest > (int64_t)std::numeric_limits<int32_t>::max()) return KS_EUNSUPPORTED;
+  }
+  if (n_replicas == 0) return KS_OK;
+
+  Arena A;
+  A.n_fam = m.tp > 1 ? 4 : 3;
+  const int n_cols[4] = {3, 3, 2, 2};
+  const int fam_id[4] = {KS_FAM_GEMM, KS_FAM_ATTN, KS_FAM_ELEMWISE, KS_FAM_ALLREDUCE};
+  int64_t attn_rows = 0;
+  for (int r = 0; r < n_replicas; ++r) attn_rows += scheds[r]->cfg.max_num_seqs;
+  A.cap_rows[0] = 5 * n_replicas;
+  A.cap_rows[1] = (int)std::min<int64_t>(attn_rows, std::numeric_limits<int32_t>::max() / 8);
+  A.cap_rows[2] = 6 * n_replicas;
+  A.cap_rows[3] = n_replicas;
+  if (attn_rows > A.cap_rows[1]) return KS_EUNSUPPORTED;
+  size_t at = 0;
+  for (int f = 0; f < A.n_fam; ++f) {
+    for (int c = 0; c < n_cols[f]; ++c) { A.col[f][c] = at; at = a16(at + (size_t)A.cap_rows[f] * 4); }
+    A.mult[f] = at; at = a16(at + (size_t)A.cap_rows[f] * 4);
+    A.off[f] = at; at = a16(at + (size_t)(n_replicas + 1) * 4);
+  }
+  const size_t in_bytes = at;
+  A.out = at; at = a16(at + (size_t)n_replicas * 4);
+  A.bytes = at;
+
+  cudaStream_t st = ks_internal_stream(ctx);
+  if (ks_internal_set_device(ctx) != cudaSuccess) return KS_ECUDA;
+  if (cudaMallocHost((void**)&A.host, A.bytes) != cudaSuccess) { cudaGetLastError(); return KS_ENOMEM; }
+  if (cudaMalloc((void**)&A.dev, A.bytes) != cudaSuccess) { cudaGetLastError(); cudaFreeHost(A.host); return KS_ENOMEM; }
+  memset(A.host, 0, A.bytes);
+
+  std::vector<int> active;
+  active.reserve(n_replicas);
+  ks_status rc = KS_OK;
+  int64_t iters = 0, logged = 0, steps = 0, rows_total = 0, inst_total = 0;
+  const int L = m.n_layers;
+  const int32_t qkv_n = (m.hq + 2 * m.hkv) * m.head_dim;
+  auto I = [&A](size_t off) { return reinterpret_cast<int32_t*>(A.host + off); };
+
+  while (max_iters <= 0 || iters < max_iters) {
+    active.clear();
+    int n_rows[4] = {0, 0, 0, 0};
+    for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[0] = 0;
+    for (int r = 0; r < n_replicas; ++r) {
+      ks_sched* s = scheds[r];
+      if (sched_done(s)) continue;
+      sched_form_batch(s, clock[r]);
+      while (s->b_req.empty()) {                    // idle: the clock jumps to the next arrival
+        const double nxt = sched_next_arrival(s);
+        if (!std::isfinite(nxt)) break;
+        clock[r] = std::max(clock[r], nxt);
+        sched_form_batch(s, clock[r]);
+      }
+      if (s->b_req.empty()) continue;
+      // rows of this step: dense kernels at the total token count, attention per request
+      int32_t T = 0;
+      for (int32_t v : s->b_new) T += v;
+      const int32_t n_seq = (int32_t)s->b_req.size();
+      {
+        int k = n_rows[0];
+        const int32_t gM[5] = {T, T, T, T, n_seq};
+        const int32_t gN[5] = {qkv_n, m.hidden, 2 * m.ffn, m.hidden, m.vocab};
+        const int32_t gK[5] = {m.hidden, m.hidden, m.hidden, m.ffn, m.hidden};
+        for (int j = 0; j < 5; ++j, ++k) {
+          I(A.col[0][0])[k] = gM[j]; I(A.col[0][1])[k] = gN[j]; I(A.col[0][2])[k] = gK[j];
+          I(A.mult[0])[k] = j < 4 ? L : 1;
+        }
+        n_rows[0] = k;
+      }
+      {
+        int k = n_rows[1];
+        for (int32_t j = 0; j < n_seq; ++j, ++k) {
+          I(A.col[1][0])[k] = 1; I(A.col[1][1])[k] = s->b_new[j]; I(A.col[1][2])[k] = s->b_hist[j] + s->b_new[j];
+          I(A.mult[1])[k] = L;
+        }
+        n_rows[1] = k;
+      }
+      {
+        int k = n_rows[2];
+        const int32_t width[6] = {m.hidden, m.hidden, (m.hq + m.hkv) * m.head_dim, 2 * m.hkv * m.head_dim, m.ffn, m.hidden};
+        const int32_t sub[6] = {4, 0, 2, 3, 1, 0};   // embedding, RMSNorm, RoPE, KV write, SiLU*Mul, final RMSNorm
+        const int32_t mu[6] = {1, L, L, L, L, 1};
+        for (int j = 0; j < 6; ++j, ++k) {
+          I(A.col[2][0])[k] = T * width[j]; I(A.col[2][1])[k] = sub[j]; I(A.mult[2])[k] = mu[j];
+        }
+        n_rows[2] = k;
+      }
+      if (A.n_fam == 4) {
+        const int k = n_rows[3]++;
+        I(A.col[3][0])[k] = T * m.hidden * m.dtype_bytes; I(A.col[3][1])[k] = m.tp; I(A.mult[3])[k] = 2 * L;
+      }
+      active.push_back(r);
+      const int a = (int)active.size();
+      for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[a] = n_rows[f];
+      inst_total += (int64_t)L * (4 + n_seq + 4 + (A.n_fam == 4 ? 2 : 0)) + 3;
+    }
+    const int n_act = (int)active.size();
+    if (n_act == 0) break;
+
+    // one copy in, one pass of the hot path on device pointers, one copy out
+    if (cudaMemcpyAsync(A.dev, A.host, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = KS_ECUDA; break; }
+    ks_desc_batch b[4];
+    const int32_t* offs[4];
+    memset(b, 0, sizeof(b));
+    for (int f = 0; f < A.n_fam; ++f) {
+      b[f].family = fam_id[f];
+      b[f].n = n_rows[f];
+      b[f].col_dtype = KS_COL_I32;
+      b[f].dtype_bytes = m.dtype_bytes;
+      b[f].n_cols = n_cols[f];
+      if (fam_id[f] == KS_FAM_ATTN) { b[f].attn_hq = m.hq; b[f].attn_hkv = m.hkv; b[f].attn_head_dim = m.head_dim; }
+      for (int c = 0; c < n_cols[f]; ++c) b[f].cols[c] = A.dev + A.col[f][c];
+      b[f].mult = reinterpret_cast<const int32_t*>(A.dev + A.mult[f]);
+      offs[f] = reinterpret_cast<const int32_t*>(A.dev + A.off[f]);
+      rows_total += n_rows[f];
+    }
+    rc = ks_run_steps(ctx, b, offs, A.n_fam, spec, 1, tier, n_act, params, nullptr, 0, KS_MEM_DEVICE, nullptr,
+                      reinterpret_cast<float*>(A.dev + A.out), nullptr);
+    if (rc != KS_OK) break;
+    if (cudaMemcpyAsync(A.host + A.out, A.dev + A.out, (size_t)n_act * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) { rc = KS_ECUDA; break; }
+
+    const float* t_step = reinterpret_cast<const float*>(A.host + A.out);
+    for (int a = 0; a < n_act; ++a) {
+      const int r = active[a];
+      clock[r] += (double)t_step[a];                 // completion at now + t_step
+      sched_commit(scheds[r], clock[r]);
+      if (logged < log_cap) { step_replica[logged] = r; step_time[logged] = t_step[a]; ++logged; }
+    }
+    steps += n_act;
+    ++iters;
+  }
+  if (rc != KS_OK) {
+    cudaStreamSynchronize(st);
+    cudaGetLastError();
+  }
+  cudaFree(A.dev);
+  cudaFreeHost(A.host);
+  if (n_logged) *n_logged = logged;
+  if (stats) { stats->iterations = iters; stats->steps = steps; stats->rows = rows_total; stats->kernel_instances = inst_total; }
+  return rc;
+}

@@ -490,3 +490,56 @@ def config5(n_rows: int = 2 ** 22, n_specs: int = 64, seed: int = 4, n_in: int =
 
 
 CONFIGS = {"cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5}
+
+
+# ----------------------------------------------------------------------------- serving traces (NEXT-4)
+@dataclass
+class ServingModel:
+    """Dense decoder the simulated steps are priced for (defaults: config 4's model)."""
+    n_layers: int = N_LAYERS
+    hidden: int = HIDDEN
+    ffn: int = FFN
+    vocab: int = VOCAB
+    hq: int = HQ
+    hkv: int = HKV
+    head_dim: int = HEAD_DIM
+    dtype_bytes: int = 2
+    tp: int = 1
+
+
+@dataclass
+class Replica:
+    """One simulated serving replica: scheduler limits + its request trace."""
+    max_num_batched_tokens: int
+    max_num_seqs: int
+    block_size: int
+    num_blocks: int
+    arrival: np.ndarray      # float64 [n] seconds
+    prompt_len: np.ndarray   # int32 [n]
+    max_new: np.ndarray      # int32 [n]
+
+
+def serving_trace(rng, n: int, rate: float, prompt_mean: float = 512.0, out_mean: float = 128.0):
+    """Poisson arrivals at `rate` requests/s; log-normal prompt and output lengths (sigma 1.0 / 0.8)
+    clipped to [8, 8192] / [1, 1024] — the shape of chat-style serving traces (synthetic stand-in for the
+    paper's request traces)."""
+    arrival = np.cumsum(rng.exponential(1.0 / rate, size=n))
+    p = np.clip(np.round(rng.lognormal(np.log(prompt_mean) - 0.5, 1.0, size=n)), 8, 8192).astype(np.int32)
+    o = np.clip(np.round(rng.lognormal(np.log(out_mean) - 0.32, 0.8, size=n)), 1, 1024).astype(np.int32)
+    return arrival.astype(np.float64), p, o
+
+
+def sim_replicas(n_replicas: int = 64, n_requests: int = 200, seed: int = 6, pressure: bool = False) -> List[Replica]:
+    """A what-if sweep over scheduler limits and load: token budget in {1024, 2048, 4096, 8192}, max_num_seqs in
+    {32, 64, 128, 256}, arrival rate log-uniform in [4, 64] requests/s.  pressure=True shrinks the KV cache so
+    that preemption/recompute happens."""
+    rng = _rng(seed)
+    out = []
+    for _ in range(n_replicas):
+        T = int(rng.choice([1024, 2048, 4096, 8192]))
+        S = int(rng.choice([32, 64, 128, 256]))
+        rate = float(np.exp(rng.uniform(np.log(4.0), np.log(64.0))))
+        a, p, o = serving_trace(rng, n_requests, rate)
+        nb = 1024 if pressure else 65536      # blocks of 16 tokens: 16k tokens (tight) or 1M tokens (ample)
+        out.append(Replica(T, S, 16, nb, a, p, o))
+    return out
