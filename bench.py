@@ -403,7 +403,62 @@ def run_extras(h: Harness, peaks):
                              tflops=float(tf), frac_tensor_sustained=float(tf / peaks["bf16_sustained"]))
     del st
     torch.cuda.empty_cache()
+    ex["sim_closed_loop"] = sim_extras(h)
     return ex
+
+
+def sim_extras(h):
+    """NEXT-4: the closed simulation loop (host schedulers + one pass of the GPU path per iteration):
+    256 what-if replicas x 200 requests each; wall-clock throughput of ks_sim_run (latency-bound: every
+    iteration waits for its step times before the next batches can be formed)."""
+    import time
+    B = h.B
+    out = {}
+    n_rep, n_req = (256, 200) if not PROFILE else (8, 10)
+    reps = W.sim_replicas(n_replicas=n_rep, n_requests=n_req, seed=6)
+    model, spec = W.ServingModel(), W.spec_gb200()
+    for name, tier in (("tierNONE", W.TIER_NONE), ("tierA", W.TIER_A)):
+        if tier == W.TIER_A:
+            rng = np.random.Generator(np.random.PCG64(1))
+            for f in (W.FAM_GEMM, W.FAM_ATTN, W.FAM_ELEMWISE):
+                h.ctx.load_heads(f, W.make_head(rng, 12, 128))
+        best = None
+        for _ in range(1 if PROFILE else 3):
+            scheds = []
+            for r in reps:
+                s = B.Scheduler(r.max_num_batched_tokens, r.max_num_seqs, r.block_size, r.num_blocks)
+                s.add_requests(r.arrival, r.prompt_len, r.max_new)
+                scheds.append(s)
+            clock = np.zeros(n_rep, np.float64)
+            t0 = time.perf_counter()
+            st, _, _ = B.sim_run(h.ctx, scheds, clock, model, spec, tier, W.STEP_PARAMS_CFG4)
+            dt = time.perf_counter() - t0
+            for s in scheds:
+                s.close()
+            if best is None or dt < best[0]:
+                best = (dt, st, float(clock.max()))
+        dt, st, sim_end = best
+        it = max(st["iterations"], 1)
+        out[name] = dict(replicas=n_rep, requests_per_replica=n_req, iterations=st["iterations"], steps=st["steps"],
+                         rows=st["rows"], kernel_instances=st["kernel_instances"], wall_s=dt,
+                         steps_per_s=st["steps"] / dt, kernel_instances_per_s=st["kernel_instances"] / dt,
+                         us_per_iteration=dt / it * 1e6, simulated_s=sim_end,
+                         us_per_iteration_by_phase=dict(schedule_and_pack=st["schedule_s"] / it * 1e6,
+                                                        enqueue=st["enqueue_s"] / it * 1e6, wait_gpu=st["wait_s"] / it * 1e6,
+                                                        commit=st["commit_s"] / it * 1e6))
+    # the oracle's closed loop (Python scheduler + C predictor), one replica, bounded: 30 requests
+    from oracle import sched as OS
+    r = reps[0]
+    o = OS.Scheduler(OS.SchedConfig(r.max_num_batched_tokens, r.max_num_seqs, r.block_size, r.num_blocks),
+                     r.arrival[:30], r.prompt_len[:30], r.max_new[:30])
+    om = OS.Model(**vars(model))
+    t0 = time.perf_counter()
+    _, priced, _ = OS.simulate(o, lambda b: float(OS.price_steps([b], om, spec, W.TIER_NONE, W.STEP_PARAMS_CFG4)[0]),
+                               max_steps=None if not PROFILE else 20)
+    dt = time.perf_counter() - t0
+    out["oracle_tierNONE"] = dict(kind="oracle", sample="1 replica x 30 requests", steps=len(priced), wall_s=dt,
+                                  steps_per_s=len(priced) / dt)
+    return out
 
 
 def run_ours(args):

@@ -253,6 +253,8 @@ typedef struct {
   int64_t steps;                   /* serving steps priced, all replicas */
   int64_t rows;                    /* kernel rows priced */
   int64_t kernel_instances;        /* sum of multiplicities = kernel launches those steps stand for */
+  double schedule_s, enqueue_s, wait_s, commit_s;  /* host wall time spent forming + packing batches, enqueueing
+                                      the GPU pass, waiting for it, and committing the steps */
 } ks_sim_stats;
 
 /* Run n_replicas schedulers in lock step until all have finished or max_iters iterations have run

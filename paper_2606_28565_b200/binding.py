@@ -69,7 +69,8 @@ class ks_sched_stats(C.Structure):
 
 
 class ks_sim_stats(C.Structure):
-    _fields_ = [("iterations", C.c_int64), ("steps", C.c_int64), ("rows", C.c_int64), ("kernel_instances", C.c_int64)]
+    _fields_ = [("iterations", C.c_int64), ("steps", C.c_int64), ("rows", C.c_int64), ("kernel_instances", C.c_int64),
+                ("schedule_s", C.c_double), ("enqueue_s", C.c_double), ("wait_s", C.c_double), ("commit_s", C.c_double)]
 
 
 _lib = None
