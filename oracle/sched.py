@@ -22,7 +22,7 @@ caching, the second half of NEXT-4, is not modelled).  Plain Python loops, one r
 from __future__ import annotations
 
 import math
-from collections import deque
+from collections import OrderedDict, deque
 from dataclasses import dataclass
 from typing import Callable, List, Optional, Sequence, Tuple
 
@@ -35,13 +35,16 @@ class SchedConfig:
     max_num_seqs: int             # S: most requests running at once
     block_size: int               # tokens per KV-cache block
     num_blocks: int               # KV-cache blocks on the GPU
+    enable_prefix_cache: bool = False   # content-hashed prefix cache, GPU tier (Q19)
+    disk_blocks: int = 0          # capacity of the persistent disk tier in blocks (0 = no disk tier)
 
 
 class Scheduler:
     """One replica's scheduler.  step(now) forms the batch of the step that starts at `now`;
     commit(t_end) applies it at the step's completion time."""
 
-    def __init__(self, cfg: SchedConfig, arrival: Sequence[float], prompt_len: Sequence[int], max_new: Sequence[int]):
+    def __init__(self, cfg: SchedConfig, arrival: Sequence[float], prompt_len: Sequence[int], max_new: Sequence[int],
+                 prefix_id: Optional[Sequence[int]] = None, prefix_len: Optional[Sequence[int]] = None):
         self.cfg = cfg
         n = len(arrival)
         self.arrival = [float(a) for a in arrival]
@@ -69,9 +72,84 @@ class Scheduler:
         self.n_finished = 0
         self.n_steps = 0
         self.tokens_scheduled = 0
+        # prefix cache.  The first prefix_len[i] prompt tokens of request i are the content
+        # named prefix_id[i]; full block j of that content has the hash key (prefix_id, j).
+        self.pid = [-1] * n if prefix_id is None else [int(v) for v in prefix_id]
+        self.plen = [0] * n if prefix_len is None else [int(v) for v in prefix_len]
+        for i in range(n):
+            if self.pid[i] < 0:
+                self.plen[i] = 0
+            if not 0 <= self.plen[i] <= self.P[i]:
+                raise ValueError("0 <= prefix_len <= prompt_len")
+        self.held: List[List[Tuple[int, int]]] = [[] for _ in range(n)]   # cache keys a request holds a reference on
+        self.registered = [0] * n          # prefix blocks of the request already looked up / offered to the cache
+        self.gpu_ref: dict = {}            # key -> reference count (GPU tier)
+        self.lru: OrderedDict = OrderedDict()     # keys with reference count 0, least recently released first
+        self.disk: OrderedDict = OrderedDict()    # disk tier, least recently used first
+        self.cached_tokens = [0] * n       # prompt tokens served from the cache over all (re)admissions
+        self.gpu_hit_blocks = 0
+        self.disk_hit_blocks = 0
+        self.evictions = 0
 
     def _blocks_for(self, tokens: int) -> int:
         return -(-tokens // self.cfg.block_size)
+
+    def avail(self) -> int:
+        """Blocks an allocation may use: free ones plus cached ones nobody references (evicted on demand)."""
+        return self.free_blocks + len(self.lru)
+
+    def _alloc(self, k: int) -> None:
+        """Take k blocks: free ones first, then evict unreferenced cached blocks, least recently released first
+        (a block evicted from the GPU tier stays in the disk tier if it is there)."""
+        assert k <= self.avail()
+        while k > 0:
+            if self.free_blocks > 0:
+                self.free_blocks -= 1
+            else:
+                key, _ = self.lru.popitem(last=False)
+                del self.gpu_ref[key]
+                self.evictions += 1
+            k -= 1
+
+    def _release(self, r: int) -> None:
+        """Request r gives up its blocks: private ones become free, shared ones lose a reference."""
+        self.free_blocks += self.blocks[r] - len(self.held[r])
+        for key in self.held[r]:
+            self.gpu_ref[key] -= 1
+            if self.gpu_ref[key] == 0:
+                self.lru[key] = True
+        self.held[r] = []
+        self.blocks[r] = 0
+        self.registered[r] = 0
+
+    def _disk_put(self, key) -> None:
+        if self.cfg.disk_blocks <= 0:
+            return
+        if key in self.disk:
+            self.disk.move_to_end(key)
+            return
+        self.disk[key] = True
+        if len(self.disk) > self.cfg.disk_blocks:
+            self.disk.popitem(last=False)
+
+    def _lookup(self, r: int):
+        """Longest leading run of request r's prefix blocks present in the GPU tier or, failing that, the disk
+        tier; at least one token of the request is always left to compute.  -> (keys, where) lists."""
+        if not self.cfg.enable_prefix_cache or self.pid[r] < 0:
+            return [], []
+        bs = self.cfg.block_size
+        limit = min(self.plen[r] // bs, (self.n_tok[r] - 1) // bs)
+        keys, where = [], []
+        for j in range(limit):
+            key = (self.pid[r], j)
+            if key in self.gpu_ref:
+                where.append("gpu")
+            elif key in self.disk:
+                where.append("disk")
+            else:
+                break
+            keys.append(key)
+        return keys, where
 
     def done(self) -> bool:
         return self.n_finished == len(self.P)
@@ -98,11 +176,10 @@ class Scheduler:
             n_new = min(self.n_tok[r] - self.c[r], budget)
             need = self._blocks_for(self.c[r] + n_new) - self.blocks[r]
             alive = True
-            while need > self.free_blocks:
+            while need > self.avail():
                 # KV pressure: preempt the request at the back of the running queue; it will be recomputed
                 v = self.running.pop()
-                self.free_blocks += self.blocks[v]
-                self.blocks[v] = 0
+                self._release(v)
                 self.c[v] = 0
                 self.n_preempt[v] += 1
                 self.waiting.appendleft(v)
@@ -112,7 +189,7 @@ class Scheduler:
                     break
             if not alive:
                 break
-            self.free_blocks -= need
+            self._alloc(need)
             self.blocks[r] += need
             batch.append((r, n_new, self.c[r]))
             budget -= n_new
@@ -121,12 +198,34 @@ class Scheduler:
         if not preempted:
             while self.waiting and budget > 0 and len(self.running) < cfg.max_num_seqs:
                 r = self.waiting[0]
-                n_new = min(self.n_tok[r] - self.c[r], budget)
-                need = self._blocks_for(self.c[r] + n_new) - self.blocks[r]
-                if need > self.free_blocks:
+                # prefix-cache-aware admission: cached leading blocks are not recomputed
+                keys, where = self._lookup(r) if self.c[r] == 0 else ([], [])
+                hit = len(keys) * cfg.block_size
+                n_new = min(self.n_tok[r] - (self.c[r] + hit), budget)
+                need = self._blocks_for(self.c[r] + hit + n_new) - self.blocks[r] - len(keys)
+                # blocks leaving the allocatable pool: unreferenced GPU hits, one new block per disk hit, the rest
+                taken = sum(1 for k, w in zip(keys, where) if w == "gpu" and self.gpu_ref[k] == 0)
+                taken += sum(1 for w in where if w == "disk") + need
+                if taken > self.avail():
                     break
-                self.free_blocks -= need
-                self.blocks[r] += need
+                for k, w in zip(keys, where):          # reference the GPU hits first so they cannot be evicted
+                    if w == "gpu":
+                        if self.gpu_ref[k] == 0:
+                            del self.lru[k]
+                        self.gpu_ref[k] += 1
+                        self.gpu_hit_blocks += 1
+                for k, w in zip(keys, where):          # disk hits are loaded into newly allocated GPU blocks
+                    if w == "disk":
+                        self._alloc(1)
+                        self.gpu_ref[k] = 1
+                        self._disk_put(k)
+                        self.disk_hit_blocks += 1
+                self._alloc(need)
+                self.held[r] = list(keys)
+                self.registered[r] = len(keys)
+                self.blocks[r] += need + len(keys)
+                self.c[r] += hit
+                self.cached_tokens[r] += hit
                 self.waiting.popleft()
                 self.running.append(r)
                 batch.append((r, n_new, self.c[r]))
@@ -140,14 +239,24 @@ class Scheduler:
         for r, n_new, _ in self.batch:
             self.c[r] += n_new
             self.tokens_scheduled += n_new
+            if self.cfg.enable_prefix_cache and self.pid[r] >= 0:
+                # full prefix blocks whose KV now exists are offered to the cache (and written through to disk);
+                # if the key is already there (another request got there first) the block stays private
+                full = min(self.c[r], self.plen[r]) // self.cfg.block_size
+                for j in range(self.registered[r], full):
+                    key = (self.pid[r], j)
+                    if key not in self.gpu_ref:
+                        self.gpu_ref[key] = 1
+                        self.held[r].append(key)
+                    self._disk_put(key)
+                self.registered[r] = max(self.registered[r], full)
             if self.c[r] == self.n_tok[r]:
                 self.g[r] += 1
                 if self.g[r] == 1:
                     self.first_token[r] = t_end
                 if self.g[r] == self.O[r]:
                     self.finish[r] = t_end
-                    self.free_blocks += self.blocks[r]
-                    self.blocks[r] = 0
+                    self._release(r)
                     self.running.remove(r)
                     self.n_finished += 1
                 else:

@@ -174,3 +174,129 @@ def test_price_steps_equals_hand_composition():
     body = 32 * layer + one(0, [3, 131072, 4096]) + one(3, [T * 4096, 4]) + one(3, [T * 4096, 0])
     n = 32 * (4 + 3 + 4) + 3
     assert abs(t - (body + n * 4e-6)) < 1e-12
+
+
+# ------------------------------------------------------------------ prefix cache (Q19)
+def pc_cfg(T=4096, S=16, bs=16, nb=4096, disk=0):
+    return S_cfg(T, S, bs, nb, True, disk)
+
+
+def S_cfg(T, S_, bs, nb, on, disk):
+    return S.SchedConfig(T, S_, bs, nb, enable_prefix_cache=on, disk_blocks=disk)
+
+
+def drive(s, dt=1.0, until=None):
+    now, log = 0.0, []
+    while not s.done():
+        b = s.step(now)
+        if not b:
+            now = max(now, s.next_arrival())
+            continue
+        log.append(b)
+        now += dt
+        s.commit(now)
+        held = sum(1 for k, v in s.gpu_ref.items() if v > 0)
+        assert s.free_blocks + len(s.lru) + sum(s.blocks[r] - len(s.held[r]) for r in range(len(s.P))) + held == s.cfg.num_blocks
+        assert s.free_blocks >= 0 and set(s.lru) == {k for k, v in s.gpu_ref.items() if v == 0}
+    return log
+
+
+def test_prefix_hit_recomputes_only_the_uncached_suffix():
+    # "A prefix hit reuses cached blocks so only the uncached suffix is recomputed"
+    s = S.Scheduler(pc_cfg(), [0.0, 1.5], [100, 100], [2, 2], prefix_id=[7, 7], prefix_len=[64, 64])
+    log = drive(s)
+    assert log[0] == [(0, 100, 0)]
+    assert log[2] == [(1, 36, 64)]                      # 4 cached blocks of 16 tokens: history 64, 36 new tokens
+    assert s.cached_tokens == [0, 64] and s.gpu_hit_blocks == 4
+    # without the cache the second request recomputes everything
+    s0 = S.Scheduler(S_cfg(4096, 16, 16, 4096, False, 0), [0.0, 1.5], [100, 100], [2, 2], prefix_id=[7, 7], prefix_len=[64, 64])
+    assert drive(s0)[2] == [(1, 100, 0)]
+    # a different prefix id, or no prefix, never hits
+    s2 = S.Scheduler(pc_cfg(), [0.0, 1.5, 1.5], [100, 100, 100], [2, 2, 2], prefix_id=[7, 8, -1], prefix_len=[64, 64, 64])
+    assert drive(s2)[2] == [(1, 100, 0), (2, 100, 0)]
+
+
+def test_only_full_blocks_are_shared_and_one_token_is_always_computed():
+    # prefix of 70 tokens = 4 full blocks (64 tokens) + 6 tokens that are not cacheable
+    s = S.Scheduler(pc_cfg(), [0.0, 1.5], [90, 90], [1, 1], prefix_id=[1, 1], prefix_len=[70, 70])
+    assert drive(s)[1] == [(1, 26, 64)]
+    # the whole prompt is cached (64 = 4 blocks): the last block is recomputed so that a token can be sampled
+    s = S.Scheduler(pc_cfg(), [0.0, 1.5], [64, 64], [1, 1], prefix_id=[1, 1], prefix_len=[64, 64])
+    assert drive(s)[1] == [(1, 16, 48)]
+    # requests of the same content but different prefix lengths share the common leading blocks
+    s = S.Scheduler(pc_cfg(), [0.0, 1.5], [200, 200], [1, 1], prefix_id=[1, 1], prefix_len=[128, 40])
+    assert drive(s)[1] == [(1, 168, 32)]
+
+
+def test_shared_blocks_are_counted_once_so_more_requests_run_concurrently():
+    # "... and more concurrent requests from freed KV capacity": a 512-token shared prefix
+    # (32 blocks) + 16 own tokens; 80 blocks hold two such requests without the cache, many with it
+    n = 8
+    args = ([0.0] + [1.5] * (n - 1), [528] * n, [8] * n)
+    on = S.Scheduler(pc_cfg(nb=80), *args, prefix_id=[3] * n, prefix_len=[512] * n)
+    off = S.Scheduler(S_cfg(4096, 16, 16, 80, False, 0), *args, prefix_id=[3] * n, prefix_len=[512] * n)
+    lon, loff = drive(on), drive(off)
+    assert max(len(b) for b in lon) == 8 and max(len(b) for b in loff) == 2
+    assert lon[2] == [(0, 1, 529)] + [(r, 16, 512) for r in range(1, 8)]
+    assert max(on.finish) < max(off.finish) and len(lon) < len(loff)
+    assert sum(on.n_preempt) == 0
+
+
+def test_lru_eviction_and_the_disk_tier():
+    # cache of 12 blocks.  A (prefix 1, 8 blocks) runs and leaves; B (no prefix, 10 blocks) needs the space:
+    # A's unreferenced blocks are evicted.  C (prefix 1) then misses on the GPU tier ...
+    def run(disk):
+        s = S.Scheduler(pc_cfg(bs=16, nb=12, disk=disk), [0.0, 5.0, 10.0], [129, 150, 129], [1, 1, 1],
+                        prefix_id=[1, -1, 1], prefix_len=[128, 0, 128])
+        return s, drive(s)
+    s, log = run(0)
+    assert log == [[(0, 129, 0)], [(1, 150, 0)], [(2, 129, 0)]] and s.evictions == 6 and s.disk_hit_blocks == 0   # 4 free + 6 evicted = B's 10 blocks
+    # ... unless the persistent disk tier still has them: they are loaded instead of recomputed
+    s, log = run(64)
+    assert log[2] == [(2, 1, 128)] and s.disk_hit_blocks == 6 and s.gpu_hit_blocks == 2
+    # a disk tier of 4 blocks keeps only the 4 most recently written blocks (4..7): block 0 is gone, so no leading run
+    s, log = run(4)
+    assert log[2] == [(2, 129, 0)]
+
+
+def test_eviction_takes_the_least_recently_released_blocks_first():
+    # A (prefix 1, 4 blocks) finishes at t = 1, B (prefix 2, 4 blocks) at t = 2; cache of 10 blocks.
+    # D (no prefix, 6 blocks + nothing shared) needs 4 evictions: all of A's go, B's stay.
+    s = S.Scheduler(pc_cfg(bs=16, nb=10), [0.0, 1.0, 2.0, 3.0, 3.0], [65, 65, 90, 65, 65], [1, 1, 1, 1, 1],
+                    prefix_id=[1, 2, -1, 1, 2], prefix_len=[64, 64, 0, 64, 64])
+    log = drive(s)
+    assert log[2] == [(2, 90, 0)] and s.evictions >= 2
+    assert log[3][0] == (3, 65, 0)                      # prefix 1 was evicted (released first) ...
+    assert log[3][1] == (4, 1, 64)                      # ... prefix 2 survived
+
+
+def test_cache_without_prefixes_is_the_plain_scheduler():
+    rng = np.random.Generator(np.random.PCG64(5))
+    n = 50
+    arrival = np.sort(rng.uniform(0, 5, n)).tolist()
+    P, O = rng.integers(1, 300, n).tolist(), rng.integers(1, 40, n).tolist()
+    a = S.Scheduler(S_cfg(256, 8, 16, 60, True, 100), arrival, P, O)
+    b = S.Scheduler(S_cfg(256, 8, 16, 60, False, 0), arrival, P, O)
+    assert drive(a, dt=0.05) == drive(b, dt=0.05) and a.finish == b.finish
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_prefix_cache_invariants_on_random_traces(seed):
+    rng = np.random.Generator(np.random.PCG64(40 + seed))
+    n = 70
+    arrival = np.sort(rng.uniform(0, 10, n)).tolist()
+    pid = rng.integers(-1, 5, n).tolist()
+    plen_of = {p: int(rng.integers(20, 400)) for p in range(5)}
+    own = rng.integers(1, 120, n)
+    plen = [plen_of[p] if p >= 0 else 0 for p in pid]
+    P = [pl + int(o) for pl, o in zip(plen, own)]
+    O = rng.integers(1, 50, n).tolist()
+    nb = int(max(-(-(p + o) // 16) for p, o in zip(P, O)) + rng.integers(5, 60))
+    s = S.Scheduler(S_cfg(int(rng.integers(64, 600)), int(rng.integers(2, 16)), 16, nb, True, int(rng.integers(0, 80))),
+                    arrival, P, O, prefix_id=pid, prefix_len=plen)
+    log = drive(s, dt=0.03)                              # drive() checks the block accounting after every step
+    assert all(math.isfinite(f) for f in s.finish) and s.free_blocks + len(s.lru) == nb
+    assert all(h % 16 == 0 and h <= pl for h, pl in zip(s.cached_tokens, [x * (1 + k) for x, k in zip(plen, s.n_preempt)]))
+    assert sum(s.cached_tokens) > 0
+    if sum(s.n_preempt) == 0:                            # every token is either computed once or served from the cache
+        assert s.tokens_scheduled + sum(s.cached_tokens) == sum(p + o - 1 for p, o in zip(P, O))
