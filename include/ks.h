@@ -210,6 +210,10 @@ typedef struct {
   int32_t max_num_seqs;            /* most requests running at once, >= 1 */
   int32_t block_size;              /* tokens per KV-cache block, >= 1 */
   int32_t num_blocks;              /* KV-cache blocks, >= 1 */
+  int32_t enable_prefix_cache;     /* 0 / 1: content-hashed prefix cache (Q19).  Cached blocks
+                                      live in the same num_blocks pool; unreferenced ones are evicted on demand,
+                                      least recently released first */
+  int32_t disk_blocks;             /* capacity of the persistent disk tier in blocks (LRU); 0 = no disk tier */
 } ks_sched_config;
 
 /* Dense decoder the steps are priced for. */
@@ -221,7 +225,10 @@ typedef struct {
 
 typedef struct {
   int64_t n_steps, tokens_scheduled, n_preemptions;
-  int32_t n_requests, n_finished, n_running, n_waiting, free_blocks, pad;
+  int64_t gpu_hit_blocks, disk_hit_blocks, evictions;     /* prefix cache: blocks served by each tier, GPU-tier evictions */
+  int32_t n_requests, n_finished, n_running, n_waiting;
+  int32_t free_blocks;             /* allocatable blocks: free + cached-but-unreferenced */
+  int32_t pad;
 } ks_sched_stats;
 
 KS_API ks_status ks_sched_create(ks_sched **out, const ks_sched_config *cfg);
@@ -231,6 +238,11 @@ KS_API ks_status ks_sched_create(ks_sched **out, const ks_sched_config *cfg);
  * KS_ESTATE once the first step has been formed. */
 KS_API ks_status ks_sched_add_requests(ks_sched *s, int n, const double *arrival, const int32_t *prompt_len,
                                 const int32_t *max_new);
+/* Same with a shared prefix per request (prefix cache): the first prefix_len[i] prompt tokens of request i are
+ * the content named prefix_id[i] >= 0 (0 <= prefix_len <= prompt_len; prefix_id < 0 = no shared prefix).  Two
+ * requests with the same prefix_id share their common leading FULL blocks.  Both arrays or neither. */
+KS_API ks_status ks_sched_add_prefixed_requests(ks_sched *s, int n, const double *arrival, const int32_t *prompt_len,
+                                         const int32_t *max_new, const int32_t *prefix_id, const int32_t *prefix_len);
 /* Form the batch of the step that starts at `now`.  Writes up to cap entries (request index, new tokens
  * n_new >= 1, cached history hist = computed tokens before the step) in queue order and their number
  * to *n_sched; KS_EINVAL if cap is too small (max_num_seqs always suffices).  *n_sched == 0 means the
@@ -243,8 +255,10 @@ KS_API ks_status ks_sched_step(ks_sched *s, double now, int32_t cap, int32_t *n_
  * leaves and frees its blocks). */
 KS_API ks_status ks_sched_commit(ks_sched *s, double t_end);
 /* Per-request results, each [n_requests] in insertion order (any pointer may be NULL): time of the first
- * and of the last emitted token (NaN while not reached), number of preemptions. */
-KS_API ks_status ks_sched_results(ks_sched *s, double *first_token, double *finish, int32_t *n_preempt);
+ * and of the last emitted token (NaN while not reached), number of preemptions, prompt tokens served from
+ * the prefix cache over all (re)admissions. */
+KS_API ks_status ks_sched_results(ks_sched *s, double *first_token, double *finish, int32_t *n_preempt,
+                           int32_t *cached_tokens);
 KS_API ks_status ks_sched_get_stats(ks_sched *s, ks_sched_stats *out);
 KS_API ks_status ks_sched_destroy(ks_sched *s);
 

@@ -23,7 +23,7 @@ KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
 EXPORTS = ["ks_create", "ks_load_heads", "ks_load_head_ensemble", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
            "ks_compose_steps_weighted",
-           "ks_run_steps", "ks_sched_create", "ks_sched_add_requests", "ks_sched_step", "ks_sched_commit",
+           "ks_run_steps", "ks_sched_create", "ks_sched_add_requests", "ks_sched_add_prefixed_requests", "ks_sched_step", "ks_sched_commit",
            "ks_sched_results", "ks_sched_get_stats", "ks_sched_destroy", "ks_sim_run",
            "ks_get_launch_count", "ks_set_gelu_mode", "ks_destroy", "ks_status_string"]
 
@@ -54,7 +54,7 @@ class ks_step_params(C.Structure):
 
 class ks_sched_config(C.Structure):
     _fields_ = [("max_num_batched_tokens", C.c_int32), ("max_num_seqs", C.c_int32), ("block_size", C.c_int32),
-                ("num_blocks", C.c_int32)]
+                ("num_blocks", C.c_int32), ("enable_prefix_cache", C.c_int32), ("disk_blocks", C.c_int32)]
 
 
 class ks_model_desc(C.Structure):
@@ -64,6 +64,7 @@ class ks_model_desc(C.Structure):
 
 class ks_sched_stats(C.Structure):
     _fields_ = [("n_steps", C.c_int64), ("tokens_scheduled", C.c_int64), ("n_preemptions", C.c_int64),
+                ("gpu_hit_blocks", C.c_int64), ("disk_hit_blocks", C.c_int64), ("evictions", C.c_int64),
                 ("n_requests", C.c_int32), ("n_finished", C.c_int32), ("n_running", C.c_int32),
                 ("n_waiting", C.c_int32), ("free_blocks", C.c_int32), ("pad", C.c_int32)]
 
@@ -102,9 +103,10 @@ def load() -> C.CDLL:
     dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int32)
     L.ks_sched_create.argtypes = [C.POINTER(vp), C.POINTER(ks_sched_config)]
     L.ks_sched_add_requests.argtypes = [vp, i32, dp, ip, ip]
+    L.ks_sched_add_prefixed_requests.argtypes = [vp, i32, dp, ip, ip, ip, ip]
     L.ks_sched_step.argtypes = [vp, C.c_double, C.c_int32, ip, ip, ip, ip, dp]
     L.ks_sched_commit.argtypes = [vp, C.c_double]
-    L.ks_sched_results.argtypes = [vp, dp, dp, ip]
+    L.ks_sched_results.argtypes = [vp, dp, dp, ip, ip]
     L.ks_sched_get_stats.argtypes = [vp, C.POINTER(ks_sched_stats)]
     L.ks_sched_destroy.argtypes = [vp]
     L.ks_sim_run.argtypes = [vp, C.POINTER(vp), dp, i32, C.POINTER(ks_model_desc), C.POINTER(ks_hw_spec), i32,
@@ -298,10 +300,12 @@ class Context:
 class Scheduler:
     """One replica's serving scheduler (ks_sched_*): host logic, needs no GPU.  Marshalling only."""
 
-    def __init__(self, max_num_batched_tokens: int, max_num_seqs: int, block_size: int, num_blocks: int):
+    def __init__(self, max_num_batched_tokens: int, max_num_seqs: int, block_size: int, num_blocks: int,
+                 enable_prefix_cache: bool = False, disk_blocks: int = 0):
         self._lib = load()
         self._h = C.c_void_p()
-        cfg = ks_sched_config(int(max_num_batched_tokens), int(max_num_seqs), int(block_size), int(num_blocks))
+        cfg = ks_sched_config(int(max_num_batched_tokens), int(max_num_seqs), int(block_size), int(num_blocks),
+                              int(bool(enable_prefix_cache)), int(disk_blocks))
         _check(self._lib.ks_sched_create(C.byref(self._h), C.byref(cfg)), "ks_sched_create")
         self.cap = int(max_num_seqs)
         self.n_requests = 0
@@ -309,15 +313,24 @@ class Scheduler:
         self._new = np.zeros(self.cap, np.int32)
         self._hist = np.zeros(self.cap, np.int32)
 
-    def add_requests(self, arrival, prompt_len, max_new) -> None:
+    def add_requests(self, arrival, prompt_len, max_new, prefix_id=None, prefix_len=None) -> None:
         a = np.ascontiguousarray(arrival, dtype=np.float64)
         p = np.ascontiguousarray(prompt_len, dtype=np.int32)
         o = np.ascontiguousarray(max_new, dtype=np.int32)
         if not (a.shape == p.shape == o.shape and a.ndim == 1):
             raise ValueError("arrival, prompt_len, max_new: 1-D arrays of one length")
         ip = C.POINTER(C.c_int32)
-        _check(self._lib.ks_sched_add_requests(self._h, a.shape[0], a.ctypes.data_as(C.POINTER(C.c_double)),
-                                               p.ctypes.data_as(ip), o.ctypes.data_as(ip)), "ks_sched_add_requests")
+        if prefix_id is None and prefix_len is None:
+            _check(self._lib.ks_sched_add_requests(self._h, a.shape[0], a.ctypes.data_as(C.POINTER(C.c_double)),
+                                                   p.ctypes.data_as(ip), o.ctypes.data_as(ip)), "ks_sched_add_requests")
+        else:
+            pi = np.ascontiguousarray(prefix_id, dtype=np.int32)
+            pl = np.ascontiguousarray(prefix_len, dtype=np.int32)
+            if not (pi.shape == pl.shape == a.shape):
+                raise ValueError("prefix_id, prefix_len: one entry per request")
+            _check(self._lib.ks_sched_add_prefixed_requests(self._h, a.shape[0], a.ctypes.data_as(C.POINTER(C.c_double)),
+                                                            p.ctypes.data_as(ip), o.ctypes.data_as(ip), pi.ctypes.data_as(ip),
+                                                            pl.ctypes.data_as(ip)), "ks_sched_add_prefixed_requests")
         self.n_requests += int(a.shape[0])
 
     def step(self, now: float):
@@ -338,10 +351,11 @@ class Scheduler:
         ft = np.zeros(self.n_requests, np.float64)
         fin = np.zeros(self.n_requests, np.float64)
         npre = np.zeros(self.n_requests, np.int32)
-        dp = C.POINTER(C.c_double)
+        cached = np.zeros(self.n_requests, np.int32)
+        dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int32)
         _check(self._lib.ks_sched_results(self._h, ft.ctypes.data_as(dp), fin.ctypes.data_as(dp),
-                                          npre.ctypes.data_as(C.POINTER(C.c_int32))), "ks_sched_results")
-        return dict(first_token=ft, finish=fin, n_preempt=npre)
+                                          npre.ctypes.data_as(ip), cached.ctypes.data_as(ip)), "ks_sched_results")
+        return dict(first_token=ft, finish=fin, n_preempt=npre, cached_tokens=cached)
 
     def stats(self) -> dict:
         st = ks_sched_stats()

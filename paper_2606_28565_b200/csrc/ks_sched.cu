@@ -13,7 +13,9 @@
 #include <cstring>
 #include <deque>
 #include <limits>
+#include <list>
 #include <new>
+#include <unordered_map>
 #include <vector>
 
 #include "ks_internal.h"
@@ -31,11 +33,77 @@ struct ks_sched {
   // the batch being executed
   std::vector<int32_t> b_req, b_new, b_hist;
   bool pending = false;
-  int32_t free_blocks = 0;
+  int32_t free_blocks = 0;             // blocks holding nothing (cached blocks nobody references are in `lru`)
   int64_t n_steps = 0, tokens = 0, preemptions = 0;
   int32_t n_finished = 0;
 
+  // prefix cache (Q19).  Key of full block j of prefix content p: p << 32 | j.
+  struct GpuBlock {
+    int32_t ref = 0;
+    std::list<uint64_t>::iterator pos;   // position in `lru` while ref == 0
+  };
+  std::vector<int32_t> prefix_id, prefix_len, registered, cached_tokens;
+  std::vector<std::vector<uint64_t>> held;                 // keys a request holds a reference on
+  std::unordered_map<uint64_t, GpuBlock> gpu;              // GPU tier
+  std::list<uint64_t> lru;                                 // unreferenced cached blocks, least recently released first
+  std::list<uint64_t> disk_order;                          // disk tier, least recently used first
+  std::unordered_map<uint64_t, std::list<uint64_t>::iterator> disk;
+  int64_t gpu_hits = 0, disk_hits = 0, evictions = 0;
+  std::vector<uint64_t> hit_keys;                          // scratch of the admission lookup
+  std::vector<uint8_t> hit_on_disk;
+
   int32_t blocks_for(int64_t tokens_) const { return (int32_t)((tokens_ + cfg.block_size - 1) / cfg.block_size); }
+  int32_t avail() const { return free_blocks + (int32_t)lru.size(); }
+  static uint64_t key_of(int32_t p, int32_t j) { return ((uint64_t)(uint32_t)p << 32) | (uint32_t)j; }
+
+  // k <= avail() blocks for a request: free ones first, then the least recently released cached ones
+  void alloc(int32_t k) {
+    const int32_t from_free = std::min(k, free_blocks);
+    free_blocks -= from_free;
+    for (k -= from_free; k > 0; --k) {
+      gpu.erase(lru.front());
+      lru.pop_front();
+      ++evictions;
+    }
+  }
+  // request r gives everything back: private blocks become free, shared ones lose a reference
+  void release(int32_t r) {
+    free_blocks += blocks[r] - (int32_t)held[r].size();
+    for (uint64_t key : held[r]) {
+      GpuBlock& g = gpu[key];
+      if (--g.ref == 0) g.pos = lru.insert(lru.end(), key);
+    }
+    held[r].clear();
+    blocks[r] = 0;
+    registered[r] = 0;
+  }
+  void disk_put(uint64_t key) {
+    if (cfg.disk_blocks <= 0) return;
+    auto it = disk.find(key);
+    if (it != disk.end()) {
+      disk_order.splice(disk_order.end(), disk_order, it->second);
+      return;
+    }
+    disk[key] = disk_order.insert(disk_order.end(), key);
+    if ((int64_t)disk_order.size() > cfg.disk_blocks) {
+      disk.erase(disk_order.front());
+      disk_order.pop_front();
+    }
+  }
+  // leading run of r's prefix blocks found in the GPU tier, else the disk tier; one token is always left
+  void lookup(int32_t r) {
+    hit_keys.clear();
+    hit_on_disk.clear();
+    if (!cfg.enable_prefix_cache || prefix_id[r] < 0) return;
+    const int32_t limit = std::min(prefix_len[r] / cfg.block_size, (n_tok[r] - 1) / cfg.block_size);
+    for (int32_t j = 0; j < limit; ++j) {
+      const uint64_t key = key_of(prefix_id[r], j);
+      if (gpu.count(key)) hit_on_disk.push_back(0);
+      else if (disk.count(key)) hit_on_disk.push_back(1);
+      else break;
+      hit_keys.push_back(key);
+    }
+  }
 };
 
 namespace {
@@ -57,7 +125,7 @@ void sched_form_batch(ks_sched* s, double now) {
   int32_t budget = s->cfg.max_num_batched_tokens;
   bool preempted = false;
   auto take = [s, &budget](int32_t r, int32_t n_new, int32_t need) {
-    s->free_blocks -= need;
+    s->alloc(need);
     s->blocks[r] += need;
     s->b_req.push_back(r); s->b_new.push_back(n_new); s->b_hist.push_back(s->computed[r]);
     budget -= n_new;
@@ -68,11 +136,10 @@ void sched_form_batch(ks_sched* s, double now) {
     const int32_t n_new = std::min(s->n_tok[r] - s->computed[r], budget);
     const int32_t need = s->blocks_for((int64_t)s->computed[r] + n_new) - s->blocks[r];
     bool self = false;
-    while (need > s->free_blocks) {        // KV pressure: the back of the running queue is recomputed later
+    while (need > s->avail()) {            // KV pressure: the back of the running queue is recomputed later
       const int32_t v = s->running.back();
       s->running.pop_back();
-      s->free_blocks += s->blocks[v];
-      s->blocks[v] = 0;
+      s->release(v);
       s->computed[v] = 0;
       ++s->n_preempt[v];
       ++s->preemptions;
@@ -88,9 +155,34 @@ void sched_form_batch(ks_sched* s, double now) {
   if (!preempted) {
     while (!s->waiting.empty() && budget > 0 && (int32_t)s->running.size() < s->cfg.max_num_seqs) {
       const int32_t r = s->waiting.front();
-      const int32_t n_new = std::min(s->n_tok[r] - s->computed[r], budget);
-      const int32_t need = s->blocks_for((int64_t)s->computed[r] + n_new) - s->blocks[r];
-      if (need > s->free_blocks) break;
+      // prefix-cache-aware admission: cached leading blocks are referenced (GPU tier) or loaded (disk tier)
+      // instead of recomputed; a waiting request always starts from computed == 0
+      s->lookup(r);
+      const int32_t n_hit = (int32_t)s->hit_keys.size();
+      const int32_t hit = n_hit * s->cfg.block_size;
+      const int32_t n_new = std::min(s->n_tok[r] - hit, budget);
+      const int32_t need = s->blocks_for((int64_t)hit + n_new) - n_hit;
+      int32_t taken = need;                 // blocks that leave the allocatable pool
+      for (int32_t j = 0; j < n_hit; ++j) taken += s->hit_on_disk[j] ? 1 : (s->gpu[s->hit_keys[j]].ref == 0 ? 1 : 0);
+      if (taken > s->avail()) break;
+      for (int32_t j = 0; j < n_hit; ++j) {          // reference the GPU hits first: they must not be evicted below
+        if (s->hit_on_disk[j]) continue;
+        ks_sched::GpuBlock& g = s->gpu[s->hit_keys[j]];
+        if (g.ref++ == 0) s->lru.erase(g.pos);
+        ++s->gpu_hits;
+      }
+      for (int32_t j = 0; j < n_hit; ++j) {
+        if (!s->hit_on_disk[j]) continue;
+        s->alloc(1);
+        s->gpu[s->hit_keys[j]].ref = 1;
+        s->disk_put(s->hit_keys[j]);
+        ++s->disk_hits;
+      }
+      s->held[r].assign(s->hit_keys.begin(), s->hit_keys.end());
+      s->registered[r] = n_hit;
+      s->blocks[r] = n_hit;
+      s->computed[r] = hit;
+      s->cached_tokens[r] += hit;
       s->waiting.pop_front();
       s->running.push_back(r);
       take(r, n_new, need);
@@ -108,12 +200,25 @@ void sched_commit(ks_sched* s, double t_end) {
     const int32_t r = s->b_req[k];
     s->computed[r] += s->b_new[k];
     s->tokens += s->b_new[k];
+    if (s->cfg.enable_prefix_cache && s->prefix_id[r] >= 0) {
+      // full prefix blocks whose KV now exists go to the cache (one of r's private blocks becomes the shared
+      // copy; if the key is already cached r keeps a private duplicate) and, written through, to the disk tier
+      const int32_t full = std::min(s->computed[r], s->prefix_len[r]) / s->cfg.block_size;
+      for (int32_t j = s->registered[r]; j < full; ++j) {
+        const uint64_t key = ks_sched::key_of(s->prefix_id[r], j);
+        if (!s->gpu.count(key)) {
+          s->gpu[key].ref = 1;
+          s->held[r].push_back(key);
+        }
+        s->disk_put(key);
+      }
+      s->registered[r] = std::max(s->registered[r], full);
+    }
     if (s->computed[r] != s->n_tok[r]) continue;
     if (++s->generated[r] == 1) s->first_token[r] = t_end;
     if (s->generated[r] == s->max_new[r]) {
       s->finish[r] = t_end;
-      s->free_blocks += s->blocks[r];
-      s->blocks[r] = 0;
+      s->release(r);
       s->running.erase(std::find(s->running.begin(), s->running.end(), r));
       ++s->n_finished;
     } else {
@@ -134,7 +239,8 @@ extern "C" {
 ks_status ks_sched_create(ks_sched** out, const ks_sched_config* cfg) {
   if (!out) return KS_EINVAL;
   *out = nullptr;
-  if (!cfg || cfg->max_num_batched_tokens < 1 || cfg->max_num_seqs < 1 || cfg->block_size < 1 || cfg->num_blocks < 1)
+  if (!cfg || cfg->max_num_batched_tokens < 1 || cfg->max_num_seqs < 1 || cfg->block_size < 1 || cfg->num_blocks < 1 ||
+      cfg->disk_blocks < 0 || (cfg->enable_prefix_cache != 0 && cfg->enable_prefix_cache != 1))
     return KS_EINVAL;
   ks_sched* s = new (std::nothrow) ks_sched();
   if (!s) return KS_ENOMEM;
@@ -145,10 +251,17 @@ ks_status ks_sched_create(ks_sched** out, const ks_sched_config* cfg) {
 }
 
 ks_status ks_sched_add_requests(ks_sched* s, int n, const double* arrival, const int32_t* prompt_len, const int32_t* max_new) {
+  return ks_sched_add_prefixed_requests(s, n, arrival, prompt_len, max_new, nullptr, nullptr);
+}
+
+ks_status ks_sched_add_prefixed_requests(ks_sched* s, int n, const double* arrival, const int32_t* prompt_len,
+                                         const int32_t* max_new, const int32_t* prefix_id, const int32_t* prefix_len) {
   if (!s || n < 0 || (n > 0 && (!arrival || !prompt_len || !max_new))) return KS_EINVAL;
+  if ((prefix_id == nullptr) != (prefix_len == nullptr)) return KS_EINVAL;
   if (s->started) return KS_ESTATE;
   for (int i = 0; i < n; ++i) {
     if (!std::isfinite(arrival[i]) || prompt_len[i] < 1 || max_new[i] < 1) return KS_EINVAL;
+    if (prefix_id && prefix_id[i] >= 0 && (prefix_len[i] < 0 || prefix_len[i] > prompt_len[i])) return KS_EINVAL;
     if (s->blocks_for((int64_t)prompt_len[i] + max_new[i]) > s->cfg.num_blocks) return KS_EINVAL;
   }
   if ((int64_t)s->arrival.size() + n > (int64_t)std::numeric_limits<int32_t>::max()) return KS_EINVAL;
@@ -162,6 +275,12 @@ ks_status ks_sched_add_requests(ks_sched* s, int n, const double* arrival, const
       s->generated.push_back(0);
       s->blocks.push_back(0);
       s->n_preempt.push_back(0);
+      const bool pre = prefix_id && prefix_id[i] >= 0;
+      s->prefix_id.push_back(pre ? prefix_id[i] : -1);
+      s->prefix_len.push_back(pre ? prefix_len[i] : 0);
+      s->registered.push_back(0);
+      s->cached_tokens.push_back(0);
+      s->held.emplace_back();
       s->first_token.push_back(std::numeric_limits<double>::quiet_NaN());
       s->finish.push_back(std::numeric_limits<double>::quiet_NaN());
     }
@@ -196,12 +315,13 @@ ks_status ks_sched_commit(ks_sched* s, double t_end) {
   return KS_OK;
 }
 
-ks_status ks_sched_results(ks_sched* s, double* first_token, double* finish, int32_t* n_preempt) {
+ks_status ks_sched_results(ks_sched* s, double* first_token, double* finish, int32_t* n_preempt, int32_t* cached_tokens) {
   if (!s) return KS_EINVAL;
   const size_t n = s->arrival.size();
   if (first_token && n) memcpy(first_token, s->first_token.data(), n * sizeof(double));
   if (finish && n) memcpy(finish, s->finish.data(), n * sizeof(double));
   if (n_preempt && n) memcpy(n_preempt, s->n_preempt.data(), n * sizeof(int32_t));
+  if (cached_tokens && n) memcpy(cached_tokens, s->cached_tokens.data(), n * sizeof(int32_t));
   return KS_OK;
 }
 
@@ -215,7 +335,10 @@ ks_status ks_sched_get_stats(ks_sched* s, ks_sched_stats* out) {
   out->n_finished = s->n_finished;
   out->n_running = (int32_t)s->running.size();
   out->n_waiting = (int32_t)s->waiting.size();
-  out->free_blocks = s->free_blocks;
+  out->free_blocks = s->avail();
+  out->gpu_hit_blocks = s->gpu_hits;
+  out->disk_hit_blocks = s->disk_hits;
+  out->evictions = s->evictions;
   return KS_OK;
 }
 

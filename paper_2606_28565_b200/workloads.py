@@ -517,6 +517,10 @@ class Replica:
     arrival: np.ndarray      # float64 [n] seconds
     prompt_len: np.ndarray   # int32 [n]
     max_new: np.ndarray      # int32 [n]
+    enable_prefix_cache: bool = False
+    disk_blocks: int = 0
+    prefix_id: Optional[np.ndarray] = None    # int32 [n], -1 = no shared prefix
+    prefix_len: Optional[np.ndarray] = None   # int32 [n]
 
 
 def serving_trace(rng, n: int, rate: float, prompt_mean: float = 512.0, out_mean: float = 128.0):
@@ -527,6 +531,21 @@ def serving_trace(rng, n: int, rate: float, prompt_mean: float = 512.0, out_mean
     p = np.clip(np.round(rng.lognormal(np.log(prompt_mean) - 0.5, 1.0, size=n)), 8, 8192).astype(np.int32)
     o = np.clip(np.round(rng.lognormal(np.log(out_mean) - 0.32, 0.8, size=n)), 1, 1024).astype(np.int32)
     return arrival.astype(np.float64), p, o
+
+
+def add_shared_prefixes(rng, rep: Replica, n_prefixes: int = 8, share: float = 0.7, disk_blocks: int = 0) -> Replica:
+    """Give `share` of the requests one of n_prefixes shared system prompts (log-uniform 64..2048 tokens, Zipf-like
+    popularity) in front of their own prompt, and switch the replica's prefix cache on."""
+    n = rep.arrival.shape[0]
+    plen_of = _log_uniform_int(rng, 64, 2048, n_prefixes)
+    pop = 1.0 / np.arange(1, n_prefixes + 1)
+    pid = np.where(rng.random(n) < share, rng.choice(n_prefixes, size=n, p=pop / pop.sum()), -1).astype(np.int32)
+    plen = np.where(pid >= 0, plen_of[np.maximum(pid, 0)], 0).astype(np.int32)
+    rep.prefix_id, rep.prefix_len = pid, plen
+    rep.prompt_len = np.minimum(rep.prompt_len + plen, 8192).astype(np.int32)
+    rep.prefix_len = np.minimum(rep.prefix_len, rep.prompt_len).astype(np.int32)
+    rep.enable_prefix_cache, rep.disk_blocks = True, int(disk_blocks)
+    return rep
 
 
 def sim_replicas(n_replicas: int = 64, n_requests: int = 200, seed: int = 6, pressure: bool = False) -> List[Replica]:

@@ -35,7 +35,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(B.ks_step_params) == 20
     assert C.sizeof(B.ks_desc_batch) == 32 + 8 * B.KS_MAX_COLS + 8
     assert (C.sizeof(B.ks_sched_config), C.sizeof(B.ks_model_desc), C.sizeof(B.ks_sched_stats),
-            C.sizeof(B.ks_sim_stats)) == (16, 36, 48, 64)
+            C.sizeof(B.ks_sim_stats)) == (24, 36, 72, 64)
 
 
 def test_status_strings(lib):

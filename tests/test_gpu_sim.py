@@ -32,8 +32,9 @@ def ks():
 def make_scheds(B, reps):
     out = []
     for r in reps:
-        s = B.Scheduler(r.max_num_batched_tokens, r.max_num_seqs, r.block_size, r.num_blocks)
-        s.add_requests(r.arrival, r.prompt_len, r.max_new)
+        s = B.Scheduler(r.max_num_batched_tokens, r.max_num_seqs, r.block_size, r.num_blocks, r.enable_prefix_cache,
+                        r.disk_blocks)
+        s.add_requests(r.arrival, r.prompt_len, r.max_new, r.prefix_id, r.prefix_len)
         out.append(s)
     return out
 
@@ -44,8 +45,9 @@ def replay_and_check(B, reps, model, spec, tier, params, heads, scheds, clock, s
     worst = 0.0
     for i, r in enumerate(reps):
         forced = time_log[rep_log == i].astype(np.float64)
-        o = S.Scheduler(S.SchedConfig(r.max_num_batched_tokens, r.max_num_seqs, r.block_size, r.num_blocks),
-                        r.arrival, r.prompt_len, r.max_new)
+        o = S.Scheduler(S.SchedConfig(r.max_num_batched_tokens, r.max_num_seqs, r.block_size, r.num_blocks,
+                                      r.enable_prefix_cache, r.disk_blocks),
+                        r.arrival, r.prompt_len, r.max_new, r.prefix_id, r.prefix_len)
         end, _, batches = S.simulate(o, lambda b: 0.0, forced=forced, max_steps=len(forced))
         assert len(batches) == len(forced)
         res = scheds[i].results()
@@ -53,7 +55,8 @@ def replay_and_check(B, reps, model, spec, tier, params, heads, scheds, clock, s
         # identical clocks => identical decisions: per-request times and counters are bit-equal
         assert np.array_equal(res["first_token"], np.array(o.first_token), equal_nan=True)
         assert np.array_equal(res["finish"], np.array(o.finish), equal_nan=True)
-        assert res["n_preempt"].tolist() == o.n_preempt
+        assert res["n_preempt"].tolist() == o.n_preempt and res["cached_tokens"].tolist() == o.cached_tokens
+        assert (st["gpu_hit_blocks"], st["disk_hit_blocks"], st["evictions"]) == (o.gpu_hit_blocks, o.disk_hit_blocks, o.evictions)
         assert (st["n_steps"], st["tokens_scheduled"], st["n_finished"]) == (o.n_steps, o.tokens_scheduled, o.n_finished)
         assert clock[i] == end
         # every step time the CUDA path produced vs the oracle's price of the same batch
@@ -67,16 +70,22 @@ def replay_and_check(B, reps, model, spec, tier, params, heads, scheds, clock, s
     return worst
 
 
-@pytest.mark.parametrize("tier,pressure,tp", [(W.TIER_NONE, False, 1), (W.TIER_NONE, True, 4), (W.TIER_A, False, 1)])
-def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp):
+@pytest.mark.parametrize("tier,pressure,tp,prefix", [(W.TIER_NONE, False, 1, False), (W.TIER_NONE, True, 4, False),
+                                                     (W.TIER_A, False, 1, False), (W.TIER_NONE, True, 1, True)])
+def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp, prefix):
     B = ks
     reps = W.sim_replicas(n_replicas=5, n_requests=40, seed=70 + tp, pressure=pressure)
+    if prefix:          # shared system prompts + a two-tier prefix cache
+        rng = np.random.Generator(np.random.PCG64(77))
+        reps = [W.add_shared_prefixes(rng, r, disk_blocks=256) for r in reps]
     if pressure:        # a burst of requests into a cache of 1024 tokens: decoding outgrows it and forces recomputation
         for r in reps:
             r.prompt_len = np.minimum(r.prompt_len, 600).astype(np.int32)
             r.max_new = np.minimum(r.max_new, 200).astype(np.int32)
             r.arrival = r.arrival * 0.01
             r.num_blocks = 64
+            if prefix:
+                r.prefix_len = np.minimum(r.prefix_len, r.prompt_len).astype(np.int32)
     model = W.ServingModel(tp=tp)
     spec = W.spec_gb200()
     params = W.STEP_PARAMS_CFG4
@@ -97,6 +106,8 @@ def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp):
               f"preemptions {sum(s.stats()['n_preemptions'] for s in scheds)}")
         if pressure:
             assert sum(s.stats()["n_preemptions"] for s in scheds) > 0
+        if prefix:
+            assert sum(s.stats()["gpu_hit_blocks"] for s in scheds) > 0
     finally:
         ctx.close()
 

@@ -25,10 +25,12 @@ def step_time(batch):
 
 
 def run_both(rep: W.Replica, max_steps=200000):
-    o = S.Scheduler(S.SchedConfig(rep.max_num_batched_tokens, rep.max_num_seqs, rep.block_size, rep.num_blocks),
-                    rep.arrival, rep.prompt_len, rep.max_new)
-    p = B.Scheduler(rep.max_num_batched_tokens, rep.max_num_seqs, rep.block_size, rep.num_blocks)
-    p.add_requests(rep.arrival, rep.prompt_len, rep.max_new)
+    o = S.Scheduler(S.SchedConfig(rep.max_num_batched_tokens, rep.max_num_seqs, rep.block_size, rep.num_blocks,
+                                  rep.enable_prefix_cache, rep.disk_blocks),
+                    rep.arrival, rep.prompt_len, rep.max_new, rep.prefix_id, rep.prefix_len)
+    p = B.Scheduler(rep.max_num_batched_tokens, rep.max_num_seqs, rep.block_size, rep.num_blocks,
+                    rep.enable_prefix_cache, rep.disk_blocks)
+    p.add_requests(rep.arrival, rep.prompt_len, rep.max_new, rep.prefix_id, rep.prefix_len)
     now, steps = 0.0, 0
     while not o.done():
         bo = o.step(now)
@@ -50,7 +52,9 @@ def run_both(rep: W.Replica, max_steps=200000):
     assert np.array_equal(res["first_token"], np.array(o.first_token))
     assert np.array_equal(res["finish"], np.array(o.finish))
     assert res["n_preempt"].tolist() == o.n_preempt
+    assert res["cached_tokens"].tolist() == o.cached_tokens
     st = p.stats()
+    assert (st["gpu_hit_blocks"], st["disk_hit_blocks"], st["evictions"]) == (o.gpu_hit_blocks, o.disk_hit_blocks, o.evictions)
     assert (st["n_steps"], st["tokens_scheduled"], st["n_preemptions"]) == (o.n_steps, o.tokens_scheduled, sum(o.n_preempt))
     assert (st["n_requests"], st["n_finished"], st["n_running"], st["n_waiting"]) == (len(o.P), len(o.P), 0, 0)
     assert st["free_blocks"] == rep.num_blocks
@@ -82,6 +86,43 @@ def test_matches_oracle_on_small_adversarial_configs(seed):
     arrival = np.round(np.sort(rng.uniform(0, 2.0, n)), 2)          # many equal arrival times: ties by index
     rep = W.Replica(int(rng.integers(8, 400)), int(rng.integers(1, 20)), bs, nb, arrival, P, O)
     run_both(rep)
+
+
+@pytest.mark.parametrize("seed,disk", [(0, 0), (1, 0), (2, 300), (3, 2000), (4, 40), (5, 0)])
+def test_prefix_cache_matches_oracle(seed, disk):
+    rng = np.random.Generator(np.random.PCG64(800 + seed))
+    hits = ev = dh = 0
+    for rep in W.sim_replicas(n_replicas=3, n_requests=120, seed=80 + seed):
+        rep = W.add_shared_prefixes(rng, rep, disk_blocks=disk)
+        rep.arrival = rep.arrival * 0.05                       # a burst: many requests in flight at once
+        rep.num_blocks = int(-(-int((rep.prompt_len + rep.max_new).max()) // 16) + rng.integers(50, 400))
+        o = run_both(rep)
+        hits, ev, dh = hits + o.gpu_hit_blocks, ev + o.evictions, dh + o.disk_hit_blocks
+    assert hits > 0 and ev > 0
+    if disk >= 300:
+        assert dh > 0                                          # evicted blocks came back from the disk tier
+
+
+def test_prefix_cache_hand_worked():
+    # tests/test_oracle_sched.py::test_lru_eviction_and_the_disk_tier, product side
+    p = B.Scheduler(4096, 16, 16, 12, True, 64)
+    p.add_requests([0.0, 5.0, 10.0], [129, 150, 129], [1, 1, 1], [1, -1, 1], [128, 0, 128])
+    now, log = 0.0, []
+    while True:
+        b, nxt = p.step(now)
+        if not b:
+            if not math.isfinite(nxt):
+                break
+            now = max(now, nxt)
+            continue
+        log.append(b)
+        now += 1.0
+        p.commit(now)
+    assert log == [[(0, 129, 0)], [(1, 150, 0)], [(2, 1, 128)]]
+    st = p.stats()
+    assert (st["gpu_hit_blocks"], st["disk_hit_blocks"], st["evictions"]) == (2, 6, 6)
+    assert p.results()["cached_tokens"].tolist() == [0, 0, 128]
+    p.close()
 
 
 def test_hand_worked_schedule():
