@@ -362,6 +362,16 @@ def run_extras(h: Harness, peaks):
                                    launches=3, note="streaming kernel, ~300 instructions per row: issue-bound")
     del st
     torch.cuda.empty_cache()
+    # the packed bf16x2 activation mode of the Tier-A kernels (ks_set_gelu_mode(1); not the default: ~4x the
+    # activation rounding error, still 10x inside the 1e-2 bar) on the bench workload
+    st = h.prepare(W.config2())
+    h.ctx.set_gelu_mode(1)
+    ms = h.timed([lambda: h.predict(st)], EX_ITERS, EX_WARM)[:, 0]
+    h.ctx.set_gelu_mode(0)
+    ex["cfg2_gelu_mode1"] = dict(ms=float(ms.mean()), predictions_per_s=float(st["w"].n_rows / (ms.mean() * 1e-3)),
+                                 note="Tier-A kernel only; packed bf16x2 GELU arithmetic")
+    del st
+    torch.cuda.empty_cache()
     # NEXT-2: MLP ensembles (Q17), 4 members of width 32 per family of cfg2, packed into one pass of the Tier-A kernel
     we = W.config2()
     rng = np.random.Generator(np.random.PCG64(13))

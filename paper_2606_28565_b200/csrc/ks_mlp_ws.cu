@@ -2,7 +2,8 @@
 // cores.  S1-S3, S4a, S5 of DESIGN.md §1 (PAPER.md:191 Eq. 2, :199-201 per-family heads), fused.
 //
 // One persistent CTA per SM walks a contiguous range of 128-row tiles.  A work item q is one
-// (tile, spec) pair; item q uses buffer q & 1 of every double-buffered resource.
+// (tile, spec) pair; item q uses buffer q & 1 of every double-buffered resource (A1, D1, D2) and
+// buffer q % 3 of the layer-2 operand A2.
 //
 //   warps 0-3    PRODUCER  thread r owns row r: prefetch next tile's columns, decode + roofline +
 //                          features -> bf16 A1[q&1] row in smem (K-major UMMA image), t_roof -> ring
@@ -18,9 +19,14 @@
 //   a1_full[2]   128 producer arrivals      -> MMA may read A1[b]
 //   mma1_done[2] tcgen05.commit             -> EPI1 may read D1[b]; producer may rewrite A1[b]
 //   d1_free[2]   128 EPI1 arrivals          -> D1[b] has been drained: MMA1(q+2) may overwrite it
-//   a2_full[2]   128 EPI1 arrivals          -> MMA may read A2[b]
-//   mma2_done[2] tcgen05.commit             -> EPI2 may read D2[b]; EPI1 may rewrite A2[b]
-//   d2_free[2]   128 EPI2 arrivals          -> MMA may overwrite D2[b]
+//   a2_full[3]   128 EPI1 arrivals          -> MMA may read A2[q % 3]
+//   mma2_done[2] tcgen05.commit             -> EPI2 may read D2[b]
+//   a2_free[3]   tcgen05.commit             -> MMA2(q) has read A2[q % 3]: EPI1 of item q + 3 may rewrite it
+//   d2_free[2]   128 EPI2 arrivals          -> D2[b] has been drained: MMA2(q+2) may overwrite it
+// A2 has three buffers and D1/D2 are released as soon as their last tcgen05.ld has completed, because
+// the warpgroup that finishes item q is the one that continues with item q + 2 of the same buffer: with
+// two A2 buffers (or a late release) it would sit out a whole MMA2 per item (cycle trace of one CTA:
+// ~1100 of ~6300 cycles per item and group).
 // A waiter for completion k of a barrier always runs before completion k+1 can happen (k+1 depends
 // on the waiter's own progress), so single-bit phase parity is sufficient.
 // The t_roof ring has 8 entries: the producer can be at most 7 items ahead of EPI2 (item q+8 needs
@@ -39,6 +45,7 @@ constexpr int kProducerWarps = 4, kEpiWarps = 8;
 constexpr int kWsThreads = (kProducerWarps + 2 * kEpiWarps + 1) * 32;   // 672
 constexpr int kMmaWarp = kProducerWarps + 2 * kEpiWarps;
 constexpr int kRing = 8;
+constexpr int kA2Bufs = 3;     // A2 (layer-2 operand) is triple-buffered: item q uses A2[q % 3]
 
 template <int NIN, int H>
 struct WsCfg {
@@ -55,16 +62,16 @@ struct WsCfg {
   static constexpr int OFF_ONES = OFF_W2 + W2_BYTES;
   static constexpr int OFF_A1 = OFF_ONES + ONES_BYTES;
   static constexpr int OFF_A2 = OFF_A1 + 2 * A1_BYTES;
-  static constexpr int OFF_W3 = OFF_A2 + 2 * A2_BYTES;                 // [KS_MLP_MAX_BUCKETS][H] fp32
+  static constexpr int OFF_W3 = OFF_A2 + kA2Bufs * A2_BYTES;           // [KS_MLP_MAX_BUCKETS][H] fp32
   static constexpr int OFF_RING = OFF_W3 + KS_MLP_MAX_BUCKETS * H * 4; // [kRing][128] fp32 t_roof
   static constexpr int OFF_BAR = OFF_RING + kRing * kRows * 4;
-  static constexpr int SMEM_BYTES = OFF_BAR + 192;   // barriers + TMEM slot (128) + TileMap
+  static constexpr int SMEM_BYTES = OFF_BAR + 224;   // barriers + TMEM slot (160) + TileMap
   static constexpr int NCHUNK = H / 32;
 };
 
 // barrier slots inside the OFF_BAR block
-enum { BAR_W = 0, BAR_DRAIN = 1, BAR_A1_FULL = 2, BAR_MMA1 = 4, BAR_A2_FULL = 6, BAR_MMA2 = 8, BAR_D2_FREE = 10,
-       BAR_D1_FREE = 12, BAR_COUNT = 14 };
+enum { BAR_W = 0, BAR_DRAIN = 1, BAR_A1_FULL = 2, BAR_MMA1 = 4, BAR_A2_FULL = 6, BAR_MMA2 = 9, BAR_D2_FREE = 11,
+       BAR_D1_FREE = 13, BAR_A2_FREE = 15, BAR_COUNT = 18 };
 
 struct Range { int lo, hi; };
 KS_DEV Range bucket_range(const TileMap& tm, int b, int t_lo, int t_hi) {
@@ -140,9 +147,10 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
   const uint32_t grp = (uint32_t)e >> 7;                           // warpgroup of this role: owns buffer grp
   const int r = e & 127;                                           // TMEM lane = tile row
   const uint32_t lane_off = (uint32_t)((r >> 5) * 32) << 16;
+  uint32_t a2i = grp, a2p = 0;                                     // q % 3 and the parity of q / 3
   for (uint32_t q = grp; q < n_items; q += 2) {
     const uint32_t buf = q & 1u, par = (q >> 1) & 1u;
-    unsigned char* A2 = smem + C::OFF_A2 + buf * C::A2_BYTES;
+    unsigned char* A2 = smem + C::OFF_A2 + a2i * C::A2_BYTES;
     const uint32_t d1 = tmem_base + buf * H + lane_off;
     ks_mbar_wait(bars + BAR_MMA1 + buf, par);                       // D1[buf] holds item q
     ks_tc_fence_after();
@@ -151,7 +159,9 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
     // roles together fits the 32 KB instruction cache.
     uint32_t accA[16], accB[16];
     ks_tmem_ld16(d1, accA);
-    if (q >= 2u) ks_mbar_wait(bars + BAR_MMA2 + buf, par ^ 1u);     // MMA2(q-2) has consumed A2[buf]
+    // MMA2(q-3) has consumed A2[q % 3].  With two A2 buffers this group would sit out the whole MMA2(q-2),
+    // which can only start when the group's previous item is finished (measured: ~1100 of ~6300 cycles).
+    if (q >= 3u) ks_mbar_wait(bars + BAR_A2_FREE + a2i, a2p ^ 1u);
     auto act_store = [&](const uint32_t* a, int c16) {
       uint32_t pk[8];
       if (GM == 0) {
@@ -180,7 +190,9 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
       act_store(accB, c + 1);
     }
     ks_fence_proxy_async();
-    ks_mbar_arrive(bars + BAR_A2_FULL + buf);
+    ks_mbar_arrive(bars + BAR_A2_FULL + a2i);
+    a2i += 2u;
+    if (a2i >= 3u) { a2i -= 3u; a2p ^= 1u; }
   }
 }
 
@@ -204,19 +216,31 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble, members of H / members columns
     const int ens_mask = members > 1 ? H / 16 / members - 1 : 0;     // member width is 32 or 64: a power-of-two chunk count
     const int tile0 = tm.tb[b], ne = tm.ne[b];
-    for (int t = tr.lo; t < tr.hi; ++t) {
-      const int pos = (t - tile0) * kRows + r;
-      const bool valid = pos < ne;
-      const int row = valid ? map_row(bk, pos) : 0;
-      for (int s = 0; s < p.n_specs; ++s, ++q) {
-        if ((q & 1u) != grp) continue;
-        const uint32_t buf = q & 1u, par = (q >> 1) & 1u;
+    // Everything the item loop needs from the kernel parameters is read once per bucket into registers
+    // (the asm keeps the compiler from re-reading it with indexed constant loads on every item: measured
+    // ~900 idle cycles between two items of a group), and a thread only walks its own group's items.
+    const int* idx = bk.idx;
+    float* lat = bk.lat;
+    int bn = bk.n, n_specs = p.n_specs;
+    asm volatile("" : "+l"(idx), "+l"(lat), "+r"(bn), "+r"(n_specs));
+    const uint32_t n_it = tr.lo < tr.hi ? (uint32_t)(tr.hi - tr.lo) * (uint32_t)n_specs : 0u;
+    const uint32_t q0 = q;
+    q += n_it;
+    int t = tr.lo, s = (int)((q0 & 1u) ^ grp);       // first item of this group in the bucket: i = (q0 & 1) ^ grp
+    while (n_it != 0u && s >= n_specs) { s -= n_specs; ++t; }
+    for (uint32_t i = (q0 & 1u) ^ grp; i < n_it; i += 2u) {
+      const uint32_t qi = q0 + i;
+      {
+        const int pos = (t - tile0) * kRows + r;
+        const bool valid = pos < ne;
+        const int row = valid ? (idx ? __ldg(idx + pos) : pos) : 0;
+        const uint32_t buf = qi & 1u, par = (qi >> 1) & 1u;
         const uint32_t d2 = tmem_base + 2 * H + buf * H + lane_off;
         ks_mbar_wait(bars + BAR_MMA2 + buf, par);                   // D2[buf] holds item q
         ks_tc_fence_after();
         uint32_t accA[16], accB[16];
         ks_tmem_ld16(d2, accA);
-        const float t_roof = ring[(q & (kRing - 1)) * kRows + r];
+        const float t_roof = ring[(qi & (kRing - 1)) * kRows + r];
         float z0 = 0.0f, z1 = 0.0f, z2 = 0.0f, z3 = 0.0f;
         auto act_dot = [&](const uint32_t* a, int c16) {
           if (GM == 0) {
@@ -250,7 +274,15 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
             ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
             act_dot(accA, c);
             ks_tmem_ld_wait();
-            if (c + 2 < H / 16) ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
+            if (c + 2 < H / 16) {
+              ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
+            } else {
+              // D2[buf] is drained: MMA2(q+2) may overwrite it while the last sub-chunk is still being
+              // activated.  This group is the one that will wait for that MMA2 (measured: a bubble of a
+              // whole MMA2, ~1150 cycles per item, when the release came after the loop).
+              ks_tc_fence_before();
+              ks_mbar_arrive(bars + BAR_D2_FREE + buf);
+            }
             act_dot(accB, c + 1);
             if (decltype(ens)::value && ((c + 2) & ens_mask) == 0) {   // last column of member m (Q17)
               const float z = ((z0 + z1) + (z2 + z3)) + hd.b3m[m++];
@@ -260,8 +292,6 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
           }
         };
         if (members > 1) sweep(std::true_type{}); else sweep(std::false_type{});
-        ks_tc_fence_before();                      // orders this thread's tcgen05.ld before MMA2(q+2)
-        ks_mbar_arrive(bars + BAR_D2_FREE + buf);
         if (valid) {
           float eta;
           if (members > 1) {
@@ -272,9 +302,11 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
             // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
             eta = fminf(1.0f + __expf(-z), 1024.0f);
           }
-          bk.lat[(long long)s * bk.n + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
+          lat[(long long)s * bn + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
         }
       }
+      s += 2;
+      while (s >= n_specs) { s -= n_specs; ++t; }
     }
   }
 }
@@ -292,14 +324,15 @@ KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, con
   const uint32_t a1_addr = ks_smem_u32(smem + C::OFF_A1);
   const uint32_t a2_addr = ks_smem_u32(smem + C::OFF_A2);
   uint32_t wphase = 0, dphase = 0, q = 0;
+  uint32_t m2i = 0, m2p = 0;                        // A2 buffer (q % 3) and parity of q / 3 of the next MMA2
 
   auto mma2 = [&](uint32_t i) {                     // D2[i&1] = A2[i&1] . W2 + ones x b2
     const uint32_t buf = i & 1u, par = (i >> 1) & 1u;
-    ks_mbar_wait_backoff(bars + BAR_A2_FULL + buf, par);
+    ks_mbar_wait_backoff(bars + BAR_A2_FULL + m2i, m2p);
     if (i >= 2u) ks_mbar_wait_backoff(bars + BAR_D2_FREE + buf, par ^ 1u);
     ks_tc_fence_after();
     const uint32_t d2 = tmem_base + 2 * H + buf * H;
-    const uint32_t a = a2_addr + buf * C::A2_BYTES;
+    const uint32_t a = a2_addr + m2i * C::A2_BYTES;
 #pragma unroll
     for (int k16 = 0; k16 < H / 16; ++k16) {
       const uint64_t ad = ks_umma_desc(a + k16 * 2 * kChunkBytes, kChunkBytes, 128);
@@ -309,7 +342,9 @@ KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, con
     const uint64_t ad = ks_umma_desc(ones_addr, kChunkBytes, 128);
     const uint64_t bd = ks_umma_desc(w2_addr + (H / 8) * B_LBO, B_LBO, 128);
     ks_umma_bf16(d2, ad, bd, idesc, 1u);
-    ks_umma_commit(bars + BAR_MMA2 + buf);
+    ks_umma_commit(bars + BAR_MMA2 + buf);          // D2[buf] is complete (EPI2)
+    ks_umma_commit(bars + BAR_A2_FREE + m2i);       // ... and A2[q % 3] has been read (EPI1 of item q + 3)
+    if (++m2i == 3u) { m2i = 0; m2p ^= 1u; }
   };
 
   auto mma1 = [&](uint32_t i) {                     // D1[i&1] = A1[i&1] . W1
@@ -365,7 +400,7 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + BAR_COUNT);
-  TileMap* tmp = reinterpret_cast<TileMap*>(smem + C::OFF_BAR + 128);
+  TileMap* tmp = reinterpret_cast<TileMap*>(smem + C::OFF_BAR + 160);
   const int tid = threadIdx.x;
   const int warp = tid >> 5;
 
@@ -373,10 +408,13 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
   if (tid == 0) {
     ks_mbar_init(bars + BAR_W, 1);
     ks_mbar_init(bars + BAR_DRAIN, 1);
+    for (int i = 0; i < kA2Bufs; ++i) {
+      ks_mbar_init(bars + BAR_A2_FULL + i, 128);
+      ks_mbar_init(bars + BAR_A2_FREE + i, 1);
+    }
     for (int i = 0; i < 2; ++i) {
       ks_mbar_init(bars + BAR_A1_FULL + i, 128);
       ks_mbar_init(bars + BAR_MMA1 + i, 1);
-      ks_mbar_init(bars + BAR_A2_FULL + i, 128);
       ks_mbar_init(bars + BAR_MMA2 + i, 1);
       ks_mbar_init(bars + BAR_D2_FREE + i, 128);
       ks_mbar_init(bars + BAR_D1_FREE + i, 128);

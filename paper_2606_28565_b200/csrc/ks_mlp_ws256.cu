@@ -206,11 +206,17 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble (2, 4 or 8 members here)
     const int ens_mask = members > 1 ? H / 16 / members - 1 : 0;     // chunks per member - 1 (member width 32 .. 128)
     const int tile0 = tm.tb[b], ne = tm.ne[b];
+    // per-bucket parameters live in registers across the item loop (the asm keeps the compiler from
+    // re-reading them with indexed constant loads between two items; see ks_mlp_ws.cu)
+    const int* idx = bk.idx;
+    float* lat = bk.lat;
+    int bn = bk.n, n_specs = p.n_specs;
+    asm volatile("" : "+l"(idx), "+l"(lat), "+r"(bn), "+r"(n_specs));
     for (int t = tr.lo; t < tr.hi; ++t) {
       const int pos = (t - tile0) * kRows + r;
       const bool valid = pos < ne;
-      const int row = valid ? map_row(bk, pos) : 0;
-      for (int s = 0; s < p.n_specs; ++s, ++q) {
+      const int row = valid ? (idx ? __ldg(idx + pos) : pos) : 0;
+      for (int s = 0; s < n_specs; ++s, ++q) {
         ks_mbar_wait(bars + BAR_MMA2, q & 1u);                      // D2 holds item q
         ks_tc_fence_after();
         uint32_t accA[16], accB[16];
@@ -273,7 +279,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
           // eta = 1/e, guarded at e >= 2^-10 (Q3): 1 + exp(-z) for one head, k / sum of the members'
           // sigmoids for an ensemble; Eq. 2 floor after eta
           const float eta = fminf(members > 1 ? __fdividef((float)members, z) : 1.0f + __expf(-(z + b3)), 1024.0f);
-          bk.lat[(long long)s * bk.n + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
+          lat[(long long)s * bn + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
         }
       }
     }
