@@ -53,10 +53,12 @@ struct Cfg256 {
   static constexpr int OFF_RING = OFF_B2 + H * 4;             // [kRing][128] fp32 t_roof
   static constexpr int OFF_ZP = OFF_RING + kRing * kRows * 4; // [2][128] fp32 partial dots of warpgroup 1
   static constexpr int OFF_BAR = OFF_ZP + 2 * kRows * 4;
-  static constexpr int SMEM_BYTES = OFF_BAR + 192;
+  static constexpr int SMEM_BYTES = OFF_BAR + 256;   // 21 barriers + TMEM slot (192) + TileMap
 };
 
-enum { BAR_W = 0, BAR_DRAIN, BAR_A1_FULL, BAR_MMA1, BAR_D1_FREE, BAR_MMA2, BAR_D2_FREE, BAR_A2_FULL,
+// MMA2, D2_FREE, Z_FULL, Z_FREE come in pairs (column half of D2 / parity of the item)
+enum { BAR_W = 0, BAR_DRAIN, BAR_A1_FULL, BAR_MMA1, BAR_D1_FREE, BAR_MMA2, BAR_D2_FREE = BAR_MMA2 + 2,
+       BAR_Z_FULL = BAR_D2_FREE + 2, BAR_Z_FREE = BAR_Z_FULL + 2, BAR_A2_FULL = BAR_Z_FREE + 2,
        BAR_A2_FREE = BAR_A2_FULL + kGroups, BAR_COUNT = BAR_A2_FREE + kGroups };
 
 struct Range { int lo, hi; };
@@ -196,11 +198,11 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     const Range tr = bucket_range(tm, b, t_lo, t_hi);
     if (tr.lo >= tr.hi) continue;
     const KsBucketDev& bk = p.bk[b];
-    // this family's layer-3 weights and layer-2 bias (all 256 EPI2 threads; nobody still reads the old ones)
-    ks_bar_sync(2, 2 * 128);
+    // this family's layer-3 weights and layer-2 bias: a warpgroup stages and reads only its own 128 columns
+    ks_bar_sync(2 + wg, 128);
     sw3[e] = __ldg(p.head[b].w3 + e);
     sb2[e] = __ldg(p.head[b].b2 + e);
-    ks_bar_sync(2, 2 * 128);
+    ks_bar_sync(2 + wg, 128);
     const KsHeadDev& hd = p.head[b];
     const float b3 = hd.b3;
     const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble (2, 4 or 8 members here)
@@ -217,7 +219,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
       const bool valid = pos < ne;
       const int row = valid ? (idx ? __ldg(idx + pos) : pos) : 0;
       for (int s = 0; s < n_specs; ++s, ++q) {
-        ks_mbar_wait(bars + BAR_MMA2, q & 1u);                      // D2 holds item q
+        ks_mbar_wait(bars + BAR_MMA2 + wg, q & 1u);                 // this half of D2 holds item q
         ks_tc_fence_after();
         uint32_t accA[16], accB[16];
         ks_tmem_ld16(d2, accA);
@@ -258,7 +260,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
               ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
             } else {                                                  // D2 is drained: MMA2(q+1) may overwrite it
               ks_tc_fence_before();
-              ks_mbar_arrive(bars + BAR_D2_FREE);
+              ks_mbar_arrive(bars + BAR_D2_FREE + wg);
             }
             act_dot(accB, c + 1);
             if (decltype(ens)::value && ((c + 2) & ens_mask) == 0) {  // last column of member m (Q17)
@@ -271,11 +273,20 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
         if (members > 1) sweep(std::true_type{}); else sweep(std::false_type{});
         // single head: partial logit of this half; ensemble: partial sum of efficiencies
         float z = members > 1 ? esum : (z0 + z1) + (z2 + z3);
-        // the two column halves meet in shared memory (double-buffered by item parity)
-        if (wg == 1) zpart[(q & 1u) * kRows + r] = z;
-        ks_bar_sync(2, 2 * 128);
-        if (wg == 0 && valid) {
-          z += zpart[(q & 1u) * kRows + r];
+        // The two column halves meet in shared memory.  Warpgroup 0 (first half of D2, ready one MMA pass
+        // earlier) leaves its partial in zpart[q & 1] and moves on; warpgroup 1 picks it up and writes
+        // the result.  z_full / z_free hand the two slots back and forth.
+        const uint32_t zb = q & 1u, zpar = (q >> 1) & 1u;
+        if (wg == 0) {
+          if (q >= 2u) ks_mbar_wait(bars + BAR_Z_FREE + zb, zpar ^ 1u);
+          zpart[zb * kRows + r] = z;
+          ks_mbar_arrive(bars + BAR_Z_FULL + zb);
+        } else {
+          ks_mbar_wait(bars + BAR_Z_FULL + zb, zpar);
+          z += zpart[zb * kRows + r];
+          ks_mbar_arrive(bars + BAR_Z_FREE + zb);
+        }
+        if (wg == 1 && valid) {
           // eta = 1/e, guarded at e >= 2^-10 (Q3): 1 + exp(-z) for one head, k / sum of the members'
           // sigmoids for an ensemble; Eq. 2 floor after eta
           const float eta = fminf(members > 1 ? __fdividef((float)members, z) : 1.0f + __expf(-(z + b3)), 1024.0f);
@@ -291,7 +302,8 @@ template <int NIN>
 KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
                     uint64_t* bars, const uint32_t tmem_base) {
   using C = Cfg256<NIN>;
-  constexpr uint32_t idesc = ks_umma_idesc_bf16(128, H);
+  constexpr uint32_t idesc = ks_umma_idesc_bf16(128, H);          // layer 1: N = 256
+  constexpr uint32_t idesc_half = ks_umma_idesc_bf16(128, H / 2); // layer 2: one column half per pass
   constexpr uint32_t B_LBO = H * 16;
   const uint32_t w1_addr = ks_smem_u32(smem + C::OFF_W1);
   const uint32_t w2_addr = ks_smem_u32(smem + C::OFF_W2);
@@ -311,19 +323,24 @@ KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, con
     }
     ks_umma_commit(bars + BAR_MMA1);
   };
-  auto mma2_group = [&](uint32_t i, int g, bool first, bool last) {   // K group g (64 columns) of D2 += A2 . W2
-    ks_mbar_wait_backoff(bars + BAR_A2_FULL + g, i & 1u);
-    if (first && i >= 1u) ks_mbar_wait_backoff(bars + BAR_D2_FREE, (i - 1u) & 1u);
+  // Layer 2 runs as two passes over K, one per 128-column half of D2 (W2 rows [128 h, 128 h + 128) =
+  // byte offset 2048 h inside every 8-deep K chunk of the image): EPI2's warpgroup 0 activates half 0
+  // while the tensor core is still accumulating half 1, and half h of item q+1 only waits for
+  // warpgroup h to have drained half h of item q.  With one N = 256 pass the activation of D2 and the
+  // next MMA2 could never overlap (D1 + D2 fill TMEM, so D2 cannot be double-buffered).
+  auto mma2_group = [&](uint32_t i, int h, int g, bool first, bool last) {   // K group g of D2[half h] += A2 . W2
+    if (h == 0) ks_mbar_wait_backoff(bars + BAR_A2_FULL + g, i & 1u);
+    if (first && i >= 1u) ks_mbar_wait_backoff(bars + BAR_D2_FREE + h, (i - 1u) & 1u);
     ks_tc_fence_after();
 #pragma unroll
     for (int kk = 0; kk < 4; ++kk) {
       const int k16 = g * 4 + kk;
       const uint64_t ad = ks_umma_desc(a2_addr + k16 * 2 * kChunkBytes, kChunkBytes, 128);
-      const uint64_t bd = ks_umma_desc(w2_addr + k16 * 2 * B_LBO, B_LBO, 128);
-      ks_umma_bf16(d2, ad, bd, idesc, (first && kk == 0) ? 0u : 1u);
+      const uint64_t bd = ks_umma_desc(w2_addr + k16 * 2 * B_LBO + h * (H / 2) * 16, B_LBO, 128);
+      ks_umma_bf16(d2 + (uint32_t)(h * (H / 2)), ad, bd, idesc_half, (first && kk == 0) ? 0u : 1u);
     }
-    ks_umma_commit(bars + BAR_A2_FREE + g);         // EPI1 may rewrite this K group for the next item
-    if (last) ks_umma_commit(bars + BAR_MMA2);
+    if (h == 1) ks_umma_commit(bars + BAR_A2_FREE + g);   // both passes have read this K group: EPI1 may rewrite it
+    if (last) ks_umma_commit(bars + BAR_MMA2 + h);
   };
 
   for (int b = 0; b < p.n_buckets; ++b) {
@@ -343,14 +360,18 @@ KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, con
     const uint32_t q1 = q + (uint32_t)(tr.hi - tr.lo) * (uint32_t)p.n_specs;
     mma1(q);                                        // D1 is free: the previous family's last item was drained
     for (; q < q1; ++q) {
-      mma2_group(q, 0, true, false);
-      mma2_group(q, 2, false, false);
+      mma2_group(q, 0, 0, true, false);
+      mma2_group(q, 0, 2, false, false);
       if (q + 1u < q1) {                            // layer 1 of the next item as soon as D1 is drained
         ks_mbar_wait_backoff(bars + BAR_D1_FREE, q & 1u);
         mma1(q + 1u);
       }
-      mma2_group(q, 1, false, false);
-      mma2_group(q, 3, false, true);
+      mma2_group(q, 0, 1, false, false);
+      mma2_group(q, 0, 3, false, true);
+      mma2_group(q, 1, 0, true, false);
+      mma2_group(q, 1, 2, false, false);
+      mma2_group(q, 1, 1, false, false);
+      mma2_group(q, 1, 3, false, true);
     }
   }
 }
@@ -362,7 +383,7 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + BAR_COUNT);
-  TileMap* tmp = reinterpret_cast<TileMap*>(smem + C::OFF_BAR + 128);
+  TileMap* tmp = reinterpret_cast<TileMap*>(smem + C::OFF_BAR + 192);
   const int tid = threadIdx.x;
   const int warp = tid >> 5;
 
@@ -373,8 +394,12 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
     ks_mbar_init(bars + BAR_A1_FULL, 128);
     ks_mbar_init(bars + BAR_MMA1, 1);
     ks_mbar_init(bars + BAR_D1_FREE, 256);
-    ks_mbar_init(bars + BAR_MMA2, 1);
-    ks_mbar_init(bars + BAR_D2_FREE, 256);
+    for (int h = 0; h < 2; ++h) {
+      ks_mbar_init(bars + BAR_MMA2 + h, 1);
+      ks_mbar_init(bars + BAR_D2_FREE + h, 128);
+      ks_mbar_init(bars + BAR_Z_FULL + h, 128);
+      ks_mbar_init(bars + BAR_Z_FREE + h, 128);
+    }
     for (int g = 0; g < kGroups; ++g) {
       ks_mbar_init(bars + BAR_A2_FULL + g, 128);
       ks_mbar_init(bars + BAR_A2_FREE + g, 1);
