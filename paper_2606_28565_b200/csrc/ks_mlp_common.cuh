@@ -22,6 +22,16 @@ KS_PTX float gelu2_f32(float x) {
   const float t = ks_tanh_approx(x * p);
   return fmaf(x, t, x);
 }
+// Two activations at once with packed fp32 instructions (FMUL2, FFMA2, FMUL2, 2 x MUFU.TANH, FFMA2):
+// bit-identical to gelu2_f32 on each element, 3 issue slots per activation instead of 5.
+KS_PTX void gelu2_f32x2(float xa, float xb, float& ga, float& gb) {
+  float x2a, x2b, pa, pb, ua, ub;
+  ks_mul2(x2a, x2b, xa, xb, xa, xb);
+  ks_fma2(pa, pb, x2a, x2b, 0.0356774081f, 0.0356774081f, 0.7978845608f, 0.7978845608f);
+  ks_mul2(ua, ub, xa, xb, pa, pb);
+  const float ta = ks_tanh_approx(ua), tb = ks_tanh_approx(ub);
+  ks_fma2(ga, gb, xa, xb, ta, tb, xa, xb);
+}
 // packed bf16x2 variant (two activations per FMA-pipe instruction; MUFU.TANH.BF16 per half)
 KS_PTX uint32_t gelu2_bf16x2(float a, float b) {
   const uint32_t x = ks_pack_bf16x2(a, b);

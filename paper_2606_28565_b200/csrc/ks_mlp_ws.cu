@@ -166,8 +166,11 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
       uint32_t pk[8];
       if (GM == 0) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
-          pk[j] = ks_pack_bf16x2_alu(gelu2_f32(__uint_as_float(a[2 * j])), gelu2_f32(__uint_as_float(a[2 * j + 1])));
+        for (int j = 0; j < 8; ++j) {
+          float g0, g1;
+          gelu2_f32x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]), g0, g1);
+          pk[j] = ks_pack_bf16x2_alu(g0, g1);
+        }
       } else {
 #pragma unroll
         for (int j = 0; j < 8; ++j) pk[j] = gelu2_bf16x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]));
@@ -247,10 +250,11 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
 #pragma unroll
             for (int j = 0; j < 16; j += 4) {
               const float4 w4 = *reinterpret_cast<const float4*>(sw3 + c16 * 16 + j);
-              z0 = fmaf(gelu2_f32(__uint_as_float(a[j + 0])), w4.x, z0);
-              z1 = fmaf(gelu2_f32(__uint_as_float(a[j + 1])), w4.y, z1);
-              z2 = fmaf(gelu2_f32(__uint_as_float(a[j + 2])), w4.z, z2);
-              z3 = fmaf(gelu2_f32(__uint_as_float(a[j + 3])), w4.w, z3);
+              float g0, g1, g2, g3;
+              gelu2_f32x2(__uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), g0, g1);
+              gelu2_f32x2(__uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), g2, g3);
+              ks_fma2(z0, z1, g0, g1, w4.x, w4.y, z0, z1);
+              ks_fma2(z2, z3, g2, g3, w4.z, w4.w, z2, z3);
             }
           } else {
 #pragma unroll

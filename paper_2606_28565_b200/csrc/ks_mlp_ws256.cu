@@ -141,8 +141,11 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
     uint32_t pk[8];
     if (GM == 0) {
 #pragma unroll
-      for (int j = 0; j < 8; ++j)
-        pk[j] = ks_pack_bf16x2_alu(gelu2_f32(__uint_as_float(a[2 * j])), gelu2_f32(__uint_as_float(a[2 * j + 1])));
+      for (int j = 0; j < 8; ++j) {
+        float g0, g1;
+        gelu2_f32x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]), g0, g1);
+        pk[j] = ks_pack_bf16x2_alu(g0, g1);
+      }
     } else {
 #pragma unroll
       for (int j = 0; j < 8; ++j) pk[j] = gelu2_bf16x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]));
@@ -231,13 +234,15 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
           for (int j = 0; j < 16; j += 4) {
             const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col + j);
             const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
-            const float x0 = __uint_as_float(a[j + 0]) + b4.x, x1 = __uint_as_float(a[j + 1]) + b4.y;
-            const float x2 = __uint_as_float(a[j + 2]) + b4.z, x3 = __uint_as_float(a[j + 3]) + b4.w;
+            float x0, x1, x2, x3;
+            ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
+            ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
             if (GM == 0) {
-              z0 = fmaf(gelu2_f32(x0), w4.x, z0);
-              z1 = fmaf(gelu2_f32(x1), w4.y, z1);
-              z2 = fmaf(gelu2_f32(x2), w4.z, z2);
-              z3 = fmaf(gelu2_f32(x3), w4.w, z3);
+              float g0, g1, g2, g3;
+              gelu2_f32x2(x0, x1, g0, g1);
+              gelu2_f32x2(x2, x3, g2, g3);
+              ks_fma2(z0, z1, g0, g1, w4.x, w4.y, z0, z1);
+              ks_fma2(z2, z3, g2, g3, w4.z, w4.w, z2, z3);
             } else {
               const uint32_t g0 = gelu2_bf16x2(x0, x1), g1 = gelu2_bf16x2(x2, x3);
               z0 = fmaf(__uint_as_float(g0 << 16), w4.x, z0);
