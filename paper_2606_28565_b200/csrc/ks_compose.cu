@@ -54,6 +54,7 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
 
   // launched with programmatic stream serialization: the launch itself overlaps the tail of the
   // prediction kernel; nothing it produced (nor anything copied in for this call) is read before this
+  ks_launch_dependents();            // ... and the totals kernel may be scheduled under this one
   cudaGridDependencySynchronize();
   for (int idx = tid; idx < p.n_batches * (kS + 1); idx += kThreads) {
     const int b = idx / (kS + 1), j = idx - b * (kS + 1);

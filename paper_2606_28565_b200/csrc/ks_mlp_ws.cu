@@ -408,6 +408,7 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
   const int tid = threadIdx.x;
   const int warp = tid >> 5;
 
+  ks_launch_dependents();     // the step kernel's launch overlaps this kernel (it waits for our completion itself)
   if (tid == 32) tile_map_init(p, tmp);
   if (tid == 0) {
     ks_mbar_init(bars + BAR_W, 1);

@@ -107,6 +107,11 @@ KS_PTX void ks_add2(float& d0, float& d1, float a0, float a1, float b0, float b1
       : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
 }
 
+// Programmatic dependent launch: lets the next kernel of the stream (if it was launched with the
+// programmatic-stream-serialization attribute) be scheduled now; it still waits in
+// cudaGridDependencySynchronize() until this grid has completed and flushed its writes.
+KS_PTX void ks_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 KS_PTX void ks_bar_sync(uint32_t id, uint32_t nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }

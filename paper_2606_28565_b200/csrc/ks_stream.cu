@@ -141,6 +141,7 @@ KS_DEV float trilinear(const int* v, const KsGridDev& g, const float* __restrict
 template <int FAM, int TIER, bool F32, bool ONE>
 __global__ void __launch_bounds__(TIER == KS_TIER_B ? (FAM == KS_FAM_GROUPED_GEMM ? 512 : 1024) : 256)
 ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
+  ks_launch_dependents();     // a step kernel launched behind this one may be scheduled now (it waits for us itself)
   constexpr int NC = NCols<FAM>::v;
   extern __shared__ __align__(128) float sgrid[];
 
