@@ -66,7 +66,6 @@ struct WsCfg {
   static constexpr int OFF_RING = OFF_W3 + KS_MLP_MAX_BUCKETS * H * 4; // [kRing][128] fp32 t_roof
   static constexpr int OFF_BAR = OFF_RING + kRing * kRows * 4;
   static constexpr int SMEM_BYTES = OFF_BAR + 224;   // barriers + TMEM slot (160) + TileMap
-  static constexpr int NCHUNK = H / 32;
 };
 
 // barrier slots inside the OFF_BAR block
