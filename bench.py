@@ -413,6 +413,23 @@ def run_extras(h: Harness, peaks):
                              tflops=float(tf), frac_tensor_sustained=float(tf / peaks["bf16_sustained"]))
     del st
     torch.cuda.empty_cache()
+    # SURVEY.md §8(d) caveat (i): cfg 3's kernels last ~20 us and cfg 4a's attention bucket 16 us (launch ramp,
+    # 128 KiB grid staging per CTA); the same kernels at 16x / 8x the row count show the steady rate
+    if not PROFILE:
+        st = h.prepare(W.config3(n=16 * 4_194_304))
+        ex["asymptotic_cfg3_tierB_x16"] = dict(stream=stream_roofline(h, st, peaks, iters=3))
+        del st
+        torch.cuda.empty_cache()
+        w4 = W.config4()
+        attn = next(b for b in w4.buckets if b.family == W.FAM_ATTN)
+        big = W.Bucket(W.FAM_ATTN, [np.tile(c, 8) for c in attn.cols], dtype_bytes=attn.dtype_bytes, hq=attn.hq,
+                       hkv=attn.hkv, head_dim=attn.head_dim)
+        w8 = W.Workload("cfg4a_attention_x8", [big], w4.specs, W.TIER_NONE)
+        del w4
+        st = h.prepare_rows(w8)
+        ex["asymptotic_cfg4a_attention_x8"] = dict(stream=stream_roofline(h, st, peaks, iters=3))
+        del st
+        torch.cuda.empty_cache()
     ex["sim_closed_loop"] = sim_extras(h)
     return ex
 
