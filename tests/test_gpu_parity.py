@@ -153,6 +153,27 @@ def test_tier_a_all_head_shapes_with_wide_weights(ks, n_in, h):
     print(n_in, h, "wide-weight max rel err", errs)
 
 
+def test_tier_a_and_composition_are_bit_reproducible(ks):
+    # no atomics, fixed reduction orders, one warp-specialized pipeline per SM: two runs of the same call (and a run
+    # on a second context) give identical bits, for 128- and 256-wide heads and for the step composition
+    B, D = ks
+    for w in (W.config2(n=50021), W.config5(n_rows=30011, n_specs=3, n_layers=4)):
+        outs = []
+        for rep in range(3):
+            ctx = B.Context(0)
+            try:
+                D.load_models(ctx, w)
+                db = D.to_device(w)
+                g = D.predict(ctx, w, dbuckets=db)
+                step, tot = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+                outs.append(([x["lat"].copy() for x in g], step.copy(), tot.copy()))
+            finally:
+                ctx.close()
+        for o in outs[1:]:
+            assert all(np.array_equal(a, b) for a, b in zip(o[0], outs[0][0]))
+            assert np.array_equal(o[1], outs[0][1]) and np.array_equal(o[2], outs[0][2])
+
+
 def test_tier_a_packed_gelu_mode_within_tolerance(ks):
     w = W.config2(n=40013)
     errs = run_and_check(ks, w, TOL_MLP, gelu_mode=1)
