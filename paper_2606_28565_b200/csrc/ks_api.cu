@@ -841,10 +841,21 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   KS_CUDA(c, cudaStreamWaitEvent(c->h2d, c->ev_start, 0));
   for (int b = 0; b < n_batches; ++b) {
     const size_t n = batches[b].n;
-    for (int k = 0; k < batches[b].n_cols; ++k) {
-      void* d = ws_take(c, n * 4);
-      if (n) KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[k], n * 4, cudaMemcpyHostToDevice, c->h2d));
-      cols[b][k] = d;
+    // columns that lie back to back in host memory (one block per bucket) move with ONE copy: a step is
+    // PCIe-bound and every separate copy costs a few microseconds of link idle time
+    bool adjacent = n > 0 && n % 4 == 0 && batches[b].n_cols > 1;
+    for (int k = 0; adjacent && k + 1 < batches[b].n_cols; ++k)
+      adjacent = static_cast<const char*>(batches[b].cols[k + 1]) == static_cast<const char*>(batches[b].cols[k]) + n * 4;
+    if (adjacent) {
+      char* d = static_cast<char*>(ws_take(c, n * 4 * batches[b].n_cols));
+      KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[0], n * 4 * batches[b].n_cols, cudaMemcpyHostToDevice, c->h2d));
+      for (int k = 0; k < batches[b].n_cols; ++k) cols[b][k] = d + (size_t)k * n * 4;
+    } else {
+      for (int k = 0; k < batches[b].n_cols; ++k) {
+        void* d = ws_take(c, n * 4);
+        if (n) KS_CUDA(c, cudaMemcpyAsync(d, batches[b].cols[k], n * 4, cudaMemcpyHostToDevice, c->h2d));
+        cols[b][k] = d;
+      }
     }
     int32_t* dofs = static_cast<int32_t*>(ws_take(c, (size_t)(n_steps + 1) * 4));
     KS_CUDA(c, cudaMemcpyAsync(dofs, step_off[b], (size_t)(n_steps + 1) * 4, cudaMemcpyHostToDevice, c->h2d));

@@ -54,7 +54,12 @@ def to_pinned(w: Workload) -> List[DeviceBucket]:
     torch = _torch()
     out = []
     for b in w.buckets:
-        cols = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in b.cols]
+        # one pinned block per bucket, columns back to back: the library moves adjacent columns with one copy
+        if b.cols and all(c.dtype == b.cols[0].dtype and c.shape == b.cols[0].shape for c in b.cols):
+            block = torch.from_numpy(np.ascontiguousarray(np.stack(b.cols))).pin_memory()
+            cols = [block[k] for k in range(block.shape[0])]
+        else:
+            cols = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in b.cols]
         so = torch.from_numpy(np.ascontiguousarray(b.step_off, dtype=np.int32)).pin_memory() if b.step_off is not None else None
         mu = torch.from_numpy(np.ascontiguousarray(b.mult, dtype=np.int32)).pin_memory() if b.mult is not None else None
         out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu))
