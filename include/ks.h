@@ -186,7 +186,10 @@ KS_API ks_status ks_compose_steps_weighted(ks_ctx *ctx, const float *const *late
 /* Convenience: ks_predict_kernels followed by ks_compose_steps in one call (one pass of the whole
  * hot path; rows with batches[b].mult are weighted as in ks_compose_steps_weighted).  latency may be NULL (or hold NULL entries): per-kernel latencies then stay in the
  * library workspace and only the step/config results are returned.  With KS_MEM_HOST this is the
- * end-to-end call: descriptors and offsets go host->device, results device->host, then sync. */
+ * end-to-end call: descriptors and offsets go host->device, results device->host, then sync.  Buckets are
+ * pipelined in the caller's order (bucket b is copied while bucket b-1 is predicted: largest first is best);
+ * pinned host memory is what makes the copies asynchronous, and the columns of a bucket that lie back to
+ * back in host memory (cols[k+1] == cols[k] + 4 n, n a multiple of 4) move with a single copy. */
 KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const int32_t *const *step_off,
                        int n_batches, const ks_hw_spec *specs, int n_specs, ks_tier tier, int n_steps,
                        const ks_step_params *params, const int32_t *cfg_off, int n_cfg,
