@@ -403,14 +403,20 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
   A.cap_rows[2] = 6 * n_replicas;
   A.cap_rows[3] = n_replicas;
   if (attn_rows > A.cap_rows[1]) return KS_EUNSUPPORTED;
+  // Fixed-size arrays first (a few rows per replica), the step times, and last the attention columns, which
+  // are packed behind each other every iteration at their actual length: what an iteration reads is one
+  // prefix of the arena, a few hundred KB at most.
   size_t at = 0;
   for (int f = 0; f < A.n_fam; ++f) {
-    for (int c = 0; c < n_cols[f]; ++c) { A.col[f][c] = at; at = a16(at + (size_t)A.cap_rows[f] * 4); }
-    A.mult[f] = at; at = a16(at + (size_t)A.cap_rows[f] * 4);
+    if (f != 1) {
+      for (int c = 0; c < n_cols[f]; ++c) { A.col[f][c] = at; at = a16(at + (size_t)A.cap_rows[f] * 4); }
+      A.mult[f] = at; at = a16(at + (size_t)A.cap_rows[f] * 4);
+    }
     A.off[f] = at; at = a16(at + (size_t)(n_replicas + 1) * 4);
   }
-  const size_t in_bytes = at;
   A.out = at; at = a16(at + (size_t)n_replicas * 4);
+  const size_t attn_base = at;
+  at += 4 * a16((size_t)A.cap_rows[1] * 4);
   A.bytes = at;
 
   cudaStream_t st = ks_internal_stream(ctx);
@@ -421,10 +427,8 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
 
   // Pinned host memory is addressable from the device (unified addressing), and an iteration is bound by
   // launch and copy latency, not bandwidth: the step times are always written straight into the pinned arena,
-  // and a small arena is also read in place (measured 47 vs 55 us per iteration at 256 replicas); a large one
-  // is moved by one DMA copy.
-  const bool in_place = in_bytes <= (256u << 10);
-  char* in_base = in_place ? A.host : A.dev;
+  // and an iteration whose rows fit 256 KB is also read in place (measured 47 vs 55 us per iteration); a
+  // larger one is moved by one DMA copy of exactly the bytes in use.
   char* out_base = A.host;
   std::vector<int> active;
   active.reserve(n_replicas);
@@ -441,6 +445,8 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
     active.clear();
     int n_rows[4] = {0, 0, 0, 0};
     for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[0] = 0;
+    // pass 1: every unfinished replica forms its batch
+    int64_t attn_total = 0;
     for (int r = 0; r < n_replicas; ++r) {
       ks_sched* s = scheds[r];
       if (sched_done(s)) continue;
@@ -452,6 +458,20 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
         sched_form_batch(s, clock[r]);
       }
       if (s->b_req.empty()) continue;
+      active.push_back(r);
+      attn_total += (int64_t)s->b_req.size();
+    }
+    const int n_act = (int)active.size();
+    if (n_act == 0) break;
+    // pass 2: the batches' rows; the attention columns are packed at their actual length
+    const size_t attn_stride = a16((size_t)attn_total * 4);
+    for (int c = 0; c < 3; ++c) A.col[1][c] = attn_base + (size_t)c * attn_stride;
+    A.mult[1] = attn_base + 3 * attn_stride;
+    const size_t in_bytes = attn_base + 4 * attn_stride;
+    const bool in_place = in_bytes <= (256u << 10);
+    char* in_base = in_place ? A.host : A.dev;
+    for (int ai = 0; ai < n_act; ++ai) {
+      ks_sched* s = scheds[active[ai]];
       // rows of this step: dense kernels at the total token count, attention per request
       int32_t T = 0;
       for (int32_t v : s->b_new) T += v;
@@ -489,13 +509,9 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
         const int k = n_rows[3]++;
         I(A.col[3][0])[k] = T * m.hidden * m.dtype_bytes; I(A.col[3][1])[k] = m.tp; I(A.mult[3])[k] = 2 * L;
       }
-      active.push_back(r);
-      const int a = (int)active.size();
-      for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[a] = n_rows[f];
+      for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[ai + 1] = n_rows[f];
       inst_total += (int64_t)L * (4 + n_seq + 4 + (A.n_fam == 4 ? 2 : 0)) + 3;
     }
-    const int n_act = (int)active.size();
-    if (n_act == 0) break;
 
     const double tt1 = tnow();
     // one copy in, one pass of the hot path on device pointers, one copy out
