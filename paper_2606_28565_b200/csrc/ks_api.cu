@@ -260,6 +260,26 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
   const bool lists = routed && pass == 1;
   for (int s0 = 0; s0 < n_specs; s0 += KS_MAX_SPECS_PER_LAUNCH) {
     const int ns = n_specs - s0 < KS_MAX_SPECS_PER_LAUNCH ? n_specs - s0 : KS_MAX_SPECS_PER_LAUNCH;
+    // a small Tier-NONE call with several buckets: one launch for all of them
+    if (tier == KS_TIER_NONE && !lists && !routed && n_batches > 1) {
+      long long total = 0;
+      int nonempty = 0;
+      for (int b = 0; b < n_batches; ++b) { total += batches[b].n; nonempty += batches[b].n > 0; }
+      if (nonempty > 1 && total <= KS_STREAM_SMALL_MAX_ROWS) {
+        KsStreamSmallParams p;
+        memset(&p, 0, sizeof(p));
+        for (int b = 0; b < n_batches; ++b) {
+          p.bk[b] = make_bucket_dev(batches[b], cols[b], outs[b], s0);
+          p.row_begin[b + 1] = p.row_begin[b] + batches[b].n;
+        }
+        p.n_buckets = n_batches;
+        p.n_specs = ns;
+        for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
+        KS_CUDA(c, ks_launch_stream_small(p, c->stream));
+        c->launches += 1;
+        continue;
+      }
+    }
     for (int b = 0; b < n_batches; ++b) {               // streaming kernels: Tier NONE / B, and Eq. 3 rows under any tier
       const bool ar = batches[b].family == KS_FAM_ALLREDUCE;
       if (ar && lists) continue;                        // Eq. 3 rows were finished by pass 1

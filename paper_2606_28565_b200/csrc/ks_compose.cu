@@ -84,6 +84,30 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
     }
   }
   if (used > kCapFloats) staged = false;                          // very long steps: straight from global
+  // Multiplicities (shared by all specs) ride in the same cp.async group behind the latencies when they fit:
+  // a chunk then costs one trip to memory for all buckets instead of one per bucket inside the reduction —
+  // which matters when the arrays live in pinned host memory (the simulation loop reads its arena in place).
+  int mbase[NB], mlen[NB], m0[NB];
+  bool mstaged = MULT && staged;
+  int* smult = reinterpret_cast<int*>(sdata + ((used + 3) & ~3));
+  int mused = 0;
+  if (MULT) {
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      mbase[b] = 0; mlen[b] = 0; m0[b] = 0;
+      if (b < p.n_batches && p.mult[b] != nullptr) {
+        m0[b] = offs[b][0] & ~3;
+        int m1 = (offs[b][kS] + 3) & ~3;
+        const int tot = (int)(p.spec_stride[b] & ~3ll);
+        if (m1 > tot) m1 = tot;
+        if (m1 < offs[b][kS] || (reinterpret_cast<uintptr_t>(p.mult[b]) & 15u) != 0) mstaged = false;
+        mlen[b] = m1 - m0[b];
+        mbase[b] = mused - m0[b];
+        mused += mlen[b];
+      }
+    }
+    if (((used + 3) & ~3) + mused > kCapFloats) mstaged = false;
+  }
   if (staged) {
     int base = 0;
 #pragma unroll
@@ -92,6 +116,16 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
         const float* __restrict__ src = p.lat[b] + a0[b];
         for (int i = tid * 4; i < len[b]; i += kThreads * 4) ks_cp_async16(sdata + base + i, src + i);
         base += len[b];
+      }
+    }
+    if (MULT && mstaged) {
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        if (b < p.n_batches && p.mult[b] != nullptr) {
+          const int32_t* __restrict__ src = p.mult[b] + m0[b];
+          int* dst = smult + mbase[b] + m0[b];
+          for (int i = tid * 4; i < mlen[b]; i += kThreads * 4) ks_cp_async16(dst + i, src + i);
+        }
       }
     }
     ks_cp_async_commit();
@@ -146,20 +180,22 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
           if (MULT && p.mult[b] != nullptr) {
             // layer-homogeneous form: a row stands for m_k identical kernels; the
             // multiplicities are read from global memory (they are shared by all specs)
-            const int32_t* __restrict__ mA = p.mult[b] + begA + lane;
-            const int32_t* __restrict__ mB = p.mult[b] + begB + lane;
+            // multiplicities of rows begA.. / begB..: the staged copy (shared memory) or the global array
+            const int32_t* mrow = (STAGED && mstaged) ? smult + mbase[b] : p.mult[b];
+            const int32_t* mA = mrow + begA + lane;
+            const int32_t* mB = mrow + begB + lane;
             int ka = 0, kb = 0;
             float pa = 0.0f, pb = 0.0f;
             const float xs[5] = {x0, x1, x2, x3, x4}, ys[5] = {y0, y1, y2, y3, y4};
 #pragma unroll
             for (int r = 0; r < 5; ++r) {
-              const int ma = 32 * r < mA_n(nA, lane) ? __ldg(mA + 32 * r) : 0;
-              const int mb = 32 * r < mA_n(nB, lane) ? __ldg(mB + 32 * r) : 0;
+              const int ma = 32 * r < mA_n(nA, lane) ? mA[32 * r] : 0;
+              const int mb = 32 * r < mA_n(nB, lane) ? mB[32 * r] : 0;
               pa = fmaf((float)ma, xs[r], pa); ka += ma;
               pb = fmaf((float)mb, ys[r], pb); kb += mb;
             }
-            for (int k = lane + 160; k < nA; k += 32) { const int m = __ldg(p.mult[b] + begA + k); pa = fmaf((float)m, (sA - lane)[k], pa); ka += m; }
-            for (int k = lane + 160; k < nB; k += 32) { const int m = __ldg(p.mult[b] + begB + k); pb = fmaf((float)m, (sB - lane)[k], pb); kb += m; }
+            for (int k = lane + 160; k < nA; k += 32) { const int m = mrow[begA + k]; pa = fmaf((float)m, (sA - lane)[k], pa); ka += m; }
+            for (int k = lane + 160; k < nB; k += 32) { const int m = mrow[begB + k]; pb = fmaf((float)m, (sB - lane)[k], pb); kb += m; }
             accA += pa; accB += pb;
             cntA += ka; cntB += kb;                   // per-lane partial launch counts, summed with the shuffle tree below
           } else {

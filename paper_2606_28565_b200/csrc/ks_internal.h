@@ -24,6 +24,17 @@ struct KsStreamParams {
 };
 cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st);
 
+// Small Tier-NONE calls (the closed simulation loop prices a few thousand rows per pass): all buckets in
+// ONE launch, a thread per row.  Same per-row device functions as the streaming kernel, so the same bits.
+#define KS_STREAM_SMALL_MAX_ROWS 32768
+struct KsStreamSmallParams {
+  KsBucketDev bk[KS_MAX_BATCHES];
+  int32_t row_begin[KS_MAX_BATCHES + 1];   // prefix of the buckets' row counts
+  int32_t n_buckets, n_specs, pad;
+  KsSpecTable specs;
+};
+cudaError_t ks_launch_stream_small(const KsStreamSmallParams& p, cudaStream_t st);
+
 // ---- Tier-A MLP head kernel: ks_mlp.cu
 #define KS_MLP_MAX_BUCKETS 4
 struct KsHeadDev {

@@ -291,6 +291,55 @@ cudaError_t launch_t(const KsStreamParams& p, int num_sms, cudaStream_t st) {
 
 }  // namespace
 
+namespace {
+
+template <int FAM, int NC>
+KS_DEV void small_row(const KsStreamSmallParams& p, const KsBucketDev& bk, const int i) {
+  int v[NC];
+#pragma unroll
+  for (int c = 0; c < NC; ++c)
+    v[c] = bk.col_f32 ? __float2int_rn(__ldg(static_cast<const float*>(bk.cols[c]) + i))
+                      : __ldg(static_cast<const int*>(bk.cols[c]) + i);
+  for (int s = 0; s < p.n_specs; ++s) {
+    const KsSpecDev& sp = p.specs.s[s];
+    const KsWork w = ks_decode<FAM>(v, bk, sp);
+    const KsRoof r = ks_roofline(w, sp);
+    float tr = r.t_roof, t = fmaxf(r.t_roof, sp.t0);            // Eq. 2 with eta = 1: floor after eta
+    if (FAM == KS_FAM_ALLREDUCE) tr = t = ks_allreduce(v, sp);  // Eq. 3 as it stands
+    const long long o = (long long)s * bk.n + i;
+    bk.lat[o] = t;
+    if (bk.tiles) bk.tiles[o] = (int)w.B;
+    if (bk.waves) bk.waves[o] = (int)r.W;
+    if (bk.troof) bk.troof[o] = tr;
+  }
+}
+
+__global__ void __launch_bounds__(256) ks_stream_small_kernel(const __grid_constant__ KsStreamSmallParams p) {
+  ks_launch_dependents();
+  const int g = blockIdx.x * 256 + threadIdx.x;
+  if (g >= p.row_begin[p.n_buckets]) return;
+  int b = 0;
+  while (g >= p.row_begin[b + 1]) ++b;
+  const KsBucketDev& bk = p.bk[b];
+  const int i = g - p.row_begin[b];
+  switch (bk.family) {
+    case KS_FAM_GEMM: small_row<KS_FAM_GEMM, 3>(p, bk, i); break;
+    case KS_FAM_GROUPED_GEMM: small_row<KS_FAM_GROUPED_GEMM, 10>(p, bk, i); break;
+    case KS_FAM_ATTN: small_row<KS_FAM_ATTN, 3>(p, bk, i); break;
+    case KS_FAM_ELEMWISE: small_row<KS_FAM_ELEMWISE, 2>(p, bk, i); break;
+    default: small_row<KS_FAM_ALLREDUCE, 2>(p, bk, i); break;
+  }
+}
+
+}  // namespace
+
+cudaError_t ks_launch_stream_small(const KsStreamSmallParams& p, cudaStream_t st) {
+  const int n = p.row_begin[p.n_buckets];
+  if (n <= 0) return cudaSuccess;
+  ks_stream_small_kernel<<<(n + 255) / 256, 256, 0, st>>>(p);
+  return cudaGetLastError();
+}
+
 cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st) {
   if (p.tier == KS_TIER_BOUNDED) return launch_t<KS_TIER_BOUNDED>(p, num_sms, st);
   return p.tier == KS_TIER_B ? launch_t<KS_TIER_B>(p, num_sms, st) : launch_t<KS_TIER_NONE>(p, num_sms, st);
