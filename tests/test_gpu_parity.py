@@ -99,6 +99,30 @@ def test_ragged_tails_and_misaligned_spec_stride(ks, n):
     run_and_check(ks, w, TOL_MLP, tier=W.TIER_A)
 
 
+def test_small_multi_bucket_call_equals_per_bucket_calls(ks):
+    # a Tier-NONE call with several buckets and <= 32768 rows takes the one-launch thread-per-row kernel; the same
+    # buckets one call each take the streaming kernel: same device functions, same bits (incl. Eq. 3 rows, fp32 columns)
+    B, D = ks
+    w = W.config4(n_steps=40, tp=4, n_layers=4)
+    w.specs = [W.spec_gb200(), W.spec_gb200(n_sm=96, peak_bw=3e12, ar_beta_eff=4e11)]
+    assert len(w.buckets) == 4 and sum(b.n for b in w.buckets) <= 32768
+    ctx = B.Context(0)
+    try:
+        launches0 = ctx.launch_count()
+        together = D.predict(ctx, w, tier=W.TIER_NONE)
+        assert ctx.launch_count() - launches0 == 1
+        for i, b in enumerate(w.buckets):
+            one = W.Workload("one", [b], w.specs, W.TIER_NONE)
+            alone = D.predict(ctx, one, tier=W.TIER_NONE)[0]
+            for k in ("lat", "tiles", "waves", "troof"):
+                assert np.array_equal(together[i][k], alone[k]), (i, k)
+    finally:
+        ctx.close()
+    o = oracle_all(w, W.TIER_NONE)
+    for i, (gi, oi) in enumerate(zip(together, o)):
+        check_bucket(gi, oi, TOL_F32, what=f"small call / bucket {i}")
+
+
 # ------------------------------------------------------------------ Tier B (S4b)
 def test_tier_b_parity(ks):
     errs = run_and_check(ks, W.config3(n=60001), TOL_F32)
