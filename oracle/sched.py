@@ -1,7 +1,7 @@
 """CPU oracle of the serving scheduler and the closed simulation loop.
 
 TEST INFRASTRUCTURE ONLY (same rules as oracle.py): imported by tests/ and bench.py's oracle legs, never
-by the product package; shares no code with the C++ scheduler in ``csrc/ks_sched.cpp``.
+by the product package; shares no code with the C++ scheduler in ``csrc/ks_sched.cu``.
 
 What it follows, in the paper's order:
 
@@ -16,8 +16,11 @@ What it follows, in the paper's order:
 * PAPER.md:231  t_gpu = L t_layer + t_lm_head + t_embed  (one layer's kernels with multiplicity L).
 * PAPER.md:159  the completion event of a step is scheduled at now + t_step.
 
-The paper gives the loop in one sentence; the precise rules below are DESIGN.md reading Q18 (prefix
-caching, the second half of NEXT-4, is not modelled).  Plain Python loops, one request at a time.
+* PAPER.md:247  content-hashed KV cache in two tiers (volatile GPU tier, persistent disk tier): a prefix
+  hit reuses cached blocks so only the uncached suffix is recomputed.
+
+The paper gives the loop in one sentence and the cache in two; the precise rules below are DESIGN.md
+readings Q18 (scheduler) and Q19 (prefix cache).  Plain Python loops, one request at a time.
 """
 from __future__ import annotations
 
