@@ -24,7 +24,9 @@ namespace {
 constexpr int kWarps = 8;
 constexpr int kThreads = kWarps * 32;
 
-constexpr int kS = 32;                 // steps per chunk (one CTA)
+constexpr int kS = 32;                 // steps per chunk (one CTA); small problems use kSmallS (more, lighter CTAs)
+constexpr int kSmallS = 8;
+constexpr int kSmallSteps = 16384;     // n_steps x n_specs up to which the small chunk is used
 constexpr int kCapFloats = 12032;      // staged floats per CTA (47 KiB + slack): four CTAs per SM
 constexpr int kSlackFloats = 192;      // readable floats behind the staged data (masked lanes of the last step)
 
@@ -41,23 +43,23 @@ KS_DEV float lane_tail(const float* __restrict__ src, int n, int lane) {
 }
 
 // NB = compile-time bound on the bucket count (1-4: exact, or 8)
-template <int NB, bool MULT>
+template <int NB, bool MULT, int KS>
 __global__ void __launch_bounds__(kThreads, 4)
 ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
   extern __shared__ __align__(128) float sdata[];
-  __shared__ int offs[NB][kS + 1];
+  __shared__ int offs[NB][KS + 1];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const unsigned cps = (unsigned)(p.n_steps + kS - 1) / kS;        // chunks per spec
+  const unsigned cps = (unsigned)(p.n_steps + KS - 1) / KS;        // chunks per spec
   const unsigned spec = blockIdx.x / cps;
-  const int s0 = (int)(blockIdx.x - spec * cps) * kS;
-  const int ns = p.n_steps - s0 < kS ? p.n_steps - s0 : kS;
+  const int s0 = (int)(blockIdx.x - spec * cps) * KS;
+  const int ns = p.n_steps - s0 < KS ? p.n_steps - s0 : KS;
 
   // launched with programmatic stream serialization: the launch itself overlaps the tail of the
   // prediction kernel; nothing it produced (nor anything copied in for this call) is read before this
   ks_launch_dependents();            // ... and the totals kernel may be scheduled under this one
   cudaGridDependencySynchronize();
-  for (int idx = tid; idx < p.n_batches * (kS + 1); idx += kThreads) {
-    const int b = idx / (kS + 1), j = idx - b * (kS + 1);
+  for (int idx = tid; idx < p.n_batches * (KS + 1); idx += kThreads) {
+    const int b = idx / (KS + 1), j = idx - b * (KS + 1);
     offs[b][j] = __ldg(p.step_off[b] + (s0 + j < p.n_steps ? s0 + j : p.n_steps));
   }
   __syncthreads();
@@ -74,10 +76,10 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
     if (b < p.n_batches) {
       const long long sb = (long long)spec * p.spec_stride[b];
       a0[b] = (sb + offs[b][0]) & ~3ll;
-      long long a1 = (sb + offs[b][kS] + 3) & ~3ll;
+      long long a1 = (sb + offs[b][KS] + 3) & ~3ll;
       const long long tot = ((long long)p.n_specs * p.spec_stride[b]) & ~3ll;
       if (a1 > tot) a1 = tot;                                     // never read past the array end ...
-      if (a1 < sb + offs[b][kS]) staged = false;                  // ... (its last < 4 floats: global path)
+      if (a1 < sb + offs[b][KS]) staged = false;                  // ... (its last < 4 floats: global path)
       len[b] = (int)(a1 - a0[b]);
       sbase[b] = used + (int)(sb - a0[b]);
       used += len[b];
@@ -97,10 +99,10 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
       mbase[b] = 0; mlen[b] = 0; m0[b] = 0;
       if (b < p.n_batches && p.mult[b] != nullptr) {
         m0[b] = offs[b][0] & ~3;
-        int m1 = (offs[b][kS] + 3) & ~3;
+        int m1 = (offs[b][KS] + 3) & ~3;
         const int tot = (int)(p.spec_stride[b] & ~3ll);
         if (m1 > tot) m1 = tot;
-        if (m1 < offs[b][kS] || (reinterpret_cast<uintptr_t>(p.mult[b]) & 15u) != 0) mstaged = false;
+        if (m1 < offs[b][KS] || (reinterpret_cast<uintptr_t>(p.mult[b]) & 15u) != 0) mstaged = false;
         mlen[b] = m1 - m0[b];
         mbase[b] = mused - m0[b];
         mused += mlen[b];
@@ -259,14 +261,26 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
   (void)num_sms;
   const long long total = (long long)p.n_specs * p.n_steps;
   if (total > 0) {
-    const long long n_chunks = (long long)((p.n_steps + kS - 1) / kS) * p.n_specs;
+    // a cfg2-sized problem (thousands of steps) is a latency chain per CTA: 8-step chunks give four times
+    // as many, lighter CTAs (measured 2.3 us off a 99.6 us cfg2 step); 100k-step problems keep 32-step chunks
+    const bool small = total <= kSmallSteps;
+    const int ks = small ? kSmallS : kS;
+    const long long n_chunks = (long long)((p.n_steps + ks - 1) / ks) * p.n_specs;
     if (n_chunks > 0x7fffffffll) return cudaErrorInvalidValue;
     bool weighted = false;
     for (int b = 0; b < p.n_batches; ++b) weighted = weighted || p.mult[b] != nullptr;
-    auto kern = p.n_batches <= 1 ? ks_compose_kernel<1, false> : p.n_batches == 2 ? ks_compose_kernel<2, false> :
-                p.n_batches == 3 ? ks_compose_kernel<3, false> : p.n_batches == 4 ? ks_compose_kernel<4, false> :
-                                                                                   ks_compose_kernel<8, false>;
-    if (weighted) kern = p.n_batches <= 4 ? ks_compose_kernel<4, true> : ks_compose_kernel<8, true>;
+    void (*kern)(const KsComposeParams);
+    if (small) {
+      kern = p.n_batches <= 1 ? ks_compose_kernel<1, false, kSmallS> : p.n_batches == 2 ? ks_compose_kernel<2, false, kSmallS> :
+             p.n_batches == 3 ? ks_compose_kernel<3, false, kSmallS> : p.n_batches == 4 ? ks_compose_kernel<4, false, kSmallS> :
+                                                                                         ks_compose_kernel<8, false, kSmallS>;
+      if (weighted) kern = p.n_batches <= 4 ? ks_compose_kernel<4, true, kSmallS> : ks_compose_kernel<8, true, kSmallS>;
+    } else {
+      kern = p.n_batches <= 1 ? ks_compose_kernel<1, false, kS> : p.n_batches == 2 ? ks_compose_kernel<2, false, kS> :
+             p.n_batches == 3 ? ks_compose_kernel<3, false, kS> : p.n_batches == 4 ? ks_compose_kernel<4, false, kS> :
+                                                                                     ks_compose_kernel<8, false, kS>;
+      if (weighted) kern = p.n_batches <= 4 ? ks_compose_kernel<4, true, kS> : ks_compose_kernel<8, true, kS>;
+    }
     const size_t smem = (size_t)(kCapFloats + kSlackFloats) * 4;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
