@@ -283,6 +283,11 @@ class Model:
     tp: int = 1
 
 
+def shard(x: int, tp: int) -> int:
+    """Per-GPU share of a dimension split tp ways (ceil; a dimension smaller than tp is replicated)."""
+    return -(-int(x) // max(int(tp), 1))
+
+
 def step_rows(batch: Sequence[Tuple[int, int, int]], m: Model):
     """Batch descriptor -> kernel rows of the step, layer-homogeneous form.
 
@@ -293,11 +298,16 @@ def step_rows(batch: Sequence[Tuple[int, int, int]], m: Model):
     T = sum(n for _, n, _ in batch)          # dense kernels run over the concatenated tokens
     n_seq = len(batch)                       # one logits row per scheduled request
     L = m.n_layers
-    qkv_n = (m.hq + 2 * m.hkv) * m.head_dim
-    gemm = ([[T, qkv_n, m.hidden], [T, m.hidden, m.hidden], [T, 2 * m.ffn, m.hidden], [T, m.hidden, m.ffn],
-             [n_seq, m.vocab, m.hidden]], [L, L, L, L, 1])
-    elem = ([[T * m.hidden, 4], [T * m.hidden, 0], [T * (m.hq + m.hkv) * m.head_dim, 2],
-             [T * 2 * m.hkv * m.head_dim, 3], [T * m.ffn, 1], [T * m.hidden, 0]], [1, L, L, L, L, 1])
+    # Tensor parallelism ("partial activations across the P shards"; Q20): every GPU holds
+    # ceil(1/P) of the attention heads, of the FFN columns and of the vocabulary.  QKV and Gate-Up are split
+    # along N, O and Down along K; norms and the embedding run on the full hidden size on every GPU.
+    hq_p, hkv_p = shard(m.hq, m.tp), shard(m.hkv, m.tp)
+    ffn_p, vocab_p = shard(m.ffn, m.tp), shard(m.vocab, m.tp)
+    qkv_n = (hq_p + 2 * hkv_p) * m.head_dim
+    gemm = ([[T, qkv_n, m.hidden], [T, m.hidden, hq_p * m.head_dim], [T, 2 * ffn_p, m.hidden], [T, m.hidden, ffn_p],
+             [n_seq, vocab_p, m.hidden]], [L, L, L, L, 1])
+    elem = ([[T * m.hidden, 4], [T * m.hidden, 0], [T * (hq_p + hkv_p) * m.head_dim, 2],
+             [T * 2 * hkv_p * m.head_dim, 3], [T * ffn_p, 1], [T * m.hidden, 0]], [1, L, L, L, L, 1])
     # attention per request: a decode (q = 1) over its cached context, a prefill chunk over its cached
     # history plus its own causal triangle (the family's pair count handles q x hist + triangle)
     attn = ([[1, n_new, hist + n_new] for _, n_new, hist in batch], [L] * n_seq)
@@ -354,7 +364,8 @@ def price_steps(batches: Sequence[Sequence[Tuple[int, int, int]]], m: Model, spe
     for f in fams:
         a = np.asarray(cols[f], np.int64).reshape(len(cols[f]), -1)
         bk = W.Bucket(f, [np.ascontiguousarray(a[:, j]) for j in range(a.shape[1])], dtype_bytes=m.dtype_bytes,
-                      hq=m.hq if f == 2 else 0, hkv=m.hkv if f == 2 else 0, head_dim=m.head_dim if f == 2 else 0)
+                      hq=shard(m.hq, m.tp) if f == 2 else 0, hkv=shard(m.hkv, m.tp) if f == 2 else 0,
+                      head_dim=m.head_dim if f == 2 else 0)
         head = O.Head(heads[f]) if (heads and f in heads) else None
         grid = O.Grid(grids[f]) if (grids and f in grids) else None
         lats.append(O.predict_bucket(bk, [spec], tier, head=head, grid=grid)["lat"][0])

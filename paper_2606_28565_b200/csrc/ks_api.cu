@@ -460,10 +460,13 @@ ks_status install_head(ks_ctx* c, ks_family family, int n_in, int H, const float
     cudaFree(d1); cudaFree(d2); cudaFree(d3); cudaFree(d4);
     return KS_ENOMEM;
   }
-  KS_CUDA(c, cudaMemcpy(d4, b2, (size_t)H * 4, cudaMemcpyHostToDevice));
-  KS_CUDA(c, cudaMemcpy(d1, i1.data(), i1.size() * 2, cudaMemcpyHostToDevice));
-  KS_CUDA(c, cudaMemcpy(d2, i2.data(), i2.size() * 2, cudaMemcpyHostToDevice));
-  KS_CUDA(c, cudaMemcpy(d3, w3r.data(), (size_t)H * 4, cudaMemcpyHostToDevice));
+  if (cudaMemcpy(d4, b2, (size_t)H * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(d1, i1.data(), i1.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(d2, i2.data(), i2.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(d3, w3r.data(), (size_t)H * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaFree(d1); cudaFree(d2); cudaFree(d3); cudaFree(d4);
+    return cuda_fail(c);
+  }
   hs.loaded = true;
   hs.n_in = n_in;
   hs.h = H;
@@ -524,10 +527,10 @@ ks_status ks_load_bounded_head(ks_ctx* c, ks_family family, int n_in, const floa
                                const float* w_alpha, float b_alpha) {
   if (!c || family < 0 || family >= KS_FAM_COUNT || family == KS_FAM_ALLREDUCE || !w_gamma || !w_alpha) return KS_EINVAL;
   if (n_in <= 0 || !isfinite(b_gamma) || !isfinite(b_alpha)) return KS_EINVAL;
-  for (int i = 0; i < n_in && i < 64; ++i)
+  if (n_in != 8 && n_in != 12 && n_in != 32) return KS_EUNSUPPORTED;    // before the arrays are read: their length is n_in
+  for (int i = 0; i < n_in; ++i)
     if (!isfinite(w_gamma[i]) || !isfinite(w_alpha[i])) return KS_EINVAL;
   if (c->sticky) return KS_ECUDA;
-  if (n_in != 8 && n_in != 12 && n_in != 32) return KS_EUNSUPPORTED;
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read an MLP head being replaced
   HeadState& hs = c->heads[family];
@@ -638,7 +641,8 @@ ks_status compose_device(ks_ctx* c, const float* const* lat, const int32_t* cons
 ks_status validate_compose(const ks_ctx* c, const float* const* lat, const int32_t* const* step_off,
                            const int32_t* batch_n, int n_batches, int n_steps, int n_specs,
                            const ks_step_params* params, const int32_t* cfg_off, int n_cfg, ks_mem_space space,
-                           const float* step_lat, const float* cfg_lat, bool lat_optional) {
+                           const float* step_lat, const float* cfg_lat, bool lat_optional,
+                           const int32_t* const* mult = nullptr) {
   if (!c) return KS_EINVAL;
   if (space != KS_MEM_DEVICE && space != KS_MEM_HOST) return KS_EINVAL;
   if (n_batches < 0 || n_batches > KS_MAX_BATCHES || n_steps < 0 || n_specs < 0 || n_cfg < 0) return KS_EINVAL;
@@ -647,6 +651,9 @@ ks_status validate_compose(const ks_ctx* c, const float* const* lat, const int32
   for (int b = 0; b < n_batches; ++b) {
     if (batch_n[b] < 0 || !step_off[b]) return KS_EINVAL;
     if (!lat_optional && !lat[b] && batch_n[b] > 0) return KS_EINVAL;
+    // device space: the step kernel reads latencies (and multiplicities) with 16-byte loads
+    if (space == KS_MEM_DEVICE && lat && lat[b] && !aligned16(lat[b])) return KS_EINVAL;
+    if (space == KS_MEM_DEVICE && mult && mult[b] && !aligned16(mult[b])) return KS_EINVAL;
     if (space == KS_MEM_HOST && !csr_ok(step_off[b], n_steps, batch_n[b])) return KS_EINVAL;
   }
   if (n_cfg > 0 && (!cfg_off || !cfg_lat)) return KS_EINVAL;
@@ -749,7 +756,7 @@ ks_status ks_compose_steps_weighted(ks_ctx* c, const float* const* latency, cons
                                     int n_steps, int n_specs, const ks_step_params* params, const int32_t* cfg_off,
                                     int n_cfg, ks_mem_space space, float* step_latency, float* cfg_latency) {
   ks_status st = validate_compose(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg,
-                                  space, step_latency, cfg_latency, false);
+                                  space, step_latency, cfg_latency, false, mult);
   if (st != KS_OK) return st;
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
@@ -807,9 +814,10 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   st = validate_compose(c, latency, step_off, batch_n, n_batches, n_steps, n_specs, params, cfg_off, n_cfg, space,
                         step_latency, cfg_latency, true);
   if (st != KS_OK) return st;
-  if (dev && latency)
+  if (dev)
     for (int b = 0; b < n_batches; ++b)
-      if (latency[b] && !aligned16(latency[b])) return KS_EINVAL;
+      if ((latency && latency[b] && !aligned16(latency[b])) || (batches[b].mult && !aligned16(batches[b].mult)))
+        return KS_EINVAL;
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
 

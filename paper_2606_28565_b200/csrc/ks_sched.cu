@@ -435,7 +435,14 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
   ks_status rc = KS_OK;
   int64_t iters = 0, logged = 0, steps = 0, rows_total = 0, inst_total = 0;
   const int L = m.n_layers;
-  const int32_t qkv_n = (m.hq + 2 * m.hkv) * m.head_dim;
+  // Per-GPU shapes under tensor parallelism (the all-reduces "combine partial activations
+  // across the P shards"; Q20): attention heads and FFN columns are split P ways (ceil; KV heads
+  // are replicated once P exceeds their number), QKV / Gate-Up are column-parallel (N / P), O / Down
+  // row-parallel (K / P), the LM head vocabulary-parallel; norms and the embedding see the full hidden size.
+  const int32_t P = m.tp;
+  const int32_t hq_p = (m.hq + P - 1) / P, hkv_p = (m.hkv + P - 1) / P;
+  const int32_t ffn_p = (m.ffn + P - 1) / P, vocab_p = (m.vocab + P - 1) / P;
+  const int32_t qkv_n = (hq_p + 2 * hkv_p) * m.head_dim;
   auto I = [&A](size_t off) { return reinterpret_cast<int32_t*>(A.host + off); };
 
   double t_host = 0, t_enq = 0, t_wait = 0, t_commit = 0;
@@ -479,8 +486,8 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
       {
         int k = n_rows[0];
         const int32_t gM[5] = {T, T, T, T, n_seq};
-        const int32_t gN[5] = {qkv_n, m.hidden, 2 * m.ffn, m.hidden, m.vocab};
-        const int32_t gK[5] = {m.hidden, m.hidden, m.hidden, m.ffn, m.hidden};
+        const int32_t gN[5] = {qkv_n, m.hidden, 2 * ffn_p, m.hidden, vocab_p};
+        const int32_t gK[5] = {m.hidden, hq_p * m.head_dim, m.hidden, ffn_p, m.hidden};
         for (int j = 0; j < 5; ++j, ++k) {
           I(A.col[0][0])[k] = gM[j]; I(A.col[0][1])[k] = gN[j]; I(A.col[0][2])[k] = gK[j];
           I(A.mult[0])[k] = j < 4 ? L : 1;
@@ -497,7 +504,7 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
       }
       {
         int k = n_rows[2];
-        const int32_t width[6] = {m.hidden, m.hidden, (m.hq + m.hkv) * m.head_dim, 2 * m.hkv * m.head_dim, m.ffn, m.hidden};
+        const int32_t width[6] = {m.hidden, m.hidden, (hq_p + hkv_p) * m.head_dim, 2 * hkv_p * m.head_dim, ffn_p, m.hidden};
         const int32_t sub[6] = {4, 0, 2, 3, 1, 0};   // embedding, RMSNorm, RoPE, KV write, SiLU*Mul, final RMSNorm
         const int32_t mu[6] = {1, L, L, L, L, 1};
         for (int j = 0; j < 6; ++j, ++k) {
@@ -525,7 +532,7 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
       b[f].col_dtype = KS_COL_I32;
       b[f].dtype_bytes = m.dtype_bytes;
       b[f].n_cols = n_cols[f];
-      if (fam_id[f] == KS_FAM_ATTN) { b[f].attn_hq = m.hq; b[f].attn_hkv = m.hkv; b[f].attn_head_dim = m.head_dim; }
+      if (fam_id[f] == KS_FAM_ATTN) { b[f].attn_hq = hq_p; b[f].attn_hkv = hkv_p; b[f].attn_head_dim = m.head_dim; }
       for (int c = 0; c < n_cols[f]; ++c) b[f].cols[c] = in_base + A.col[f][c];
       b[f].mult = reinterpret_cast<const int32_t*>(in_base + A.mult[f]);
       offs[f] = reinterpret_cast<const int32_t*>(in_base + A.off[f]);

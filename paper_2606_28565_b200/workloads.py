@@ -300,6 +300,11 @@ HIDDEN, FFN, HQ, HKV, HEAD_DIM, VOCAB, N_LAYERS = 4096, 14336, 32, 8, 128, 13107
 QKV_N = (HQ + 2 * HKV) * HEAD_DIM  # 6144
 
 
+def _tp_shard(x: int, tp: int) -> int:
+    """Per-GPU share of a model dimension split tp ways (ceil; Q20)."""
+    return -(-int(x) // max(int(tp), 1))
+
+
 def _draw_steps(rng, n_steps: int):
     """Continuous-batching step mix: Poisson(64) decodes + chunked prefill (512-token chunks)."""
     n_dec = np.clip(rng.poisson(64.0, size=n_steps), 1, 256).astype(np.int64)
@@ -343,23 +348,25 @@ def config4(n_steps: int = 100_000, seed: int = 3, tier: int = TIER_NONE, n_cfg:
     L = n_layers
     if dedupe:
         return _config4_dedupe(rng, n_dec, chunk, hist, kv_dec, T, L, n_steps, tier, n_cfg, step_params, tp, seed)
+    # per-GPU shapes under tensor parallelism (Q20): heads, FFN columns and vocabulary split tp ways
+    hq, hkv, ffn, vocab = _tp_shard(HQ, tp), _tp_shard(HKV, tp), _tp_shard(FFN, tp), _tp_shard(VOCAB, tp)
     # GEMM bucket: per layer QKV, O, Gate-Up, Down at M=T; then the LM head once per step
-    gN = np.array([QKV_N, HIDDEN, 2 * FFN, HIDDEN] * L + [VOCAB], np.int64)
-    gK = np.array([HIDDEN, HIDDEN, HIDDEN, FFN] * L + [HIDDEN], np.int64)
+    gN = np.array([(hq + 2 * hkv) * HEAD_DIM, HIDDEN, 2 * ffn, HIDDEN] * L + [vocab], np.int64)
+    gK = np.array([HIDDEN, hq * HEAD_DIM, HIDDEN, ffn] * L + [HIDDEN], np.int64)
     per = gN.shape[0]
     gM = np.repeat(T, per).reshape(n_steps, per)
     gM[:, -1] = n_dec + chunk
     gemm = Bucket(FAM_GEMM, _i32(gM.reshape(-1), np.tile(gN, n_steps), np.tile(gK, n_steps)))
     gemm.step_off = _csr(np.full(n_steps, per))
     # elementwise bucket: embedding; per layer RMSNorm, RoPE, KV-write, SiLU*Mul; final norm
-    mult = np.array([HIDDEN] + [HIDDEN, (HQ + HKV) * HEAD_DIM, 2 * HKV * HEAD_DIM, FFN] * L + [HIDDEN], np.int64)
+    mult = np.array([HIDDEN] + [HIDDEN, (hq + hkv) * HEAD_DIM, 2 * hkv * HEAD_DIM, ffn] * L + [HIDDEN], np.int64)
     sub = np.array([SUB_EMBED] + [SUB_RMSNORM, SUB_ROPE, SUB_KV_WRITE, SUB_SILU_MUL] * L + [SUB_RMSNORM], np.int64)
     pe = mult.shape[0]
     ne = (T[:, None] * mult[None, :]).reshape(-1)
     elem = Bucket(FAM_ELEMWISE, _i32(ne, np.tile(sub, n_steps)))
     elem.step_off = _csr(np.full(n_steps, pe))
     B_, q, kv, aoff = _attn_bucket(n_dec, chunk, hist, kv_dec, L)
-    attn = Bucket(FAM_ATTN, _i32(B_, q, kv), hq=HQ, hkv=HKV, head_dim=HEAD_DIM, step_off=aoff)
+    attn = Bucket(FAM_ATTN, _i32(B_, q, kv), hq=hq, hkv=hkv, head_dim=HEAD_DIM, step_off=aoff)
     heads = {}
     if tier == TIER_A:
         hr = _rng(1)  # cfg-2-sized heads, seed 1 (SURVEY.md §8(d) cfg 4b)
@@ -386,18 +393,19 @@ def allreduce_rows(n: int = 6_400_000, seed: int = 5, tp: int = 4) -> Workload:
 
 def _config4_dedupe(rng, n_dec, chunk, hist, kv_dec, T, L, n_steps, tier, n_cfg, step_params, tp, seed):
     i32 = lambda a: np.ascontiguousarray(a, dtype=np.int32)
-    gN = np.array([QKV_N, HIDDEN, 2 * FFN, HIDDEN, VOCAB], np.int64)
-    gK = np.array([HIDDEN, HIDDEN, HIDDEN, FFN, HIDDEN], np.int64)
+    hq, hkv, ffn, vocab = _tp_shard(HQ, tp), _tp_shard(HKV, tp), _tp_shard(FFN, tp), _tp_shard(VOCAB, tp)
+    gN = np.array([(hq + 2 * hkv) * HEAD_DIM, HIDDEN, 2 * ffn, HIDDEN, vocab], np.int64)
+    gK = np.array([HIDDEN, hq * HEAD_DIM, HIDDEN, ffn, HIDDEN], np.int64)
     gM = np.repeat(T, 5).reshape(n_steps, 5)
     gM[:, -1] = n_dec + chunk
     gemm = Bucket(FAM_GEMM, _i32(gM.reshape(-1), np.tile(gN, n_steps), np.tile(gK, n_steps)),
                   step_off=_csr(np.full(n_steps, 5)), mult=i32(np.tile([L, L, L, L, 1], n_steps)))
-    mult_e = np.array([HIDDEN, HIDDEN, (HQ + HKV) * HEAD_DIM, 2 * HKV * HEAD_DIM, FFN, HIDDEN], np.int64)
+    mult_e = np.array([HIDDEN, HIDDEN, (hq + hkv) * HEAD_DIM, 2 * hkv * HEAD_DIM, ffn, HIDDEN], np.int64)
     sub = np.array([SUB_EMBED, SUB_RMSNORM, SUB_ROPE, SUB_KV_WRITE, SUB_SILU_MUL, SUB_RMSNORM], np.int64)
     elem = Bucket(FAM_ELEMWISE, _i32((T[:, None] * mult_e[None, :]).reshape(-1), np.tile(sub, n_steps)),
                   step_off=_csr(np.full(n_steps, 6)), mult=i32(np.tile([1, L, L, L, L, 1], n_steps)))
     B_, q, kv, aoff = _attn_bucket(n_dec, chunk, hist, kv_dec, 1)
-    attn = Bucket(FAM_ATTN, _i32(B_, q, kv), hq=HQ, hkv=HKV, head_dim=HEAD_DIM, step_off=aoff,
+    attn = Bucket(FAM_ATTN, _i32(B_, q, kv), hq=hq, hkv=hkv, head_dim=HEAD_DIM, step_off=aoff,
                   mult=i32(np.full(B_.shape[0], L)))
     buckets = [gemm, attn, elem]
     if tp > 1:

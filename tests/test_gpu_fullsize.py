@@ -75,10 +75,22 @@ def test_cfg2_full_tier_a_and_composition(ks):
     assert rel(step[0], so).max() <= TOL_F32 and rel(tot[0], to).max() <= TOL_F32
 
 
+def check_composition(w, g, step, tot, specs=None):
+    """Step and configuration latencies of ALL steps against the oracle's composer (O.compose: naive segment loops in
+    double, Eq. 4) fed with the GPU's own per-kernel latencies, per spec."""
+    n_cfg = len(w.cfg_off) - 1
+    for s in (range(len(w.specs)) if specs is None else specs):
+        so, to = O.compose([x["lat"][s] for x in g], [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off,
+                           mults=[b.mult for b in w.buckets])
+        assert rel(step[s], so).max() <= TOL_F32, f"{w.name}: step latencies of spec {s}"
+        assert rel(tot[s][:n_cfg], to).max() <= TOL_F32, f"{w.name}: configuration totals of spec {s}"
+
+
 def test_cfg3_full_tier_b(ks):
     w = W.config3()                                   # 4,194,304 grid queries
-    g, _, _ = predict_full(ks, w, aux=True)
+    g, step, tot = predict_full(ks, w, aux=True)
     print("cfg3 full: sampled max rel err", check_sampled(w, g, 4099, TOL_F32))
+    check_composition(w, g, step, tot)                # 16,384 steps, 16 configurations
     t0 = w.specs[0]["t0"]
     for b, gi in zip(w.buckets, g):
         # interpolation never leaves [min, max] of the grid, so on EVERY row
@@ -105,6 +117,14 @@ def test_cfg4_full_tier_none_closed_form(ks):
     assert rel(step[0], want).max() <= TOL_F32
     cfg_ref = np.add.reduceat(want, w.cfg_off[:-1])
     assert rel(tot[0], cfg_ref).max() <= TOL_F32
+    check_composition(w, g, step, tot)                # and against the oracle's own composer
+
+
+def test_cfg4b_full_tier_a(ks):
+    w = W.config4(tier=W.TIER_A)                      # the same 100,000 steps through the Tier-A heads (29.9M rows)
+    g, step, tot = predict_full(ks, w)
+    print("cfg4b full: sampled max rel err", check_sampled(w, g, 50021, TOL_MLP))
+    check_composition(w, g, step, tot)
 
 
 def test_cfg5_full_what_if_sweep(ks):
@@ -117,3 +137,5 @@ def test_cfg5_full_what_if_sweep(ks):
     key = np.stack([c[:200000] for c in b.cols], axis=1)
     _, first, inv = np.unique(key, axis=0, return_index=True, return_inverse=True)
     assert np.array_equal(gi["lat"][:, :200000], gi["lat"][:, first[inv.ravel()]])
+    # the 64-spec x 10.9k-step composition (spec_stride, chunk indexing): every step of every spec
+    check_composition(w, g, step, tot)

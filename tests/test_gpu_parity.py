@@ -602,3 +602,132 @@ def test_layer_homogeneous_steps_match_oracle_and_materialised_steps(ks, tier):
     # L identical kernels summed one by one or taken L times: the same step up to fp32 rounding of the sums
     assert rel_err(step[0], out["full"][1][0]).max() <= 2 * TOL_F32
     assert rel_err(tot[0], out["full"][2][0]).max() <= 2 * TOL_F32
+
+
+# ------------------------------------------------------------------ holes named by the round-1 review
+def grouped_grid_workload(n=20011, routed=False, seed=31):
+    """A grouped-GEMM bucket (cfg5's MoE rows: N, K, m_0..m_7) against a 12 x 5 x 6 grid over (sum m, N, K) with a
+    different span on every axis; about a fifth of the rows lie outside the hull (small or huge token totals)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    T = W._log_uniform_int(rng, 1, 1 << 15, n)                      # tokens routed top-2: sum m = 2 T
+    m = rng.multinomial(2 * T, np.full(8, 1 / 8)).astype(np.int64)
+    N = np.array([4096, 5120, 8192, 14336, 28672], np.int64)[rng.integers(0, 5, n)]
+    K = np.array([2048, 4096, 8192, 14336], np.int64)[rng.integers(0, 4, n)]
+    m[rng.random(n) < 0.01] = 0                                     # a few rows without any token (B = 0)
+    grid = W.make_grid(rng, (3.0, 12.0, 11.0), (14.0, 15.0, 13.9), dims=(12, 5, 6))
+    bk = W.Bucket(W.FAM_GROUPED, W._i32(N, K, *[m[:, e] for e in range(8)]))
+    heads = {W.FAM_GROUPED: W.make_head(rng, 32, 256)} if routed else {}
+    return W.Workload("grouped_grid", [bk], [W.spec_gb200(), W.spec_gb200(n_sm=132, tile_m=64, peak_bw=3.35e12)],
+                      W.TIER_B_ROUTED if routed else W.TIER_B, grids={W.FAM_GROUPED: grid}, heads=heads)
+
+
+def test_tier_b_grouped_gemm_bucket(ks):
+    # the 512-thread Tier-B instance, grid axes (sum m, N, K) and the integer hull test of the grouped family
+    w = grouped_grid_workload()
+    errs = run_and_check(ks, w, TOL_F32)
+    print("grouped-GEMM Tier B max rel err", errs)
+
+
+def test_density_routing_grouped_gemm_bucket(ks):
+    B, D = ks
+    w = grouped_grid_workload(n=9001, routed=True)
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        g = D.predict(ctx, w)
+    finally:
+        ctx.close()
+    o = routed_oracle(w)
+    check_routed(g, o, w.name)
+    frac = float(o[0]["routed"].mean())
+    assert 0.05 < frac < 0.6, frac
+
+
+@pytest.mark.parametrize("n_specs", [65, 130])
+def test_more_specs_than_one_launch_holds(ks, n_specs):
+    # n_specs > 64 is split into launches of <= 64 specs (output offset s0 x n; the routed row list is built once)
+    B, D = ks
+    rng = np.random.Generator(np.random.PCG64(77))
+    specs = W.sweep_specs(rng, n_specs)
+    for k in range(0, n_specs, 7):
+        specs[k]["tile_m"], specs[k]["ctas_per_sm"] = 64, 2
+    rows = [np.arange(0, 3001, 13)]
+    # Tier NONE and Tier A on a cfg2-like mix (three buckets), spec 64 onward is the second launch
+    w = W.config2(n=3001 * 2)
+    w.specs = specs
+    for tier, tol in ((W.TIER_NONE, TOL_F32), (W.TIER_A, TOL_MLP)):
+        ctx = B.Context(0)
+        try:
+            D.load_models(ctx, w)
+            db = D.to_device(w)
+            g = D.predict(ctx, w, dbuckets=db, tier=tier)
+            step, tot = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+        finally:
+            ctx.close()
+        o = oracle_all(w, tier)
+        for i, (gi, oi) in enumerate(zip(g, o)):
+            check_bucket(gi, oi, tol, what=f"{n_specs} specs tier {tier} bucket {i}")
+        for s in (0, 63, 64, n_specs - 1):
+            so, to = O.compose([x["lat"][s] for x in g], [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off)
+            assert rel_err(step[s], so).max() <= TOL_F32 and rel_err(tot[s], to).max() <= TOL_F32
+    # density-routed Tier B
+    w3 = W.config3(n=4001, routed=True)
+    w3.specs = specs
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w3)
+        g = D.predict(ctx, w3)
+    finally:
+        ctx.close()
+    check_routed(g, routed_oracle(w3), f"routed, {n_specs} specs")
+
+
+@pytest.mark.parametrize("s", [1, 4])
+def test_dtype_bytes_one_and_four(ks, s):
+    # the element size s of the modelled kernel (fp8 / fp32 tensors) enters F_mem and feature 11
+    for make, tier, tol in ((lambda: W.config2(n=9001), W.TIER_NONE, TOL_F32), (lambda: W.config2(n=9001), W.TIER_A, TOL_MLP),
+                            (lambda: W.config5(n_rows=9001, n_specs=2, n_layers=4), W.TIER_A, TOL_MLP),
+                            (lambda: W.config3(n=9001), W.TIER_B, TOL_F32)):
+        w = make()
+        for b in w.buckets:
+            b.dtype_bytes = s
+        run_and_check(ks, w, tol, tier=tier)
+    # and it changes the answer: a memory-bound GEMM row moves s/2 times the bytes
+    B, D = ks
+    w = W.config1()
+    ctx = B.Context(0)
+    try:
+        base = D.predict(ctx, w, tier=W.TIER_NONE)[0]["troof"]
+        w.buckets[0].dtype_bytes = s
+        got = D.predict(ctx, w, tier=W.TIER_NONE)[0]["troof"]
+    finally:
+        ctx.close()
+    M = w.buckets[0].cols[0]
+    mem_bound = M <= 16                                                # AI < ridge for these rows
+    assert rel_err(got[0][mem_bound], base[0][mem_bound] * (s / 2)).max() <= 2e-6
+
+
+def test_compose_many_steps_odd_stride_two_specs(ks):
+    # n_steps x n_specs > 16384 takes the 32-step chunks; odd bucket sizes make spec 1's rows start unaligned
+    import torch
+    B, D = ks
+    rng = np.random.default_rng(5)
+    n_steps, ns = 9001, 2
+    ns_rows = [270031, 90007, 13]
+    offs = [np.concatenate([[0], np.sort(rng.integers(0, n + 1, n_steps - 1)), [n]]).astype(np.int32) for n in ns_rows]
+    lat = [rng.uniform(1e-6, 1e-3, (ns, n)).astype(np.float32) for n in ns_rows]
+    cfg = np.array([0, 17, 17, 4000, 9001], np.int32)
+    ctx = B.Context(0)
+    try:
+        dl = [torch.from_numpy(x).cuda() for x in lat]
+        do = [torch.from_numpy(x).cuda() for x in offs]
+        step = torch.empty((ns, n_steps), dtype=torch.float32, device="cuda")
+        tot = torch.empty((ns, 4), dtype=torch.float32, device="cuda")
+        ctx.compose_steps(dl, do, ns_rows, n_steps, ns, W.STEP_PARAMS_HOSTBOUND, torch.from_numpy(cfg).cuda(), 4, step, tot)
+        torch.cuda.synchronize()
+    finally:
+        ctx.close()
+    for s in range(ns):
+        so, to = O.compose([x[s] for x in lat], offs, n_steps, W.STEP_PARAMS_HOSTBOUND, cfg)
+        assert rel_err(step[s].cpu().numpy(), so).max() <= TOL_F32
+        assert np.allclose(tot[s].cpu().numpy(), to, rtol=TOL_F32, atol=0)

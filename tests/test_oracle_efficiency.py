@@ -238,6 +238,33 @@ def test_tier_b_latency_and_axes():
     assert t >= r.t_roof                                                 # eta >= 1 since e <= 1
 
 
+def test_grouped_gemm_grid_axes_are_total_tokens_then_n_then_k():
+    # DESIGN.md Q5: a grouped GEMM's grid coordinates are (sum_e m_e, N, K).  A 5 x 3 x 2 grid whose node (i, j, k)
+    # holds 0.1 + 0.1 i + 0.02 j + 0.3 k, with a different span on every axis: sum m over 2^4..2^8, N over 2^10..2^12,
+    # K over 2^6..2^7.  Queries on nodes name their value; swapping N and K, or taking one expert's tokens for the
+    # total, lands on another node (or off the grid) and fails.
+    val = np.array([[[0.1 + 0.1 * i + 0.02 * j + 0.3 * k for k in range(2)] for j in range(3)] for i in range(5)])
+    g = O.Grid(_grid(val, lo=(4, 10, 6), hi=(8, 12, 7)))
+    for i in range(5):
+        for j in range(3):
+            for k in range(2):
+                tot = 2 ** (4 + i)
+                m = [tot // 2, 0, tot // 4, 0, 0, tot // 8, 0, tot // 8]           # eight experts, three idle
+                assert sum(m) == tot
+                d = O.make_desc(W.FAM_GROUPED, [2 ** (10 + j), 2 ** (6 + k)] + m)
+                _, _, e = O.predict_one(d, SPEC, W.TIER_B, grid=g)
+                assert e == pytest.approx(float(np.float32(val[i, j, k])), rel=1e-12)
+    # between nodes, by hand: sum m = 48 -> coordinate log2(48) - 4 = 1.58496 on axis 0 (cell 1, f = 0.58496);
+    # N = 2^11 (node 1), K = 2^6 (node 0): e = v[1,1,0] + f (v[2,1,0] - v[1,1,0]) = 0.22 + 0.058496
+    d = O.make_desc(W.FAM_GROUPED, [2048, 64, 40, 8, 0, 0, 0, 0, 0, 0])
+    _, _, e = O.predict_one(d, SPEC, W.TIER_B, grid=g)
+    f = math.log2(48) - 5
+    assert e == pytest.approx(float(np.float32(val[1, 1, 0])) * (1 - f) + float(np.float32(val[2, 1, 0])) * f, rel=1e-12)
+    # negative token counts are ignored by the total (like everywhere else in the family)
+    d = O.make_desc(W.FAM_GROUPED, [2048, 64, 40, 8, -7, 0, 0, 0, 0, 0])
+    assert O.predict_one(d, SPEC, W.TIER_B, grid=g)[2] == pytest.approx(e, rel=1e-15)
+
+
 # ------------------------------------------------------------------ floor
 def test_floor_applied_after_eta():
     d = O.make_desc(W.FAM_ELEMWISE, [4096, W.SUB_RMSNORM])

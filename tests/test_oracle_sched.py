@@ -149,10 +149,19 @@ def test_step_rows_follow_the_mixed_step_pricing_rule():
     m = S.Model(n_layers=4, hidden=64, ffn=128, vocab=1000, hq=4, hkv=2, head_dim=16, tp=2)
     rows = S.step_rows([(5, 1, 100), (9, 1, 7), (2, 32, 64)], m)
     T = 34
-    assert rows[0] == ([[T, 128, 64], [T, 64, 64], [T, 256, 64], [T, 64, 128], [3, 1000, 64]], [4, 4, 4, 4, 1])
+    # tp = 2 (Q20): each GPU holds 2 of the 4 query heads, 1 of the 2 KV heads, 64 of the 128
+    # FFN columns and 500 of the 1000 vocabulary rows: QKV N = (2 + 2x1) x 16 = 64, O K = 2 x 16 = 32, Gate-Up
+    # N = 2 x 64, Down K = 64, LM head N = 500; RoPE over (2 + 1) x 16 = 48 and KV write over 2 x 1 x 16 = 32 values
+    # per token; SiLU x Mul over 64; norms and the embedding over the full hidden size
+    assert rows[0] == ([[T, 64, 64], [T, 64, 32], [T, 128, 64], [T, 64, 64], [3, 500, 64]], [4, 4, 4, 4, 1])
     assert rows[2] == ([[1, 1, 101], [1, 1, 8], [1, 32, 96]], [4, 4, 4])      # per request: (B, q, kv = hist + q)
-    assert rows[3] == ([[T * 64, 4], [T * 64, 0], [T * 96, 2], [T * 64, 3], [T * 128, 1], [T * 64, 0]], [1, 4, 4, 4, 4, 1])
+    assert rows[3] == ([[T * 64, 4], [T * 64, 0], [T * 48, 2], [T * 32, 3], [T * 64, 1], [T * 64, 0]], [1, 4, 4, 4, 4, 1])
     assert rows[4] == ([[T * 64 * 2, 2]], [8])                                # two all-reduces per layer
+    # tp = 1 keeps the unsharded shapes; a dimension smaller than tp is replicated (ceil)
+    m1 = S.Model(n_layers=4, hidden=64, ffn=128, vocab=1000, hq=4, hkv=2, head_dim=16, tp=1)
+    assert S.step_rows([(5, 1, 100)], m1)[0][0][:2] == [[1, 128, 64], [1, 64, 64]] and 4 not in S.step_rows([(5, 1, 100)], m1)
+    m4 = S.Model(n_layers=4, hidden=64, ffn=128, vocab=1000, hq=4, hkv=2, head_dim=16, tp=4)
+    assert S.step_rows([(5, 1, 100)], m4)[0][0][0] == [1, (1 + 2 * 1) * 16, 64]   # 1 query head, the KV head replicated
     # kernel launches of the step: n = L (4 GEMM + 3 attention + 4 elementwise + 2 all-reduce) + lm_head + embed + final norm
     assert sum(sum(mm) for _, mm in rows.values()) == 4 * (4 + 3 + 4 + 2) + 3
 
@@ -174,6 +183,32 @@ def test_price_steps_equals_hand_composition():
     body = 32 * layer + one(0, [3, 131072, 4096]) + one(3, [T * 4096, 4]) + one(3, [T * 4096, 0])
     n = 32 * (4 + 3 + 4) + 3
     assert abs(t - (body + n * 4e-6)) < 1e-12
+
+
+def test_price_steps_tp2_equals_hand_composition():
+    # tensor parallel degree 2 (Q20): the per-GPU shapes written out by hand for config 4's
+    # decoder (16 query heads, 4 KV heads, 7168 FFN columns, 65536 vocabulary rows per GPU) plus two ring all-reduces
+    # per layer of S = T x hidden x 2 bytes (Eq. 3), every term priced one descriptor at a time
+    from oracle import oracle as O
+    from paper_2606_28565_b200 import workloads as W
+    m = S.Model(tp=2)
+    spec = W.spec_gb200()
+    batch = [(0, 1, 500), (1, 1, 2000), (2, 512, 1024)]
+    t = S.price_steps([batch], m, spec, 0, W.STEP_PARAMS_CFG4)[0]
+
+    def one(f, v, **kw):
+        return O.predict_one(O.make_desc(f, v, **kw), O.make_spec(spec), 0)[0]
+    T = 514
+    layer = (one(0, [T, 3072, 4096]) + one(0, [T, 4096, 2048]) + one(0, [T, 14336, 4096]) + one(0, [T, 4096, 7168])
+             + sum(one(2, [1, q, h + q], hq=16, hkv=4, d=128) for _, q, h in batch)
+             + one(3, [T * 4096, 0]) + one(3, [T * 20 * 128, 2]) + one(3, [T * 8 * 128, 3]) + one(3, [T * 7168, 1]))
+    ar = 10e-6 + 2.0 * (2 - 1) / 2 * (T * 4096 * 2) / 900e9          # Eq. 3 with the spec's alpha0, beta_eff
+    body = 32 * (layer + 2 * ar) + one(0, [3, 65536, 4096]) + one(3, [T * 4096, 4]) + one(3, [T * 4096, 0])
+    n = 32 * (4 + 3 + 4 + 2) + 3
+    assert abs(t - (body + n * 4e-6)) < 1e-12
+    # and the point of sharding: the per-GPU compute of a TP = 2 step is smaller than the TP = 1 step's
+    t1 = S.price_steps([batch], S.Model(tp=1), spec, 0, W.STEP_PARAMS_CFG4)[0]
+    assert body - 32 * 2 * ar < t1 - (32 * 11 + 3) * 4e-6
 
 
 # ------------------------------------------------------------------ prefix cache (Q19)
