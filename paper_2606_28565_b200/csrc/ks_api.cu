@@ -31,6 +31,7 @@ struct HeadState {
 struct GridState {
   bool loaded = false;
   KsGridDev dev;
+  KsTierBGrid tb;            // the same grid in the form the GEMM/attention Tier-B kernel takes (ks_tierb.cu)
   float* values = nullptr;
 };
 
@@ -280,7 +281,40 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
         continue;
       }
     }
+    // Tier B, GEMM and attention buckets: ONE persistent launch for all of them (per column type)
+    bool tb_done[KS_MAX_BATCHES] = {false};
+    if (tier == KS_TIER_B) {
+      for (int f32 = 0; f32 < 2; ++f32) {
+        int b0 = 0;
+        while (b0 < n_batches) {
+          KsTierBParams p;
+          memset(&p, 0, sizeof(p));
+          int nb = 0;
+          for (; b0 < n_batches && nb < KS_TIERB_MAX_BUCKETS; ++b0) {
+            const ks_desc_batch& k = batches[b0];
+            if ((k.family != KS_FAM_GEMM && k.family != KS_FAM_ATTN) || (k.col_dtype == KS_COL_F32) != (f32 == 1)) continue;
+            tb_done[b0] = true;
+            if (k.n == 0) continue;
+            p.bk[nb] = make_bucket_dev(k, cols[b0], outs[b0], s0);
+            p.grid[nb] = c->grids[k.family].tb;
+            if (routed && s0 == 0) {                      // the hull test depends on the row only: list it once
+              KS_CUDA(c, cudaMemsetAsync(rb[b0].count, 0, 4, c->stream));
+              p.grid[nb].route_idx = rb[b0].idx;
+              p.grid[nb].route_count = rb[b0].count;
+            }
+            ++nb;
+          }
+          if (nb == 0) continue;
+          p.n_buckets = nb;
+          p.n_specs = ns;
+          for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
+          KS_CUDA(c, ks_launch_tierb(p, c->num_sms, c->stream));
+          c->launches += 1;
+        }
+      }
+    }
     for (int b = 0; b < n_batches; ++b) {               // streaming kernels: Tier NONE / B, and Eq. 3 rows under any tier
+      if (tb_done[b]) continue;
       const bool ar = batches[b].family == KS_FAM_ALLREDUCE;
       if (ar && lists) continue;                        // Eq. 3 rows were finished by pass 1
       const bool bnd = tier == KS_TIER_A && !ar && c->heads[batches[b].family].bounded;
@@ -554,16 +588,23 @@ ks_status ks_load_grid(ks_ctx* c, ks_family family, const int32_t dims[3], const
   for (int a = 0; a < 3; ++a) {
     if (dims[a] < 1 || dims[a] > KS_MAX_GRID_NODES) return KS_EINVAL;
     if (dims[a] > 1 && !(hi_log2[a] > lo_log2[a])) return KS_EINVAL;
+    // axis values are int32: their log2 lies in [0, 31]; the kernels' exponent arithmetic is exact for |lo| <= 64
+    if (dims[a] > 1 && !(lo_log2[a] >= -64.0f && hi_log2[a] <= 64.0f)) return KS_EINVAL;
     nodes *= dims[a];
   }
   if (nodes > KS_MAX_GRID_NODES) return KS_EINVAL;
+  for (long long i = 0; i < nodes; ++i)
+    if (!isfinite(values[i])) return KS_EINVAL;
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));
   GridState& g = c->grids[family];
   cudaFree(g.values);
   g = GridState();
-  const size_t padded = ((size_t)nodes + 3) & ~(size_t)3;    // bulk copies move multiples of 16 bytes
+  // bulk copies move multiples of 16 bytes.  Behind the last node: one plane + one row + two floats of zeros (the
+  // Tier-B kernel reads the corners one node past an axis' end with weight exactly 0; they must be finite)
+  const size_t tail = (size_t)(dims[0] > 1 ? dims[1] * dims[2] : 0) + (size_t)(dims[1] > 1 ? dims[2] : 0) + 2;
+  const size_t padded = ((size_t)nodes + tail + 3) & ~(size_t)3;
   float* d = nullptr;
   if (cudaMalloc(reinterpret_cast<void**>(&d), padded * 4) != cudaSuccess) { cudaGetLastError(); return KS_ENOMEM; }
   KS_CUDA(c, cudaMemset(d, 0, padded * 4));
@@ -586,6 +627,21 @@ ks_status ks_load_grid(ks_ctx* c, ks_family family, const int32_t dims[3], const
   }
   g.dev.route_idx = nullptr;
   g.dev.route_count = nullptr;
+  memset(&g.tb, 0, sizeof(g.tb));
+  g.tb.values = d;
+  g.tb.bytes = (int32_t)(padded * 4);
+  for (int a = 0; a < 3; ++a) {
+    const bool flat = dims[a] <= 1;
+    const double lo = flat ? 0.0 : (double)lo_log2[a];
+    const double lor = nearbyint(lo);                    // the integer part of lo leaves with the exponent, exactly
+    g.tb.stride4[a] = g.dev.stride[a] * 4;
+    g.tb.nkc[a] = (float)-(8388608.0 + 127.0 + lor);
+    g.tb.scale[a] = g.dev.scale[a];
+    g.tb.nrs[a] = flat ? 0.0f : (float)(-(lo - lor) * (double)g.dev.scale[a]);
+    g.tb.top[a] = (float)(dims[a] - 1);
+    g.tb.vmin[a] = g.dev.vmin[a];
+    g.tb.vmax[a] = g.dev.vmax[a];
+  }
   g.values = d;
   g.loaded = true;
   return KS_OK;

@@ -24,6 +24,31 @@ struct KsStreamParams {
 };
 cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st);
 
+// ---- Tier B, GEMM and attention families, all buckets of a call in one persistent launch: ks_tierb.cu
+#define KS_TIERB_MAX_BUCKETS 4
+struct KsTierBGrid {
+  const float* values;     // device; `bytes` bytes (a multiple of 16): the nodes, then stride[0] + stride[1] + 2 zero floats
+                           // (the corners one node past the last node are read with weight 0)
+  int32_t bytes;
+  int32_t stride4[3];      // byte strides; 0 for a flat (1-node) axis
+  float nkc[3];            // -(2^23 + 127 + round(lo)): (2^23 + biased exponent) + nkc is exact
+  float nrs[3];            // -(lo - round(lo)) * scale: the remainder of lo, folded into the coordinate's FMA
+  float scale[3];          // (dims-1)/(hi-lo); 0 for a flat axis
+  float top[3];            // dims - 1
+  int32_t vmin[3], vmax[3];   // the hull on integers (Q16)
+  int32_t* route_idx;      // KS_TIER_B_ROUTED pass 1 (nullptr = plain Tier B)
+  int32_t* route_count;
+};
+struct KsTierBParams {
+  KsBucketDev bk[KS_TIERB_MAX_BUCKETS];
+  KsTierBGrid grid[KS_TIERB_MAX_BUCKETS];
+  int32_t tile_begin[KS_TIERB_MAX_BUCKETS + 1];   // filled by the launcher: prefix of the buckets' 4-row x NT tiles
+  int32_t cta_begin[KS_TIERB_MAX_BUCKETS + 1];    // ... and of the CTAs that serve them
+  int32_t n_buckets, n_specs, pad;
+  KsSpecTable specs;
+};
+cudaError_t ks_launch_tierb(const KsTierBParams& p, int num_sms, cudaStream_t st);
+
 // Small Tier-NONE calls (the closed simulation loop prices a few thousand rows per pass): all buckets in
 // ONE launch, a thread per row.  Same per-row device functions as the streaming kernel, so the same bits.
 #define KS_STREAM_SMALL_MAX_ROWS 32768
