@@ -26,7 +26,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 from paper_2606_28565_b200 import sharding as S  # noqa: E402
-from paper_2606_28565_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 
 METRIC = "kernel_latency_predictions_per_sec"
 UNIT = "predictions/s"
@@ -129,7 +129,7 @@ def oracle_sample_rate(w, stride: int, models=None):
     t0 = time.perf_counter()
     lats, offs, n = [], [], 0
     for b, r in zip(w.buckets, rows):
-        out = O.predict_bucket(b, w.specs, w.tier, head=heads.get(b.family), grid=grids.get(b.family), rows=r)
+        out = O.predict_bucket(b, w.specs, w.tier, head=heads.get(b.slot), grid=grids.get(b.slot), rows=r)
         lats.append(out["lat"][0])
         offs.append(np.searchsorted(r, b.step_off).astype(np.int64))   # sampled rows keep their step
         n += len(r) * len(w.specs)

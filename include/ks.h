@@ -49,6 +49,24 @@ typedef enum { KS_OK = 0, KS_EINVAL = 1, KS_ENOMEM = 2, KS_ECUDA = 3, KS_ESTATE 
 typedef enum { KS_FAM_GEMM = 0, KS_FAM_GROUPED_GEMM = 1, KS_FAM_ATTN = 2, KS_FAM_ELEMWISE = 3, KS_FAM_ALLREDUCE = 4,
                KS_FAM_COUNT = 5 } ks_family;
 typedef enum { KS_TIER_NONE = 0, KS_TIER_A = 1, KS_TIER_B = 2, KS_TIER_B_ROUTED = 3 } ks_tier;
+/* Efficiency-model slots.  ks_family says how a bucket's rows are DECODED (which columns, which FLOP/byte/tile
+ * formulas); the model slot says which learned head / measured grid PRICES them.  The paper learns eta
+ * "separately for each kernel family f.  This includes GEMM, the LM head, attention prefill and decode, and the
+ * elementwise and memory kernels" (the families of Tables 2 and 4), which
+ * is finer than the decode enum: an LM-head bucket decodes as KS_FAM_GEMM and prefill and decode attention both as
+ * KS_FAM_ATTN.  A slot is just an index in [0, KS_MAX_MODEL_SLOTS); the names below are a convention.  Slots 0-4
+ * coincide with ks_family, so callers that keep one model per decode family use slot = family
+ * (ks_desc_batch.model_slot = KS_SLOT_FAMILY). */
+typedef enum { KS_SLOT_FAMILY = -1,   /* in ks_desc_batch.model_slot: the slot numbered like the bucket's family */
+               KS_SLOT_GEMM = 0, KS_SLOT_GROUPED_GEMM = 1, KS_SLOT_ATTN = 2, KS_SLOT_ELEMWISE = 3, KS_SLOT_ALLREDUCE = 4,
+               KS_SLOT_LM_HEAD = 5, KS_SLOT_ATTN_PREFILL = 6, KS_SLOT_ATTN_DECODE = 7, KS_SLOT_RMSNORM = 8,
+               KS_SLOT_SILU_MUL = 9, KS_SLOT_ROPE = 10, KS_SLOT_KV_WRITE = 11, KS_SLOT_EMBEDDING = 12,
+               KS_SLOT_RESIDUAL_ADD = 13, KS_MAX_MODEL_SLOTS = 16 } ks_model_slot;
+/* What an MLP head's scalar output z means (ks_set_head_output). */
+typedef enum { KS_HEAD_UTILISATION = 0,   /* e = sigmoid(z), eta = 1 / e (BASELINE.json "sigmoid out"; Q3) */
+               KS_HEAD_LOG_ETA = 1        /* z = log eta: eta = exp(max(z, 0)) >= 1 (PAPER.md:193 "eta >= 1", :199 heads
+                                             "trained against log eta"; Q21), capped at 2^10 like the guard */
+} ks_head_output;
 typedef enum { KS_COL_I32 = 0, KS_COL_F32 = 1 } ks_col_dtype;   /* F32 columns must hold exact integers < 2^24 */
 typedef enum { KS_MEM_DEVICE = 0, KS_MEM_HOST = 1 } ks_mem_space;
 
@@ -91,6 +109,8 @@ typedef struct {
   int32_t n_cols;          /* columns supplied; must equal the family's count */
   int32_t attn_hq, attn_hkv, attn_head_dim;
   const void *cols[KS_MAX_COLS];
+  int32_t model_slot;      /* efficiency model that prices this bucket: KS_SLOT_FAMILY (-1) or a slot in
+                              [0, KS_MAX_MODEL_SLOTS).  NOTE: zero-initialised structs name slot 0 (KS_SLOT_GEMM) */
   const int32_t *mult;     /* optional (may be NULL = all ones): per-row multiplicity m_k >= 0, int32 [n], in the
                               call's memory space.  Layer-homogeneous form of PAPER.md:231 (t_gpu = L t_layer +
                               t_lm_head + t_embed): a row stands for m_k identical kernels of its step.  Read by
@@ -104,45 +124,52 @@ typedef struct { float c_disp, floor_l, c_ovl, c_tail, body_scale; } ks_step_par
  * stream) on which all work of this context is enqueued.  KS_ECUDA if the device is not sm_100. */
 KS_API ks_status ks_create(ks_ctx **out, int device, void *cuda_stream);
 
-/* Load (or replace) the Tier-A efficiency head of `family`: MLP n_in -> h1 -> h2 -> 1 with GELU
+/* Load (or replace) the Tier-A efficiency head of model slot `slot` (0 <= slot < KS_MAX_MODEL_SLOTS; a slot holds
+ * ONE Tier-A head of any kind and ONE Tier-B grid): MLP n_in -> h1 -> h2 -> 1 with GELU
  * hidden activations and a sigmoid output giving the efficiency e (sizes and
  * activations BASELINE.json; Q3, Q6).  All arrays are HOST fp32 and are copied: W1[n_in][h1],
  * b1[h1], W2[h1][h2], b2[h2], w3[h2].  Weights are rounded to bf16 (RNE) for the tensor-core
  * contraction; biases keep >= 16 significant bits.  The feature vector is fixed by the library
  * (Q2): n_in must be 8, 12 or 32.  Supported hidden sizes: h1 == h2 in {64, 128, 256};
  * anything else returns KS_EUNSUPPORTED. */
-KS_API ks_status ks_load_heads(ks_ctx *ctx, ks_family family, int n_in, int h1, int h2, const float *W1,
+KS_API ks_status ks_load_heads(ks_ctx *ctx, int slot, int n_in, int h1, int h2, const float *W1,
                         const float *b1, const float *W2, const float *b2, const float *w3, float b3);
 
-/* Load (or replace) the Tier-A head of `family` with an MLP ENSEMBLE ("small MLP ensemble";
+/* Load (or replace) the Tier-A head of `slot` with an MLP ENSEMBLE ("small MLP ensemble";
  * DESIGN.md Q17): n_members MLPs n_in -> h -> h -> 1 of one shape, each as in ks_load_heads; the efficiency is
  * the arithmetic mean of the members' sigmoid outputs, e = (1/k) sum_m sigmoid(z_m(x)), then the guard and
  * eta = 1/e.  Arrays are HOST fp32 with the member index leading, copied: W1[k][n_in][h], b1[k][h],
  * W2[k][h][h], b2[k][h], w3[k][h], b3[k].  The members run side by side in ONE pass of the Tier-A kernel
  * (layer 1 concatenated, layer 2 block-diagonal), so k * h must be a supported hidden size:
  * h in {32, 64, 128}, k <= KS_MAX_ENSEMBLE, k * h in {64, 128, 256}; anything else KS_EUNSUPPORTED.
- * Replaces any head the family held. */
+ * Replaces any head the slot held. */
 #define KS_MAX_ENSEMBLE 8
-KS_API ks_status ks_load_head_ensemble(ks_ctx *ctx, ks_family family, int n_in, int h, int n_members,
+KS_API ks_status ks_load_head_ensemble(ks_ctx *ctx, int slot, int n_in, int h, int n_members,
                                 const float *W1, const float *b1, const float *W2, const float *b2,
                                 const float *w3, const float *b3);
 
-/* Load (or replace) the Tier-A head of `family` with the BOUNDED ANALYTICAL form (PAPER.md:197 Fig. 6, :201;
+/* Load (or replace) the Tier-A head of `slot` with the BOUNDED ANALYTICAL form (PAPER.md:197 Fig. 6, :201;
  * DESIGN.md Q15): utilisation e = gamma(x) - alpha(x) / W with W the kernel's wave count,
  * gamma(x) = sigmoid(w_gamma . x + b_gamma), alpha(x) = max(0, w_alpha . x + b_alpha), e clamped to
  * [2^-10, 1], eta = 1 / e.  x = the library's dimensionless features (Q2) in fp32; n_in in {8, 12, 32}.
- * w_gamma[n_in], w_alpha[n_in]: HOST fp32, copied.  A family holds ONE Tier-A head: this call replaces
+ * w_gamma[n_in], w_alpha[n_in]: HOST fp32, copied.  A slot holds ONE Tier-A head: this call replaces
  * an MLP head loaded with ks_load_heads and vice versa.  Runs in the streaming kernel (no contraction). */
-KS_API ks_status ks_load_bounded_head(ks_ctx *ctx, ks_family family, int n_in, const float *w_gamma, float b_gamma,
+KS_API ks_status ks_load_bounded_head(ks_ctx *ctx, int slot, int n_in, const float *w_gamma, float b_gamma,
                                const float *w_alpha, float b_alpha);
 
-/* Load (or replace) the Tier-B measured-efficiency grid of `family` (Q5).
- * values: HOST fp32 [dims[0]][dims[1]][dims[2]], last index fastest, copied; each dims[a] >= 1 and
- * the product <= KS_MAX_GRID_NODES.  Axis a spans [lo_log2[a], hi_log2[a]] in log2 units with
- * dims[a] uniformly spaced nodes; queries are clamped to the span.  Axis values per family:
- * GEMM (M, N, K); GROUPED (sum m_e, N, K); ATTN (batch, q_len, kv_len); ELEMWISE (n, 2^subop, 1). */
-KS_API ks_status ks_load_grid(ks_ctx *ctx, ks_family family, const int32_t dims[3], const float lo_log2[3],
+/* Load (or replace) the Tier-B measured-efficiency grid of `slot` (Q5).
+ * values: HOST fp32 [dims[0]][dims[1]][dims[2]], last index fastest, copied, all finite; each dims[a] >= 1 and
+ * the product <= KS_MAX_GRID_NODES.  Axis a spans [lo_log2[a], hi_log2[a]] in log2 units (within [-64, 64]: the
+ * axis values are int32) with dims[a] uniformly spaced nodes; queries are clamped to the span.  The axis values
+ * are those of the FAMILY of the bucket that uses the slot: GEMM (M, N, K); GROUPED (sum m_e, N, K);
+ * ATTN (batch, q_len, kv_len); ELEMWISE (n, 2^subop, 1). */
+KS_API ks_status ks_load_grid(ks_ctx *ctx, int slot, const int32_t dims[3], const float lo_log2[3],
                        const float hi_log2[3], const float *values);
+
+/* Say what the scalar output of the MLP head loaded in `slot` means (default after every ks_load_heads:
+ * KS_HEAD_UTILISATION).  KS_ESTATE if the slot holds no single MLP head (ensembles and the bounded form have one
+ * output convention each: KS_EUNSUPPORTED). */
+KS_API ks_status ks_set_head_output(ks_ctx *ctx, int slot, ks_head_output mode);
 
 /* Predict the latency of every (spec, descriptor) pair (steps S1-S5 of DESIGN.md §1).
  *   batches[n_batches]   family buckets (<= KS_MAX_BATCHES)
@@ -156,8 +183,8 @@ KS_API ks_status ks_load_grid(ks_ctx *ctx, ks_family family, const int32_t dims[
  *   tiles[b], waves[b]   optional out (array pointer or entry may be NULL), int32 [n_specs][n]:
  *                        CTA count B and wave count W = ceil(B/S)
  *   t_roof[b]            optional out, fp32 [n_specs][n]
- * KS_ESTATE if the tier needs a head/grid that was not loaded for a bucket's family
- * (KS_FAM_ALLREDUCE needs neither). */
+ * KS_ESTATE if the tier needs a head/grid that was not loaded in a bucket's model slot
+ * (KS_FAM_ALLREDUCE buckets need neither). */
 KS_API ks_status ks_predict_kernels(ks_ctx *ctx, const ks_desc_batch *batches, int n_batches,
                              const ks_hw_spec *specs, int n_specs, ks_tier tier, ks_mem_space space,
                              float *const *latency, int32_t *const *tiles, int32_t *const *waves,
@@ -201,7 +228,7 @@ KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const i
  * ks_sched is one replica's scheduler, HOST logic (the paper's scheduler is host code too): "a single
  * token-budget loop advances every request's computed-token count toward its target", with continuous
  * batching, chunked prefill, FCFS queuing and preemption/recompute under KV pressure (
- * the exact rules are DESIGN.md Q18; prefix caching is not modelled).  It needs no GPU and no ks_ctx.
+ * the exact rules are DESIGN.md Q18; the two-tier prefix cache of PAPER.md:247 is Q19).  It needs no GPU and no ks_ctx.
  * ks_sim_run closes the loop for many replicas at once: every iteration each unfinished replica forms
  * the batch of its next step, the batches' kernel rows (layer-homogeneous form :231) are
  * priced by ONE pass of the GPU path (ks_run_steps), and each replica's clock advances by its own
@@ -289,8 +316,9 @@ KS_API ks_status ks_sim_run(ks_ctx *ctx, ks_sched *const *scheds, double *clock,
 /* Counters: number of kernel launches this context has enqueued so far (for gpu_launches). */
 KS_API ks_status ks_get_launch_count(ks_ctx *ctx, int64_t *out);
 
-/* Tier-A activation mode: 0 = fp32 tanh-form GELU (default, most accurate),
- * 1 = packed bf16x2 tanh-form GELU (faster; see DESIGN.md §5 for measured error). */
+/* Tier-A activation mode: 0 = fp32 tanh-form GELU (default: most accurate and, as measured, also the fastest),
+ * 1 = packed bf16x2 tanh-form GELU (half the MUFU work, ~4x the activation rounding error; measured 2-5 % SLOWER
+ * on B200 because the packing and the bf16x2 FMAs move the bound to the issue slots). */
 KS_API ks_status ks_set_gelu_mode(ks_ctx *ctx, int mode);
 
 /* Free everything the context owns.  NULL is a no-op returning KS_OK. */

@@ -33,6 +33,10 @@ double kso_bf16(double x) {
 double kso_gelu(double x) { return 0.5 * x * (1.0 + erf(x / sqrt(2.0))); }
 double kso_sigmoid(double z) { return 1.0 / (1.0 + exp(-z)); }
 
+/* heads are trained against log eta = log(t_meas / t_roof); eta >= 1 (the roofline is a
+ * lower bound), so a negative output is floored at log eta = 0 (Q21). */
+double kso_eta_from_log(double z) { return exp(z > 0.0 ? z : 0.0); }
+
 /* ---------------------------------------------------------------- S1: F_comp, F_mem, B
  * PAPER.md:193 names "the kernel's FLOPs and bytes" without printing formulas; Q1. */
 
@@ -201,6 +205,12 @@ double kso_mlp_z(const kso_head *h, const double *x) {
   return z;
 }
 
+/* The head's output convention: utilisation e = sigmoid(z) (Q3), or z = log eta, e = 1 / eta (Q21). */
+double kso_head_e(const kso_head *h, const double *x) {
+  const double z = kso_mlp_z(h, x);
+  return h->log_eta ? 1.0 / kso_eta_from_log(z) : kso_sigmoid(z);
+}
+
 /* ---------------------------------------------------------------- S4b: Tier-B grid
  * "eta is obtained by interpolating this grid"; scheme/clamp: DESIGN.md Q5. */
 void kso_grid_axes(const kso_desc *d, double v[3]) {
@@ -275,7 +285,7 @@ double kso_predict_one(const kso_desc *d, const kso_spec *hw, int tier, const ks
     double x[32];
     kso_features(d, hw, &r, h->n_in, x);
     for (int i = 0; i < h->n_in; ++i) x[i] = kso_bf16(x[i]);   /* bf16 inputs, Q11 */
-    e = kso_sigmoid(kso_mlp_z(h, x));
+    e = kso_head_e(h, x);
   } else if (tier == KSO_TIER_B) {
     double v[3];
     kso_grid_axes(d, v);

@@ -57,10 +57,13 @@ typedef struct {           /* everything Eq. 2's right half produces for one (de
   double u, t_comp, t_mem, t_roof;
 } kso_roof;
 
-typedef struct {           /* Tier A head: MLP n_in -> h1 -> h2 -> 1 (GELU, sigmoid out) */
+typedef struct {           /* Tier A head: MLP n_in -> h1 -> h2 -> 1 (GELU hidden units) */
   int n_in, h1, h2;
   const double *W1, *b1, *W2, *b2, *w3; /* W1[n_in][h1], W2[h1][h2]; already bf16-rounded weights */
   double b3;
+  int log_eta;             /* what the output z means: 0 = utilisation, e = sigmoid(z) (BASELINE.json; Q3);
+                              1 = z is log eta ("trained against log eta"): eta = exp(max(z, 0)) >= 1
+                              (PAPER.md:193), Q21 */
 } kso_head;
 
 typedef struct {           /* Tier B measured-efficiency grid */
@@ -82,6 +85,10 @@ double kso_bf16(double x);
 /* exact GELU 0.5 x (1 + erf(x / sqrt 2)) and logistic sigmoid */
 double kso_gelu(double x);
 double kso_sigmoid(double z);
+/* eta of a head whose output is log eta, floored at the roofline bound eta >= 1 (Q21) */
+double kso_eta_from_log(double z);
+/* utilisation e = 1 / eta that an MLP head gives for the (bf16-rounded) features x, by its output convention */
+double kso_head_e(const kso_head *h, const double *x);
 
 /* Tensor-parallel ring all-reduce, Eq. 3: t_ar = alpha0 + 2 (P - 1) / P * S / beta_eff
  * (S message bytes, P shards; P <= 1 moves nothing: t_ar = alpha0).  No roofline, no eta, no t0 floor. */

@@ -52,7 +52,7 @@ class HeadC(C.Structure):
     _fields_ = [("n_in", C.c_int), ("h1", C.c_int), ("h2", C.c_int),
                 ("W1", C.POINTER(C.c_double)), ("b1", C.POINTER(C.c_double)),
                 ("W2", C.POINTER(C.c_double)), ("b2", C.POINTER(C.c_double)),
-                ("w3", C.POINTER(C.c_double)), ("b3", C.c_double)]
+                ("w3", C.POINTER(C.c_double)), ("b3", C.c_double), ("log_eta", C.c_int)]
 
 
 class GridC(C.Structure):
@@ -78,6 +78,10 @@ def lib():
         L.kso_gelu.argtypes = [C.c_double]
         L.kso_sigmoid.restype = C.c_double
         L.kso_sigmoid.argtypes = [C.c_double]
+        L.kso_eta_from_log.restype = C.c_double
+        L.kso_eta_from_log.argtypes = [C.c_double]
+        L.kso_head_e.restype = C.c_double
+        L.kso_head_e.argtypes = [C.POINTER(HeadC), C.POINTER(C.c_double)]
         L.kso_bounded_e.restype = C.c_double
         L.kso_bounded_e.argtypes = [C.POINTER(BoundedC), C.POINTER(C.c_double), C.c_int64]
         L.kso_predict_batch_bounded.restype = C.c_int
@@ -174,7 +178,7 @@ class Head:
         self.b1 = np.ascontiguousarray(h.b1, dtype=np.float64)
         self.b2 = np.ascontiguousarray(h.b2, dtype=np.float64)
         self.c = HeadC(int(h.n_in), int(h.h1), int(h.h2), _dp(self.W1), _dp(self.b1), _dp(self.W2),
-                       _dp(self.b2), _dp(self.w3), float(h.b3))
+                       _dp(self.b2), _dp(self.w3), float(h.b3), int(getattr(h, "out_mode", 0)))
 
 
 class Ensemble:
@@ -227,6 +231,15 @@ def features(desc: Desc, spec: Spec, n_in: int) -> np.ndarray:
     x = np.zeros(n_in, np.float64)
     lib().kso_features(C.byref(desc), C.byref(spec), C.byref(r), int(n_in), _dp(x))
     return x
+
+
+def eta_from_log(z: float) -> float:
+    return float(lib().kso_eta_from_log(float(z)))
+
+
+def head_e(head: Head, x) -> float:
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    return float(lib().kso_head_e(C.byref(head.c), _dp(x)))
 
 
 def mlp_z(head: Head, x) -> float:

@@ -348,7 +348,7 @@ def price_steps(batches: Sequence[Sequence[Tuple[int, int, int]]], m: Model, spe
     """Step wall times (Eq. 4) of the given batches, priced by the oracle predictor: rows of step_rows ->
     per-kernel latency (oracle.predict_bucket) -> weighted step sums + Eq. 4 (oracle.compose)."""
     from . import oracle as O
-    from paper_2606_28565_b200 import workloads as W   # dataclasses only (no arithmetic)
+    import workloads as W   # dataclasses only (no arithmetic)
 
     fams = [0, 2, 3] + ([4] if m.tp > 1 else [])
     cols = {f: [] for f in fams}

@@ -18,10 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libks.so")
 KS_OK, KS_EINVAL, KS_ENOMEM, KS_ECUDA, KS_ESTATE, KS_EUNSUPPORTED = range(6)
 KS_FAM_GEMM, KS_FAM_GROUPED_GEMM, KS_FAM_ATTN, KS_FAM_ELEMWISE = range(4)
 KS_TIER_NONE, KS_TIER_A, KS_TIER_B = range(3)
+KS_SLOT_FAMILY, KS_MAX_MODEL_SLOTS = -1, 16
+KS_HEAD_UTILISATION, KS_HEAD_LOG_ETA = 0, 1
 KS_COL_I32, KS_COL_F32 = 0, 1
 KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
-EXPORTS = ["ks_create", "ks_load_heads", "ks_load_head_ensemble", "ks_load_bounded_head", "ks_load_grid", "ks_predict_kernels", "ks_compose_steps",
+EXPORTS = ["ks_create", "ks_load_heads", "ks_load_head_ensemble", "ks_load_bounded_head", "ks_load_grid", "ks_set_head_output",
+           "ks_predict_kernels", "ks_compose_steps",
            "ks_compose_steps_weighted",
            "ks_run_steps", "ks_sched_create", "ks_sched_add_requests", "ks_sched_add_prefixed_requests", "ks_sched_step", "ks_sched_commit",
            "ks_sched_results", "ks_sched_get_stats", "ks_sched_destroy", "ks_sim_run",
@@ -44,7 +47,8 @@ class ks_hw_spec(C.Structure):
 class ks_desc_batch(C.Structure):
     _fields_ = [("family", C.c_int32), ("n", C.c_int32), ("col_dtype", C.c_int32), ("dtype_bytes", C.c_int32),
                 ("n_cols", C.c_int32), ("attn_hq", C.c_int32), ("attn_hkv", C.c_int32),
-                ("attn_head_dim", C.c_int32), ("cols", C.c_void_p * KS_MAX_COLS), ("mult", C.c_void_p)]
+                ("attn_head_dim", C.c_int32), ("cols", C.c_void_p * KS_MAX_COLS), ("model_slot", C.c_int32),
+                ("mult", C.c_void_p)]
 
 
 class ks_step_params(C.Structure):
@@ -92,6 +96,7 @@ def load() -> C.CDLL:
     L.ks_load_head_ensemble.argtypes = [vp, i32, i32, i32, i32, fp, fp, fp, fp, fp, fp]
     L.ks_load_bounded_head.argtypes = [vp, i32, i32, fp, C.c_float, fp, C.c_float]
     L.ks_load_grid.argtypes = [vp, i32, C.POINTER(C.c_int32), fp, fp, fp]
+    L.ks_set_head_output.argtypes = [vp, i32, i32]
     L.ks_predict_kernels.argtypes = [vp, C.POINTER(ks_desc_batch), i32, C.POINTER(ks_hw_spec), i32, i32, i32,
                                      C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.ks_compose_steps.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int32), i32, i32, i32,
@@ -177,8 +182,10 @@ def make_batch(bucket) -> ks_desc_batch:
     mult = getattr(bucket, "mult", None)             # optional per-row multiplicities (int32)
     if mult is not None and "int32" not in str(mult.dtype):
         raise TypeError("multiplicities must be int32")
+    slot = getattr(bucket, "model_slot", None)      # None = the slot numbered like the family
     return ks_desc_batch(int(bucket.family), n, cd, int(bucket.dtype_bytes), len(cols), int(bucket.hq),
-                         int(bucket.hkv), int(bucket.head_dim), arr, _ptr(mult) if mult is not None else None)
+                         int(bucket.hkv), int(bucket.head_dim), arr, KS_SLOT_FAMILY if slot is None else int(slot),
+                         _ptr(mult) if mult is not None else None)
 
 
 def make_step_params(p: dict) -> ks_step_params:
@@ -205,13 +212,18 @@ class Context:
         except Exception:
             pass
 
-    # ---- loading
+    # ---- loading (the first argument of every loader is a model SLOT; slot = family for one model per family)
     def load_heads(self, family: int, head) -> None:
         f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
         W1, b1, W2, b2, w3 = f32(head.W1), f32(head.b1), f32(head.W2), f32(head.b2), f32(head.w3)
         fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
         _check(self._lib.ks_load_heads(self._h, int(family), int(head.n_in), int(head.h1), int(head.h2), fp(W1),
                                        fp(b1), fp(W2), fp(b2), fp(w3), float(head.b3)), "ks_load_heads")
+        if int(getattr(head, "out_mode", KS_HEAD_UTILISATION)) != KS_HEAD_UTILISATION:
+            self.set_head_output(family, int(head.out_mode))
+
+    def set_head_output(self, slot: int, mode: int) -> None:
+        _check(self._lib.ks_set_head_output(self._h, int(slot), int(mode)), "ks_set_head_output")
 
     def load_head_ensemble(self, family: int, members) -> None:
         """members: workloads.Head objects of one shape (n_in -> h -> h -> 1)."""

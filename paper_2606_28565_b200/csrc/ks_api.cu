@@ -26,6 +26,7 @@ struct HeadState {
   float b3 = 0.0f;
   int members = 1;           // > 1: MLP ensemble packed as one head of width h (Q17)
   float b3m[KS_MAX_ENSEMBLE] = {};
+  int out_mode = KS_HEAD_UTILISATION;   // what z means (ks_set_head_output)
 };
 
 struct GridState {
@@ -44,8 +45,8 @@ struct ks_ctx {
   bool sticky = false;
   int gelu_mode = 0;
   int64_t launches = 0;
-  HeadState heads[KS_FAM_COUNT];
-  GridState grids[KS_FAM_COUNT];
+  HeadState heads[KS_MAX_MODEL_SLOTS];   // by model slot (include/ks.h: ks_model_slot), not by decode family
+  GridState grids[KS_MAX_MODEL_SLOTS];
   // grow-only device workspace with a bump pointer (host-space staging, internal latencies)
   char* ws = nullptr;
   size_t ws_cap = 0, ws_used = 0;
@@ -63,6 +64,10 @@ namespace {
 const int kFamCols[KS_FAM_COUNT] = {3, 10, 3, 2, 2};
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// the model slot that prices a bucket: its own, or the one numbered like its family
+inline int slot_of(const ks_desc_batch& k) { return k.model_slot == KS_SLOT_FAMILY ? k.family : k.model_slot; }
+inline bool slot_ok(int slot) { return slot >= 0 && slot < KS_MAX_MODEL_SLOTS; }
 
 ks_status cuda_fail(ks_ctx* c) {
   if (c) c->sticky = true;
@@ -192,9 +197,10 @@ ks_status validate_batches(const ks_ctx* c, const ks_desc_batch* batches, int n_
         if (!k.cols[col]) return KS_EINVAL;
         if (device_ptrs && !aligned16(k.cols[col])) return KS_EINVAL;
       }
+    if (k.model_slot != KS_SLOT_FAMILY && !slot_ok(k.model_slot)) return KS_EINVAL;
     if (k.family == KS_FAM_ALLREDUCE) continue;               // Eq. 3 needs neither head nor grid
-    if ((tier == KS_TIER_A || tier == KS_TIER_B_ROUTED) && !c->heads[k.family].loaded) return KS_ESTATE;
-    if ((tier == KS_TIER_B || tier == KS_TIER_B_ROUTED) && !c->grids[k.family].loaded) return KS_ESTATE;
+    if ((tier == KS_TIER_A || tier == KS_TIER_B_ROUTED) && !c->heads[slot_of(k)].loaded) return KS_ESTATE;
+    if ((tier == KS_TIER_B || tier == KS_TIER_B_ROUTED) && !c->grids[slot_of(k)].loaded) return KS_ESTATE;
   }
   return KS_OK;
 }
@@ -296,7 +302,7 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
             tb_done[b0] = true;
             if (k.n == 0) continue;
             p.bk[nb] = make_bucket_dev(k, cols[b0], outs[b0], s0);
-            p.grid[nb] = c->grids[k.family].tb;
+            p.grid[nb] = c->grids[slot_of(k)].tb;
             if (routed && s0 == 0) {                      // the hull test depends on the row only: list it once
               KS_CUDA(c, cudaMemsetAsync(rb[b0].count, 0, 4, c->stream));
               p.grid[nb].route_idx = rb[b0].idx;
@@ -317,14 +323,14 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
       if (tb_done[b]) continue;
       const bool ar = batches[b].family == KS_FAM_ALLREDUCE;
       if (ar && lists) continue;                        // Eq. 3 rows were finished by pass 1
-      const bool bnd = tier == KS_TIER_A && !ar && c->heads[batches[b].family].bounded;
+      const bool bnd = tier == KS_TIER_A && !ar && c->heads[slot_of(batches[b])].bounded;
       if (batches[b].n == 0 || (tier == KS_TIER_A && !ar && !bnd)) continue;
       {
         KsStreamParams p;
         memset(&p, 0, sizeof(p));
         p.bk = make_bucket_dev(batches[b], cols[b], outs[b], s0);
         if (lists) { p.bk.idx = rb[b].idx; p.bk.count = rb[b].count; }
-        if (tier == KS_TIER_B && !ar) p.grid = c->grids[batches[b].family].dev;
+        if (tier == KS_TIER_B && !ar) p.grid = c->grids[slot_of(batches[b])].dev;
         if (routed && pass == 0 && !ar && s0 == 0) {    // the hull test depends on the row only: list it once
           KS_CUDA(c, cudaMemsetAsync(rb[b].count, 0, 4, c->stream));
           p.grid.route_idx = rb[b].idx;
@@ -332,7 +338,7 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
         }
         p.n_specs = ns;
         p.tier = ar ? KS_TIER_NONE : bnd ? KS_TIER_BOUNDED : tier;
-        if (bnd) p.bounded = c->heads[batches[b].family].bw;
+        if (bnd) p.bounded = c->heads[slot_of(batches[b])].bw;
         p.spec_stride = batches[b].n;
         for (int s = 0; s < ns; ++s) p.specs.s[s] = make_spec_dev(specs[s0 + s]);
         KS_CUDA(c, ks_launch_stream(p, c->num_sms, c->stream));
@@ -343,16 +349,16 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
       // group buckets by head dimensions; one persistent launch per group of <= 4 buckets
       bool done[KS_MAX_BATCHES] = {false};
       for (int b = 0; b < n_batches; ++b) {
-        if (batches[b].family == KS_FAM_ALLREDUCE || c->heads[batches[b].family].bounded) done[b] = true;
+        if (batches[b].family == KS_FAM_ALLREDUCE || c->heads[slot_of(batches[b])].bounded) done[b] = true;
         if (done[b] || batches[b].n == 0) { done[b] = true; continue; }
-        const HeadState& h0 = c->heads[batches[b].family];
+        const HeadState& h0 = c->heads[slot_of(batches[b])];
         KsMlpParams p;
         memset(&p, 0, sizeof(p));
         int nb = 0, tiles = 0;
         for (int q = b; q < n_batches && nb < KS_MLP_MAX_BUCKETS; ++q) {
           if (done[q] || batches[q].n == 0 || batches[q].family == KS_FAM_ALLREDUCE ||
-              c->heads[batches[q].family].bounded) continue;
-          const HeadState& hq = c->heads[batches[q].family];
+              c->heads[slot_of(batches[q])].bounded) continue;
+          const HeadState& hq = c->heads[slot_of(batches[q])];
           if (hq.n_in != h0.n_in || hq.h != h0.h) continue;
           p.bk[nb] = make_bucket_dev(batches[q], cols[q], outs[q], s0);
           if (lists) { p.bk[nb].idx = rb[q].idx; p.bk[nb].count = rb[q].count; }
@@ -362,6 +368,11 @@ ks_status predict_device(ks_ctx* c, const ks_desc_batch* batches, const void* co
           p.head[nb].b2 = hq.b2;
           p.head[nb].b3 = hq.b3;
           p.head[nb].members = hq.members;
+          // eta = out_add + exp(max(out_sgn * z, out_lo)): 1 + exp(-z) (utilisation) or exp(max(z, 0)) (log eta)
+          const bool log_eta = hq.out_mode == KS_HEAD_LOG_ETA;
+          p.head[nb].out_sgn = log_eta ? 1.0f : -1.0f;
+          p.head[nb].out_lo = log_eta ? 0.0f : -INFINITY;
+          p.head[nb].out_add = log_eta ? 0.0f : 1.0f;
           if (hq.members > 1) p.any_ens = 1;
           for (int m = 0; m < KS_MAX_ENSEMBLE; ++m) p.head[nb].b3m[m] = hq.b3m[m];
           p.tile_begin[nb] = tiles;
@@ -422,7 +433,7 @@ ks_status ks_destroy(ks_ctx* c) {
   if (!c) return KS_OK;
   cudaSetDevice(c->device);
   cudaStreamSynchronize(c->stream);
-  for (int f = 0; f < KS_FAM_COUNT; ++f) {
+  for (int f = 0; f < KS_MAX_MODEL_SLOTS; ++f) {
     cudaFree(c->heads[f].w1_img);
     cudaFree(c->heads[f].w2_img);
     cudaFree(c->heads[f].w3);
@@ -448,6 +459,15 @@ ks_status ks_get_launch_count(ks_ctx* c, int64_t* out) {
   return KS_OK;
 }
 
+ks_status ks_set_head_output(ks_ctx* c, int slot, ks_head_output mode) {
+  if (!c || !slot_ok(slot) || (mode != KS_HEAD_UTILISATION && mode != KS_HEAD_LOG_ETA)) return KS_EINVAL;
+  HeadState& hs = c->heads[slot];
+  if (!hs.loaded) return KS_ESTATE;
+  if (hs.bounded || hs.members > 1) return KS_EUNSUPPORTED;
+  hs.out_mode = mode;                                // read when a launch is built: no device state to update
+  return KS_OK;
+}
+
 ks_status ks_set_gelu_mode(ks_ctx* c, int mode) {
   if (!c || (mode != 0 && mode != 1)) return KS_EINVAL;
   c->gelu_mode = mode;
@@ -458,7 +478,7 @@ namespace {
 
 // Builds the operand images of a dense head n_in -> H -> H and installs it for `family`.  members > 1:
 // the arrays hold an ensemble packed by ks_load_head_ensemble and b3m its per-member output biases.
-ks_status install_head(ks_ctx* c, ks_family family, int n_in, int H, const float* W1, const float* b1,
+ks_status install_head(ks_ctx* c, int slot, int n_in, int H, const float* W1, const float* b1,
                        const float* W2, const float* b2, const float* w3, float b3, int members, const float* b3m) {
   const int K1 = ks_mlp_k1(n_in);
   const int n_real = n_in == 32 ? 22 : n_in;          // features 22..31 are identically zero (Q2)
@@ -484,7 +504,7 @@ ks_status install_head(ks_ctx* c, ks_family family, int n_in, int H, const float
 
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read the old head
-  HeadState& hs = c->heads[family];
+  HeadState& hs = c->heads[slot];
   cudaFree(hs.w1_img); cudaFree(hs.w2_img); cudaFree(hs.w3); cudaFree(hs.b2);
   hs = HeadState();
   void *d1 = nullptr, *d2 = nullptr, *d3 = nullptr, *d4 = nullptr;
@@ -516,18 +536,18 @@ ks_status install_head(ks_ctx* c, ks_family family, int n_in, int H, const float
 
 }  // namespace
 
-ks_status ks_load_heads(ks_ctx* c, ks_family family, int n_in, int h1, int h2, const float* W1, const float* b1,
+ks_status ks_load_heads(ks_ctx* c, int slot, int n_in, int h1, int h2, const float* W1, const float* b1,
                         const float* W2, const float* b2, const float* w3, float b3) {
-  if (!c || family < 0 || family >= KS_FAM_COUNT || !W1 || !b1 || !W2 || !b2 || !w3) return KS_EINVAL;
+  if (!c || !slot_ok(slot) || !W1 || !b1 || !W2 || !b2 || !w3) return KS_EINVAL;
   if (n_in <= 0 || h1 <= 0 || h2 <= 0) return KS_EINVAL;
   if (c->sticky) return KS_ECUDA;
   if ((n_in != 8 && n_in != 12 && n_in != 32) || h1 != h2 || (h1 != 64 && h1 != 128 && h1 != 256)) return KS_EUNSUPPORTED;
-  return install_head(c, family, n_in, h1, W1, b1, W2, b2, w3, b3, 1, nullptr);
+  return install_head(c, slot, n_in, h1, W1, b1, W2, b2, w3, b3, 1, nullptr);
 }
 
-ks_status ks_load_head_ensemble(ks_ctx* c, ks_family family, int n_in, int h, int n_members, const float* W1,
+ks_status ks_load_head_ensemble(ks_ctx* c, int slot, int n_in, int h, int n_members, const float* W1,
                                 const float* b1, const float* W2, const float* b2, const float* w3, const float* b3) {
-  if (!c || family < 0 || family >= KS_FAM_COUNT || family == KS_FAM_ALLREDUCE || !W1 || !b1 || !W2 || !b2 || !w3 || !b3)
+  if (!c || !slot_ok(slot) || !W1 || !b1 || !W2 || !b2 || !w3 || !b3)
     return KS_EINVAL;
   if (n_in <= 0 || h <= 0 || n_members <= 0) return KS_EINVAL;
   if (c->sticky) return KS_ECUDA;
@@ -535,7 +555,7 @@ ks_status ks_load_head_ensemble(ks_ctx* c, ks_family family, int n_in, int h, in
   if ((n_in != 8 && n_in != 12 && n_in != 32) || n_members > KS_MAX_ENSEMBLE || (h != 32 && h != 64 && h != 128) ||
       (H != 64 && H != 128 && H != 256))
     return KS_EUNSUPPORTED;
-  if (n_members == 1) return install_head(c, family, n_in, h, W1, b1, W2, b2, w3, b3[0], 1, nullptr);
+  if (n_members == 1) return install_head(c, slot, n_in, h, W1, b1, W2, b2, w3, b3[0], 1, nullptr);
   // Pack the members side by side into one head of width H = k h: layer 1 concatenated along its outputs,
   // layer 2 block-diagonal (the zero blocks contribute exact zeros to the fp32 accumulators), layer 3
   // concatenated; the kernels close one dot product + sigmoid per member and average (Q17).
@@ -553,13 +573,13 @@ ks_status ks_load_head_ensemble(ks_ctx* c, ks_family family, int n_in, int h, in
       pw3[m * h + j] = w3[(size_t)m * h + j];
     }
   }
-  return install_head(c, family, n_in, H, pW1.data(), pb1.data(), pW2.data(), pb2.data(), pw3.data(), 0.0f,
+  return install_head(c, slot, n_in, H, pW1.data(), pb1.data(), pW2.data(), pb2.data(), pw3.data(), 0.0f,
                       n_members, b3);
 }
 
-ks_status ks_load_bounded_head(ks_ctx* c, ks_family family, int n_in, const float* w_gamma, float b_gamma,
+ks_status ks_load_bounded_head(ks_ctx* c, int slot, int n_in, const float* w_gamma, float b_gamma,
                                const float* w_alpha, float b_alpha) {
-  if (!c || family < 0 || family >= KS_FAM_COUNT || family == KS_FAM_ALLREDUCE || !w_gamma || !w_alpha) return KS_EINVAL;
+  if (!c || !slot_ok(slot) || !w_gamma || !w_alpha) return KS_EINVAL;
   if (n_in <= 0 || !isfinite(b_gamma) || !isfinite(b_alpha)) return KS_EINVAL;
   if (n_in != 8 && n_in != 12 && n_in != 32) return KS_EUNSUPPORTED;    // before the arrays are read: their length is n_in
   for (int i = 0; i < n_in; ++i)
@@ -567,7 +587,7 @@ ks_status ks_load_bounded_head(ks_ctx* c, ks_family family, int n_in, const floa
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));       // nothing in flight may still read an MLP head being replaced
-  HeadState& hs = c->heads[family];
+  HeadState& hs = c->heads[slot];
   cudaFree(hs.w1_img); cudaFree(hs.w2_img); cudaFree(hs.w3); cudaFree(hs.b2);
   hs = HeadState();
   memset(&hs.bw, 0, sizeof(hs.bw));
@@ -581,9 +601,9 @@ ks_status ks_load_bounded_head(ks_ctx* c, ks_family family, int n_in, const floa
   return KS_OK;
 }
 
-ks_status ks_load_grid(ks_ctx* c, ks_family family, const int32_t dims[3], const float lo_log2[3],
+ks_status ks_load_grid(ks_ctx* c, int slot, const int32_t dims[3], const float lo_log2[3],
                        const float hi_log2[3], const float* values) {
-  if (!c || family < 0 || family >= KS_FAM_COUNT || !dims || !lo_log2 || !hi_log2 || !values) return KS_EINVAL;
+  if (!c || !slot_ok(slot) || !dims || !lo_log2 || !hi_log2 || !values) return KS_EINVAL;
   long long nodes = 1;
   for (int a = 0; a < 3; ++a) {
     if (dims[a] < 1 || dims[a] > KS_MAX_GRID_NODES) return KS_EINVAL;
@@ -598,7 +618,7 @@ ks_status ks_load_grid(ks_ctx* c, ks_family family, const int32_t dims[3], const
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
   KS_CUDA(c, cudaStreamSynchronize(c->stream));
-  GridState& g = c->grids[family];
+  GridState& g = c->grids[slot];
   cudaFree(g.values);
   g = GridState();
   // bulk copies move multiples of 16 bytes.  Behind the last node: one plane + one row + two floats of zeros (the

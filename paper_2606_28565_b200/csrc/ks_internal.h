@@ -71,6 +71,9 @@ struct KsHeadDev {
   int32_t members;         // > 1: MLP ensemble (Q17) of `members` heads, H / members columns each:
                            // W1/b1/b2/w3 concatenated, W2 block-diagonal, one output bias per member
   float b3m[KS_MAX_ENSEMBLE];
+  // single MLP head: eta = out_add + exp(max(out_sgn * z, out_lo)), i.e. 1 + exp(-z) for a utilisation output
+  // (-1, -inf, 1) or exp(max(z, 0)) for a log-eta output (+1, 0, 0); ks_set_head_output
+  float out_sgn, out_lo, out_add;
 };
 struct KsMlpParams {
   KsBucketDev bk[KS_MLP_MAX_BUCKETS];

@@ -214,7 +214,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     const KsBucketDev& bk = p.bk[b];
     const float* sw3 = reinterpret_cast<const float*>(smem + C::OFF_W3) + b * H;
     const KsHeadDev& hd = p.head[b];
-    const float b3 = hd.b3;
+    const float b3 = hd.b3, out_sgn = hd.out_sgn, out_lo = hd.out_lo, out_add = hd.out_add;
     const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble, members of H / members columns
     const int ens_mask = members > 1 ? H / 16 / members - 1 : 0;     // member width is 32 or 64: a power-of-two chunk count
     const int tile0 = tm.tb[b], ne = tm.ne[b];
@@ -302,8 +302,9 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
             eta = fminf(__fdividef((float)members, esum), 1024.0f);
           } else {
             const float z = ((z0 + z1) + (z2 + z3)) + b3;
-            // eta = 1/e = 1 + exp(-z), guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
-            eta = fminf(1.0f + __expf(-z), 1024.0f);
+            // eta = 1/e = 1 + exp(-z) (utilisation output), or exp(max(z, 0)) (log-eta output; Q21);
+            // guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
+            eta = fminf(out_add + __expf(fmaxf(out_sgn * z, out_lo)), 1024.0f);
           }
           lat[(long long)s * bn + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
         }

@@ -207,7 +207,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     sb2[e] = __ldg(p.head[b].b2 + e);
     ks_bar_sync(2 + wg, 128);
     const KsHeadDev& hd = p.head[b];
-    const float b3 = hd.b3;
+    const float b3 = hd.b3, out_sgn = hd.out_sgn, out_lo = hd.out_lo, out_add = hd.out_add;
     const int members = ENS ? hd.members : 1;                                  // > 1: MLP ensemble (2, 4 or 8 members here)
     const int ens_mask = members > 1 ? H / 16 / members - 1 : 0;     // chunks per member - 1 (member width 32 .. 128)
     const int tile0 = tm.tb[b], ne = tm.ne[b];
@@ -292,9 +292,11 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
           ks_mbar_arrive(bars + BAR_Z_FREE + zb);
         }
         if (wg == 1 && valid) {
-          // eta = 1/e, guarded at e >= 2^-10 (Q3): 1 + exp(-z) for one head, k / sum of the members'
-          // sigmoids for an ensemble; Eq. 2 floor after eta
-          const float eta = fminf(members > 1 ? __fdividef((float)members, z) : 1.0f + __expf(-(z + b3)), 1024.0f);
+          // eta = 1/e, guarded at e >= 2^-10 (Q3): 1 + exp(-z) for one head with a utilisation output,
+          // exp(max(z, 0)) with a log-eta output (Q21), k / sum of the members' sigmoids for an
+          // ensemble; Eq. 2 floor after eta
+          const float eta = fminf(members > 1 ? __fdividef((float)members, z)
+                                              : out_add + __expf(fmaxf(out_sgn * (z + b3), out_lo)), 1024.0f);
           lat[(long long)s * bn + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
         }
       }

@@ -528,6 +528,7 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
     memset(b, 0, sizeof(b));
     for (int f = 0; f < A.n_fam; ++f) {
       b[f].family = fam_id[f];
+      b[f].model_slot = KS_SLOT_FAMILY;
       b[f].n = n_rows[f];
       b[f].col_dtype = KS_COL_I32;
       b[f].dtype_bytes = m.dtype_bytes;

@@ -12,7 +12,7 @@ from typing import List, Optional
 import numpy as np
 
 from . import binding as B
-from .workloads import Workload
+from workloads import Workload
 
 
 @dataclass
@@ -25,6 +25,7 @@ class DeviceBucket:
     head_dim: int
     step_off: object = None
     mult: object = None   # optional int32 per-row multiplicities (layer-homogeneous form)
+    model_slot: object = None   # efficiency-model slot (None = the family's)
 
     @property
     def n(self) -> int:
@@ -45,7 +46,7 @@ def to_device(w: Workload, device: str = "cuda:0") -> List[DeviceBucket]:
         cols = [torch.from_numpy(np.ascontiguousarray(c)).to(device) for c in b.cols]
         so = torch.from_numpy(np.ascontiguousarray(b.step_off, dtype=np.int32)).to(device) if b.step_off is not None else None
         mu = torch.from_numpy(np.ascontiguousarray(b.mult, dtype=np.int32)).to(device) if b.mult is not None else None
-        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu))
+        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu, b.model_slot))
     return out
 
 
@@ -62,7 +63,7 @@ def to_pinned(w: Workload) -> List[DeviceBucket]:
             cols = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in b.cols]
         so = torch.from_numpy(np.ascontiguousarray(b.step_off, dtype=np.int32)).pin_memory() if b.step_off is not None else None
         mu = torch.from_numpy(np.ascontiguousarray(b.mult, dtype=np.int32)).pin_memory() if b.mult is not None else None
-        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu))
+        out.append(DeviceBucket(b.family, cols, b.dtype_bytes, b.hq, b.hkv, b.head_dim, so, mu, b.model_slot))
     return out
 
 

@@ -14,7 +14,7 @@ from typing import Tuple
 
 import numpy as np
 
-from .workloads import Bucket, Workload
+from workloads import Bucket, Workload
 
 
 def shard_range(n: int, rank: int, world: int) -> Tuple[int, int]:
@@ -42,7 +42,8 @@ def shard_workload_by_steps(w: Workload, rank: int, world: int) -> Workload:
         so = np.asarray(b.step_off, dtype=np.int64)
         r0, r1 = int(so[s0]), int(so[s1])
         out.buckets.append(Bucket(b.family, [np.ascontiguousarray(c[r0:r1]) for c in b.cols], b.dtype_bytes, b.hq,
-                                  b.hkv, b.head_dim, (so[s0:s1 + 1] - r0).astype(np.int32)))
+                                  b.hkv, b.head_dim, (so[s0:s1 + 1] - r0).astype(np.int32),
+                                  None if b.mult is None else np.ascontiguousarray(b.mult[r0:r1]), b.model_slot))
     out.n_steps = s1 - s0
     if w.cfg_off is not None:
         out.cfg_off = (np.clip(np.asarray(w.cfg_off, dtype=np.int64), s0, s1) - s0).astype(np.int32)

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -58,7 +58,7 @@ def check_sampled(w, g, stride, tol, tier=None):
     worst = 0.0
     for b, gi in zip(w.buckets, g):
         rows = sample_rows(b.n, stride)
-        o = O.predict_bucket(b, w.specs, tier, head=heads.get(b.family), grid=grids.get(b.family), rows=rows)
+        o = O.predict_bucket(b, w.specs, tier, head=heads.get(b.slot), grid=grids.get(b.slot), rows=rows)
         e = rel(gi["lat"][:, rows], o["lat"]).max(initial=0)
         assert e <= tol, f"{w.name} family {b.family}: sampled latency rel err {e}"
         assert np.all(np.isfinite(gi["lat"])) and np.all(gi["lat"] >= np.float32(w.specs[0]["t0"]) * (1 - 1e-6))
@@ -95,7 +95,7 @@ def test_cfg3_full_tier_b(ks):
     for b, gi in zip(w.buckets, g):
         # interpolation never leaves [min, max] of the grid, so on EVERY row
         # max(t_roof / e_max, t0) <= t <= max(t_roof / e_min, t0)
-        gmin, gmax = float(w.grids[b.family].values.min()), float(w.grids[b.family].values.max())
+        gmin, gmax = float(w.grids[b.slot].values.min()), float(w.grids[b.slot].values.max())
         tr = gi["troof"].astype(np.float64)
         assert np.all(gi["lat"] >= np.maximum(tr / gmax, t0) * (1 - 2e-6))
         assert np.all(gi["lat"] <= np.maximum(tr / gmin, t0) * (1 + 2e-6))

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -38,9 +38,9 @@ def oracle_all(w, tier=None, rows=None):
     out = []
     for i, b in enumerate(w.buckets):
         r = None if rows is None else rows[i]
-        bnd = O.Bounded(w.bounded[b.family]) if (tier == W.TIER_A and b.family in getattr(w, "bounded", {})) else None
-        ens = O.Ensemble(w.ensembles[b.family]) if (tier == W.TIER_A and b.family in getattr(w, "ensembles", {})) else None
-        out.append(O.predict_bucket(b, w.specs, tier, head=heads.get(b.family), grid=grids.get(b.family), rows=r,
+        bnd = O.Bounded(w.bounded[b.slot]) if (tier == W.TIER_A and b.slot in getattr(w, "bounded", {})) else None
+        ens = O.Ensemble(w.ensembles[b.slot]) if (tier == W.TIER_A and b.slot in getattr(w, "ensembles", {})) else None
+        out.append(O.predict_bucket(b, w.specs, tier, head=heads.get(b.slot), grid=grids.get(b.slot), rows=r,
                                     bounded=bnd, ensemble=ens))
     return out
 
@@ -165,6 +165,87 @@ def test_tier_a_parity(ks, make):
     errs = run_and_check(ks, w, TOL_MLP)
     print(w.name, "tier A max rel err per bucket", errs)
     assert max(errs) < TOL_MLP
+
+
+@pytest.mark.parametrize("n_in,h", [(12, 128), (32, 256), (8, 64)])
+def test_tier_a_log_eta_output(ks, n_in, h):
+    # heads whose output is log eta: eta = exp(max(z, 0)) instead of 1 / sigmoid(z); same kernels,
+    # one branch-free epilogue.  Biases are spread so that both z < 0 (eta = 1: the bound) and z > 0 occur.
+    w = W.config2(n=20011, n_in=n_in, h=h)
+    rng = np.random.Generator(np.random.PCG64(300 + h))
+    w.heads = {f: W.make_head(rng, n_in, h, bias_std=0.3) for f in w.heads}
+    for hd in w.heads.values():
+        hd.out_mode = W.HEAD_LOG_ETA
+    B, D = ks
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        g = D.predict(ctx, w)
+        # back to the utilisation convention on the same loaded weights: a different prediction
+        for f in w.heads:
+            ctx.set_head_output(f, B.KS_HEAD_UTILISATION)
+        g0 = D.predict(ctx, w)
+    finally:
+        ctx.close()
+    o = oracle_all(w)
+    errs = [check_bucket(gi, oi, TOL_MLP, what=f"log-eta/bucket{i}") for i, (gi, oi) in enumerate(zip(g, o))]
+    print(n_in, h, "log-eta max rel err", errs)
+    at_bound = sum(int(np.sum(oi["lat"] == np.maximum(oi["troof"], w.specs[0]["t0"]))) for oi in o)
+    above = sum(int(np.sum(oi["lat"] > 1.01 * np.maximum(oi["troof"], w.specs[0]["t0"]))) for oi in o)
+    assert at_bound > 100 and above > 100                       # both regimes of max(z, 0) are exercised
+    for hd in w.heads.values():
+        hd.out_mode = W.HEAD_UTILISATION
+    o0 = oracle_all(w)
+    for gi, oi in zip(g0, o0):
+        check_bucket(gi, oi, TOL_MLP, what="utilisation after switching back")
+    assert any(np.max(rel_err(a["lat"], b_["lat"])) > 0.05 for a, b_ in zip(g, g0))
+
+
+@pytest.mark.parametrize("tier", [W.TIER_A, W.TIER_B, W.TIER_B_ROUTED, W.TIER_NONE])
+def test_model_slots_eight_paper_families(ks, tier):
+    # PAPER.md:199 / Tables 2 and 4: eta is learned per kernel family — GEMM, LM head, attention prefill and decode,
+    # RMSNorm, SiLU x Mul, RoPE, KV-cache write.  Eight buckets, eight model slots, eight different heads and grids
+    # in ONE call; two buckets of one decode family must get their own model.
+    w = W.config_families(n=40_000, tier=tier)
+    B, D = ks
+    ctx = B.Context(0)
+    try:
+        D.load_models(ctx, w)
+        db = D.to_device(w)
+        g = D.predict(ctx, w, dbuckets=db)
+        step, tot = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+        # a bucket whose slot holds no model is refused before anything runs
+        if tier != W.TIER_NONE:
+            bad = W.Bucket(W.FAM_GEMM, w.buckets[0].cols, model_slot=14)
+            import torch
+            lat = [torch.empty((1, bad.n), dtype=torch.float32, device="cuda:0")]
+            with pytest.raises(B.KsError) as ei:
+                ctx.predict_kernels(D.to_device(W.Workload("bad", [bad], w.specs, tier)), w.specs, tier, lat)
+            assert ei.value.status == B.KS_ESTATE
+    finally:
+        ctx.close()
+    heads = {s: O.Head(h) for s, h in w.heads.items()}
+    grids = {s: O.Grid(x) for s, x in w.grids.items()}
+    tol = TOL_F32 if tier in (W.TIER_B, W.TIER_NONE) else TOL_MLP
+    lats = []
+    for i, (b, gi) in enumerate(zip(w.buckets, g)):
+        o = O.predict_bucket(b, w.specs, tier, head=heads.get(b.slot), grid=grids.get(b.slot))
+        if tier == W.TIER_B_ROUTED:                               # in-hull rows: the fp32 path; routed rows: the bf16 path
+            assert np.array_equal(gi["tiles"], o["tiles"]) and np.array_equal(gi["waves"], o["waves"])
+            e, out = rel_err(gi["lat"], o["lat"]), o["routed"] == 1
+            assert e[:, ~out].max(initial=0) <= TOL_F32 and e[:, out].max(initial=0) <= TOL_MLP, f"slot {b.slot}"
+        else:
+            check_bucket(gi, o, tol, what=f"slot {b.slot}")
+        lats.append(gi["lat"][0])
+        if tier == W.TIER_A and b.model_slot is not None:
+            # priced with the decode family's default model instead, the bucket comes out different: the slot matters
+            other = O.predict_bucket(b, w.specs, tier, head=heads[w.buckets[0].slot if b.family == W.FAM_GEMM else
+                                                                  W.SLOT_ATTN_PREFILL if b.slot == W.SLOT_ATTN_DECODE else
+                                                                  W.SLOT_ATTN_DECODE if b.slot == W.SLOT_ATTN_PREFILL else
+                                                                  W.SLOT_RMSNORM if b.slot != W.SLOT_RMSNORM else W.SLOT_ROPE])
+            assert np.max(rel_err(gi["lat"], other["lat"])) > 2 * TOL_MLP
+    so, to = O.compose(lats, [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off)
+    assert np.max(rel_err(step[0], so)) <= TOL_F32 and np.max(rel_err(tot[0], to)) <= TOL_F32
 
 
 @pytest.mark.parametrize("n_in,h", [(8, 64), (8, 128), (12, 64), (12, 256), (32, 64), (32, 128), (8, 256)])
@@ -486,8 +567,8 @@ def test_ensemble_closed_forms_reductions_and_shapes(ks):
 def routed_oracle(w):
     heads = {f: O.Head(h) for f, h in w.heads.items()}
     grids = {f: O.Grid(g) for f, g in w.grids.items()}
-    return [O.predict_bucket(b, w.specs, W.TIER_B_ROUTED, head=heads.get(b.family), grid=grids[b.family],
-                             bounded=O.Bounded(w.bounded[b.family]) if b.family in w.bounded else None)
+    return [O.predict_bucket(b, w.specs, W.TIER_B_ROUTED, head=heads.get(b.slot), grid=grids[b.slot],
+                             bounded=O.Bounded(w.bounded[b.slot]) if b.slot in w.bounded else None)
             for b in w.buckets]
 
 

@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 
 from oracle import sched as S
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 TOL = {W.TIER_NONE: 1e-5, W.TIER_A: 1e-2}

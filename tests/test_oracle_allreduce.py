@@ -7,7 +7,7 @@ import ctypes as C
 import numpy as np
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 SPEC = W.spec_gb200(ar_alpha0=12e-6, ar_beta_eff=900e9)   # NVLink 5 per-direction datasheet bandwidth
 

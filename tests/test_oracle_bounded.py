@@ -7,7 +7,7 @@ import pytest
 from scipy.special import expit
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 SPEC = W.spec_gb200()
 

@@ -3,7 +3,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 ZERO = dict(W.STEP_PARAMS_ZERO)
 

@@ -13,7 +13,7 @@ from scipy.interpolate import RegularGridInterpolator
 from scipy.special import erf, expit
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 SPECD = W.spec_gb200()
 SPEC = O.make_spec(SPECD)

@@ -6,7 +6,7 @@ import numpy as np
 from scipy.special import erf, expit
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 SPEC = W.spec_gb200()
 

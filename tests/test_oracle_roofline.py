@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 SPEC = O.make_spec(W.spec_gb200())
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "roofline_cases.txt")

@@ -4,7 +4,7 @@ decided on integers (Q16)."""
 import numpy as np
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 
 def setup(n=4001):
@@ -30,10 +30,10 @@ def box_mask(bucket, grid):
 def test_routing_selects_per_row_between_the_two_tiers():
     w, heads, grids = setup()
     for b in w.buckets:
-        r = O.predict_bucket(b, w.specs, W.TIER_B_ROUTED, head=heads[b.family], grid=grids[b.family])
-        tb = O.predict_bucket(b, w.specs, W.TIER_B, grid=grids[b.family])
-        ta = O.predict_bucket(b, w.specs, W.TIER_A, head=heads[b.family])
-        inside = box_mask(b, w.grids[b.family])
+        r = O.predict_bucket(b, w.specs, W.TIER_B_ROUTED, head=heads[b.slot], grid=grids[b.slot])
+        tb = O.predict_bucket(b, w.specs, W.TIER_B, grid=grids[b.slot])
+        ta = O.predict_bucket(b, w.specs, W.TIER_A, head=heads[b.slot])
+        inside = box_mask(b, w.grids[b.slot])
         assert 0.80 < inside.mean() < 0.99                      # the recipe pushes ~5-10 % of the queries outside
         assert np.array_equal(r["routed"] == 0, inside)
         assert np.array_equal(r["lat"][0][inside], tb["lat"][0][inside])      # dense interior: measured grid

@@ -168,7 +168,7 @@ def test_step_rows_follow_the_mixed_step_pricing_rule():
 
 def test_price_steps_equals_hand_composition():
     from oracle import oracle as O
-    from paper_2606_28565_b200 import workloads as W
+    import workloads as W
     m = S.Model()
     spec = W.spec_gb200()
     batch = [(0, 1, 500), (1, 1, 2000), (2, 512, 1024)]
@@ -190,7 +190,7 @@ def test_price_steps_tp2_equals_hand_composition():
     # decoder (16 query heads, 4 KV heads, 7168 FFN columns, 65536 vocabulary rows per GPU) plus two ring all-reduces
     # per layer of S = T x hidden x 2 bytes (Eq. 3), every term priced one descriptor at a time
     from oracle import oracle as O
-    from paper_2606_28565_b200 import workloads as W
+    import workloads as W
     m = S.Model(tp=2)
     spec = W.spec_gb200()
     batch = [(0, 1, 500), (1, 1, 2000), (2, 512, 1024)]

@@ -3,7 +3,7 @@ t_embed): rows carry multiplicities; the weighted sum must equal the sum over th
 import numpy as np
 
 from oracle import oracle as O
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 
 def test_multiplicity_equals_repetition():

@@ -11,7 +11,7 @@ import pytest
 from oracle import sched as S
 from paper_2606_28565_b200 import binding as B
 from paper_2606_28565_b200 import build as ksbuild
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 
 @pytest.fixture(scope="module", autouse=True)

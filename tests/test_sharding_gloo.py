@@ -16,7 +16,7 @@ import torch.multiprocessing as mp
 
 from oracle import oracle as O
 from paper_2606_28565_b200 import sharding as S
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 
 def _free_port():

@@ -1,7 +1,7 @@
 """The seeded generators: shapes, determinism, and the structure DESIGN.md §4 promises."""
 import numpy as np
 
-from paper_2606_28565_b200 import workloads as W
+import workloads as W
 
 
 def test_deterministic_and_sized():

@@ -1,7 +1,7 @@
 """Seeded synthetic workload generators for the five BASELINE.json configs.
 
-This module is the ONLY code shared by the CPU oracle (``oracle/``) and the CUDA
-path (``paper_2606_28565_b200/csrc``).  It holds none of the method's arithmetic
+This package is the ONLY code shared by the CPU oracle (``oracle/``) and the CUDA
+path (``paper_2606_28565_b200/``); it belongs to neither and imports neither.  It holds none of the method's arithmetic
 (no FLOP/byte formulas, no roofline, no features, no MLP, no interpolation, no
 sums): it only draws kernel-instance descriptors, hardware-spec vectors, head
 weights, efficiency grids and step/config segmentations with
@@ -25,6 +25,11 @@ import numpy as np
 FAM_GEMM, FAM_GROUPED, FAM_ATTN, FAM_ELEMWISE, FAM_ALLREDUCE = 0, 1, 2, 3, 4
 FAM_NAMES = {0: "gemm", 1: "grouped_gemm", 2: "attention", 3: "elementwise", 4: "allreduce"}
 TIER_NONE, TIER_A, TIER_B, TIER_B_ROUTED = 0, 1, 2, 3
+# efficiency-model slots beyond the per-decode-family ones (slot = family for 0..4), after the families of the
+# paper's Tables 2 and 4; the library and the oracle wrapper treat a slot as an index
+SLOT_LM_HEAD, SLOT_ATTN_PREFILL, SLOT_ATTN_DECODE, SLOT_RMSNORM, SLOT_SILU_MUL, SLOT_ROPE, SLOT_KV_WRITE = 5, 6, 7, 8, 9, 10, 11
+SLOT_EMBEDDING, SLOT_RESIDUAL_ADD = 12, 13
+HEAD_UTILISATION, HEAD_LOG_ETA = 0, 1      # what an MLP head's output means
 # elementwise sub-operations (reading Q1)
 SUB_RMSNORM, SUB_SILU_MUL, SUB_ROPE, SUB_KV_WRITE, SUB_EMBED, SUB_RESADD = 0, 1, 2, 3, 4, 5
 N_EXPERTS = 8
@@ -41,6 +46,12 @@ class Bucket:
     head_dim: int = 0
     step_off: Optional[np.ndarray] = None  # CSR [n_steps+1] int32 into this bucket
     mult: Optional[np.ndarray] = None      # per-row multiplicity (layer-homogeneous form); None = ones
+    model_slot: Optional[int] = None       # efficiency-model slot that prices the bucket (eta is learned
+                                           # per kernel family, finer than the decode family); None = the family's slot
+
+    @property
+    def slot(self) -> int:
+        return self.family if self.model_slot is None else int(self.model_slot)
 
     @property
     def n(self) -> int:
@@ -58,6 +69,7 @@ class Head:
     b2: np.ndarray  # [h2]
     w3: np.ndarray  # [h2]
     b3: float
+    out_mode: int = 0   # HEAD_UTILISATION (sigmoid out) or HEAD_LOG_ETA (z = log eta)
 
 
 @dataclass
@@ -293,6 +305,49 @@ def config3(n: int = 4_194_304, seed: int = 2, routed: bool = False, n_in: int =
                     TIER_B_ROUTED if routed else TIER_B, grids=grids, heads=heads,
                     n_steps=n_steps, cfg_off=cfg_offsets(rng, n_steps, min(16, n_steps)),
                     step_params=dict(STEP_PARAMS_ZERO), seed=seed)
+
+
+# ----------------------------------------------------------------------------- the paper's model families
+ELEM_SPAN = ((12.0, 0.0, 0.0), (25.0, 0.0, 0.0))   # grids of one elementwise sub-op: log2 n on axis 0, two flat axes
+
+
+def config_families(n: int = 64_000, seed: int = 7, tier: int = TIER_A, n_in: int = 12, h: int = 128,
+                    log_eta: bool = False) -> Workload:
+    """Eight buckets, one per kernel family the paper learns eta for (Tables 2 and 4, PAPER.md:269-283,
+    :321-336): GEMM, LM head, attention prefill, attention decode, RMSNorm, SiLU x Mul, RoPE, KV-cache write — each
+    with its OWN head and grid (model slots; two buckets of one decode family carry different models).  Not a
+    BASELINE.json config: the parity case for slot dispatch.  log_eta: the heads' outputs are log eta."""
+    rng = _rng(seed)
+    k = max(n // 8, 1)
+    M, N, K = _gemm_rows(rng, k)
+    Ml = _log_uniform_int(rng, 1, 512, k)                                   # LM head: M = sequences in the step
+    Nl = np.full(k, VOCAB, np.int64)
+    Kl = GEMM_NK[rng.integers(0, 5, size=k)]
+    B_, q, kv = _attn_rows(rng, 4 * k)
+    pre = np.nonzero(q > 1)[0][:k]
+    dec = np.nonzero(q == 1)[0][:k]
+    ne = [_log_uniform_int(rng, 4096, 32 * 2 ** 20, k) for _ in range(4)]
+    at = dict(hq=32, hkv=8, head_dim=128)
+    buckets = [Bucket(FAM_GEMM, _i32(M, N, K)),
+               Bucket(FAM_GEMM, _i32(Ml, Nl, Kl), model_slot=SLOT_LM_HEAD),
+               Bucket(FAM_ATTN, _i32(B_[pre], q[pre], kv[pre]), model_slot=SLOT_ATTN_PREFILL, **at),
+               Bucket(FAM_ATTN, _i32(B_[dec], q[dec], kv[dec]), model_slot=SLOT_ATTN_DECODE, **at)]
+    for sub, slot, nel in zip((SUB_RMSNORM, SUB_SILU_MUL, SUB_ROPE, SUB_KV_WRITE),
+                              (SLOT_RMSNORM, SLOT_SILU_MUL, SLOT_ROPE, SLOT_KV_WRITE), ne):
+        buckets.append(Bucket(FAM_ELEMWISE, _i32(nel, np.full(k, sub)), model_slot=slot))
+    heads, grids = {}, {}
+    for b in buckets:
+        heads[b.slot] = make_head(rng, n_in, h)
+        heads[b.slot].out_mode = HEAD_LOG_ETA if log_eta else HEAD_UTILISATION
+        span = GEMM_SPAN if b.family == FAM_GEMM else ATTN_SPAN if b.family == FAM_ATTN else ELEM_SPAN
+        if b.slot == SLOT_LM_HEAD:
+            span = ((0.0, 16.0, 10.0), (9.0, 18.0, 14.0))                   # the vocabulary axis is its own span
+        grids[b.slot] = make_grid(rng, *span, dims=(32, 32, 32) if b.family != FAM_ELEMWISE else (32, 1, 1))
+    n_steps = max(1, k // 16)
+    for b in buckets:
+        b.step_off = uniform_step_offsets(rng, b.n, n_steps)
+    return Workload("families_8_slots", buckets, [spec_gb200()], tier, heads=heads, grids=grids, n_steps=n_steps,
+                    cfg_off=cfg_offsets(rng, n_steps, min(8, n_steps)), step_params=dict(STEP_PARAMS_CFG4), seed=seed)
 
 
 # ----------------------------------------------------------------------------- serving-step emission
