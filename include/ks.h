@@ -251,6 +251,10 @@ typedef struct {
   int32_t n_layers, hidden, ffn, vocab, hq, hkv, head_dim;
   int32_t dtype_bytes;             /* bytes per tensor element (1, 2 or 4) */
   int32_t tp;                      /* tensor-parallel degree; > 1 adds two all-reduces per layer */
+  int32_t fine_slots;              /* 0: every bucket is priced by the model slot of its decode family.  1: the paper's
+                                      finer families: the LM-head row gets its own bucket priced by
+                                      KS_SLOT_LM_HEAD, prefill chunks (n_new > 1) KS_SLOT_ATTN_PREFILL, decode requests
+                                      (n_new = 1) KS_SLOT_ATTN_DECODE; GEMM and elementwise rows keep their family's slot */
 } ks_model_desc;
 
 typedef struct {

@@ -281,6 +281,12 @@ class Model:
     head_dim: int = 128
     dtype_bytes: int = 2
     tp: int = 1
+    fine_slots: int = 0    # 1: the paper's finer model families, see step_rows
+
+
+# bucket key -> decode family.  Keys 0-4 are the decode families themselves; 5, 6, 7 are the model slots of the LM
+# head (decoded as a GEMM) and of prefill / decode attention (Q22; numbering of include/ks.h, restated)
+KEY_FAMILY = {0: 0, 2: 2, 3: 3, 4: 4, 5: 0, 6: 2, 7: 2}
 
 
 def shard(x: int, tp: int) -> int:
@@ -294,6 +300,9 @@ def step_rows(batch: Sequence[Tuple[int, int, int]], m: Model):
     Returns dict family -> (columns [list of int lists], multiplicities).  Families: 0 GEMM (M, N, K),
     2 attention (B, q, kv), 3 elementwise (n, subop), 4 all-reduce (S bytes, P) when tp > 1.
     Sub-operation codes as in DESIGN.md Q1: 0 RMSNorm, 1 SiLU*Mul, 2 RoPE, 3 KV write, 4 embedding.
+    With m.fine_slots the keys are MODEL SLOTS (eta is learned separately for "GEMM, the LM head,
+    attention prefill and decode, and the elementwise and memory kernels"): 0 the four layer GEMMs, 5 the LM-head row,
+    6 the prefill chunks (n_new > 1), 7 the decode requests (n_new = 1), 3 elementwise, 4 all-reduce.
     """
     T = sum(n for _, n, _ in batch)          # dense kernels run over the concatenated tokens
     n_seq = len(batch)                       # one logits row per scheduled request
@@ -312,6 +321,11 @@ def step_rows(batch: Sequence[Tuple[int, int, int]], m: Model):
     # history plus its own causal triangle (the family's pair count handles q x hist + triangle)
     attn = ([[1, n_new, hist + n_new] for _, n_new, hist in batch], [L] * n_seq)
     out = {0: gemm, 2: attn, 3: elem}
+    if m.fine_slots:
+        pre = [i for i, (_, n_new, _) in enumerate(batch) if n_new > 1]
+        dec = [i for i, (_, n_new, _) in enumerate(batch) if n_new == 1]
+        out = {0: (gemm[0][:4], gemm[1][:4]), 5: (gemm[0][4:], gemm[1][4:]),
+               6: ([attn[0][i] for i in pre], [L] * len(pre)), 7: ([attn[0][i] for i in dec], [L] * len(dec)), 3: elem}
     if m.tp > 1:
         out[4] = ([[T * m.hidden * m.dtype_bytes, m.tp]], [2 * L])
     return out
@@ -350,7 +364,8 @@ def price_steps(batches: Sequence[Sequence[Tuple[int, int, int]]], m: Model, spe
     from . import oracle as O
     import workloads as W   # dataclasses only (no arithmetic)
 
-    fams = [0, 2, 3] + ([4] if m.tp > 1 else [])
+    # bucket keys in the order the buckets are summed (with fine slots: keys are model slots, KEY_FAMILY decodes them)
+    fams = ([0, 6, 3] if m.fine_slots else [0, 2, 3]) + ([4] if m.tp > 1 else []) + ([5, 7] if m.fine_slots else [])
     cols = {f: [] for f in fams}
     mult = {f: [] for f in fams}
     off = {f: [0] for f in fams}
@@ -362,10 +377,11 @@ def price_steps(batches: Sequence[Sequence[Tuple[int, int, int]]], m: Model, spe
             off[f].append(len(cols[f]))
     lats, offs, mults = [], [], []
     for f in fams:
-        a = np.asarray(cols[f], np.int64).reshape(len(cols[f]), -1)
-        bk = W.Bucket(f, [np.ascontiguousarray(a[:, j]) for j in range(a.shape[1])], dtype_bytes=m.dtype_bytes,
-                      hq=shard(m.hq, m.tp) if f == 2 else 0, hkv=shard(m.hkv, m.tp) if f == 2 else 0,
-                      head_dim=m.head_dim if f == 2 else 0)
+        fam = KEY_FAMILY[f]
+        a = np.asarray(cols[f], np.int64).reshape(len(cols[f]), 2 if fam in (3, 4) else 3)
+        bk = W.Bucket(fam, [np.ascontiguousarray(a[:, j]) for j in range(a.shape[1])], dtype_bytes=m.dtype_bytes,
+                      hq=shard(m.hq, m.tp) if fam == 2 else 0, hkv=shard(m.hkv, m.tp) if fam == 2 else 0,
+                      head_dim=m.head_dim if fam == 2 else 0)
         head = O.Head(heads[f]) if (heads and f in heads) else None
         grid = O.Grid(grids[f]) if (grids and f in grids) else None
         lats.append(O.predict_bucket(bk, [spec], tier, head=head, grid=grid)["lat"][0])

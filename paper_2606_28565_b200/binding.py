@@ -63,7 +63,7 @@ class ks_sched_config(C.Structure):
 
 class ks_model_desc(C.Structure):
     _fields_ = [(k, C.c_int32) for k in ("n_layers", "hidden", "ffn", "vocab", "hq", "hkv", "head_dim",
-                                         "dtype_bytes", "tp")]
+                                         "dtype_bytes", "tp", "fine_slots")]
 
 
 class ks_sched_stats(C.Structure):
@@ -388,7 +388,7 @@ class Scheduler:
 
 def make_model_desc(m) -> ks_model_desc:
     """m: any object with n_layers, hidden, ffn, vocab, hq, hkv, head_dim, dtype_bytes, tp."""
-    return ks_model_desc(*[int(getattr(m, k)) for k, _ in ks_model_desc._fields_])
+    return ks_model_desc(*[int(getattr(m, k, 0)) for k, _ in ks_model_desc._fields_])
 
 
 def sim_run(ctx: "Context", scheds: Sequence[Scheduler], clock: np.ndarray, model, spec: dict, tier: int, params: dict,

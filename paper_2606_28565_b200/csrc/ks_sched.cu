@@ -354,15 +354,21 @@ ks_status ks_sched_destroy(ks_sched* s) {
 namespace {
 
 // One iteration's rows, packed for a single H2D copy.  Every array starts on a 16-byte boundary (the
-// alignment KS_MEM_DEVICE asks for).  Families in bucket order: GEMM, attention, elementwise[, all-reduce].
+// alignment KS_MEM_DEVICE asks for).  Buckets: GEMM, attention (all requests, or the prefill chunks when the model
+// asks for the paper's fine model families), elementwise[, all-reduce][, LM head, decode attention].
+constexpr int kSimBuckets = 6;
+struct SimBucket {
+  int family = 0, slot = KS_SLOT_FAMILY, n_cols = 0, cap_rows = 0;
+  bool packed = false;                   // attention: columns packed every iteration at their actual length
+  size_t col[3] = {}, mult = 0, off = 0;
+};
 struct Arena {
   char* host = nullptr;
   char* dev = nullptr;
   size_t bytes = 0;
-  // offsets into the arena
-  size_t col[4][3] = {}, mult[4] = {}, off[4] = {}, out = 0;
-  int cap_rows[4] = {};
-  int n_fam = 3;
+  SimBucket bk[kSimBuckets];
+  size_t out = 0;
+  int n_bk = 3;
 };
 
 size_t a16(size_t x) { return (x + 15) & ~(size_t)15; }
@@ -379,7 +385,7 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
   if (log_cap > 0 && (!step_replica || !step_time)) return KS_EINVAL;
   const ks_model_desc& m = *model;
   if (m.n_layers < 1 || m.hidden < 1 || m.ffn < 1 || m.vocab < 1 || m.hq < 1 || m.hkv < 1 || m.head_dim < 1 || m.tp < 1 ||
-      (m.dtype_bytes != 1 && m.dtype_bytes != 2 && m.dtype_bytes != 4))
+      (m.dtype_bytes != 1 && m.dtype_bytes != 2 && m.dtype_bytes != 4) || (m.fine_slots != 0 && m.fine_slots != 1))
     return KS_EINVAL;
   for (int r = 0; r < n_replicas; ++r) {
     if (!scheds[r] || std::isnan(clock[r])) return KS_EINVAL;
@@ -392,31 +398,46 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
   }
   if (n_replicas == 0) return KS_OK;
 
+  // PAPER.md:199 learns eta per kernel family — "GEMM, the LM head, attention prefill and decode, and the
+  // elementwise and memory kernels": with fine_slots the LM-head row and the decode requests get buckets (and model
+  // slots) of their own; the elementwise sub-operations keep one bucket (KS_MAX_BATCHES buckets per call).
+  const bool fine = m.fine_slots != 0;
   Arena A;
-  A.n_fam = m.tp > 1 ? 4 : 3;
-  const int n_cols[4] = {3, 3, 2, 2};
-  const int fam_id[4] = {KS_FAM_GEMM, KS_FAM_ATTN, KS_FAM_ELEMWISE, KS_FAM_ALLREDUCE};
   int64_t attn_rows = 0;
   for (int r = 0; r < n_replicas; ++r) attn_rows += scheds[r]->cfg.max_num_seqs;
-  A.cap_rows[0] = 5 * n_replicas;
-  A.cap_rows[1] = (int)std::min<int64_t>(attn_rows, std::numeric_limits<int32_t>::max() / 8);
-  A.cap_rows[2] = 6 * n_replicas;
-  A.cap_rows[3] = n_replicas;
-  if (attn_rows > A.cap_rows[1]) return KS_EUNSUPPORTED;
+  if (attn_rows > std::numeric_limits<int32_t>::max() / 8) return KS_EUNSUPPORTED;
+  enum { B_GEMM = 0, B_ATTN = 1, B_ELEM = 2 };
+  int B_AR = -1, B_LM = -1, B_DEC = -1, nb = 3;
+  auto setb = [&A](int i, int family, int slot, int n_cols, int cap, bool packed) {
+    A.bk[i].family = family; A.bk[i].slot = slot; A.bk[i].n_cols = n_cols; A.bk[i].cap_rows = cap; A.bk[i].packed = packed;
+  };
+  setb(B_GEMM, KS_FAM_GEMM, KS_SLOT_FAMILY, 3, (fine ? 4 : 5) * n_replicas, false);
+  setb(B_ATTN, KS_FAM_ATTN, fine ? KS_SLOT_ATTN_PREFILL : KS_SLOT_FAMILY, 3, (int)attn_rows, true);
+  setb(B_ELEM, KS_FAM_ELEMWISE, KS_SLOT_FAMILY, 2, 6 * n_replicas, false);
+  if (m.tp > 1) { B_AR = nb++; setb(B_AR, KS_FAM_ALLREDUCE, KS_SLOT_FAMILY, 2, n_replicas, false); }
+  if (fine) {
+    B_LM = nb++; setb(B_LM, KS_FAM_GEMM, KS_SLOT_LM_HEAD, 3, n_replicas, false);
+    B_DEC = nb++; setb(B_DEC, KS_FAM_ATTN, KS_SLOT_ATTN_DECODE, 3, (int)attn_rows, true);
+  }
+  A.n_bk = nb;
   // Fixed-size arrays first (a few rows per replica), the step times, and last the attention columns, which
   // are packed behind each other every iteration at their actual length: what an iteration reads is one
   // prefix of the arena, a few hundred KB at most.
   size_t at = 0;
-  for (int f = 0; f < A.n_fam; ++f) {
-    if (f != 1) {
-      for (int c = 0; c < n_cols[f]; ++c) { A.col[f][c] = at; at = a16(at + (size_t)A.cap_rows[f] * 4); }
-      A.mult[f] = at; at = a16(at + (size_t)A.cap_rows[f] * 4);
+  size_t packed_cap = 0;
+  for (int f = 0; f < nb; ++f) {
+    SimBucket& k = A.bk[f];
+    if (!k.packed) {
+      for (int c = 0; c < k.n_cols; ++c) { k.col[c] = at; at = a16(at + (size_t)k.cap_rows * 4); }
+      k.mult = at; at = a16(at + (size_t)k.cap_rows * 4);
+    } else {
+      packed_cap += 4 * a16((size_t)k.cap_rows * 4);
     }
-    A.off[f] = at; at = a16(at + (size_t)(n_replicas + 1) * 4);
+    k.off = at; at = a16(at + (size_t)(n_replicas + 1) * 4);
   }
   A.out = at; at = a16(at + (size_t)n_replicas * 4);
   const size_t attn_base = at;
-  at += 4 * a16((size_t)A.cap_rows[1] * 4);
+  at += packed_cap;
   A.bytes = at;
 
   cudaStream_t st = ks_internal_stream(ctx);
@@ -450,10 +471,10 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
   while (max_iters <= 0 || iters < max_iters) {
     const double tt0 = tnow();
     active.clear();
-    int n_rows[4] = {0, 0, 0, 0};
-    for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[0] = 0;
+    int n_rows[kSimBuckets] = {0, 0, 0, 0, 0, 0};
+    for (int f = 0; f < nb; ++f) I(A.bk[f].off)[0] = 0;
     // pass 1: every unfinished replica forms its batch
-    int64_t attn_total = 0;
+    int64_t attn_total[2] = {0, 0};                  // requests that go to bucket B_ATTN / B_DEC
     for (int r = 0; r < n_replicas; ++r) {
       ks_sched* s = scheds[r];
       if (sched_done(s)) continue;
@@ -466,15 +487,21 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
       }
       if (s->b_req.empty()) continue;
       active.push_back(r);
-      attn_total += (int64_t)s->b_req.size();
+      for (int32_t v : s->b_new) attn_total[(fine && v == 1) ? 1 : 0] += 1;
     }
     const int n_act = (int)active.size();
     if (n_act == 0) break;
     // pass 2: the batches' rows; the attention columns are packed at their actual length
-    const size_t attn_stride = a16((size_t)attn_total * 4);
-    for (int c = 0; c < 3; ++c) A.col[1][c] = attn_base + (size_t)c * attn_stride;
-    A.mult[1] = attn_base + 3 * attn_stride;
-    const size_t in_bytes = attn_base + 4 * attn_stride;
+    size_t pk = attn_base;
+    for (int f = 0; f < nb; ++f) {
+      SimBucket& k = A.bk[f];
+      if (!k.packed) continue;
+      const size_t stride = a16((size_t)attn_total[f == B_DEC ? 1 : 0] * 4);
+      for (int c = 0; c < 3; ++c) k.col[c] = pk + (size_t)c * stride;
+      k.mult = pk + 3 * stride;
+      pk += 4 * stride;
+    }
+    const size_t in_bytes = pk;
     const bool in_place = in_bytes <= (256u << 10);
     char* in_base = in_place ? A.host : A.dev;
     for (int ai = 0; ai < n_act; ++ai) {
@@ -484,62 +511,61 @@ extern "C" ks_status ks_sim_run(ks_ctx* ctx, ks_sched* const* scheds, double* cl
       for (int32_t v : s->b_new) T += v;
       const int32_t n_seq = (int32_t)s->b_req.size();
       {
-        int k = n_rows[0];
         const int32_t gM[5] = {T, T, T, T, n_seq};
         const int32_t gN[5] = {qkv_n, m.hidden, 2 * ffn_p, m.hidden, vocab_p};
         const int32_t gK[5] = {m.hidden, hq_p * m.head_dim, m.hidden, ffn_p, m.hidden};
-        for (int j = 0; j < 5; ++j, ++k) {
-          I(A.col[0][0])[k] = gM[j]; I(A.col[0][1])[k] = gN[j]; I(A.col[0][2])[k] = gK[j];
-          I(A.mult[0])[k] = j < 4 ? L : 1;
+        for (int j = 0; j < 5; ++j) {
+          const int f = (fine && j == 4) ? B_LM : B_GEMM;     // the LM head: a GEMM-shaped row with its own model
+          const int k = n_rows[f]++;
+          I(A.bk[f].col[0])[k] = gM[j]; I(A.bk[f].col[1])[k] = gN[j]; I(A.bk[f].col[2])[k] = gK[j];
+          I(A.bk[f].mult)[k] = j < 4 ? L : 1;
         }
-        n_rows[0] = k;
+      }
+      for (int32_t j = 0; j < n_seq; ++j) {
+        const int f = (fine && s->b_new[j] == 1) ? B_DEC : B_ATTN;   // decode: one new token over the cached context
+        const int k = n_rows[f]++;
+        I(A.bk[f].col[0])[k] = 1; I(A.bk[f].col[1])[k] = s->b_new[j]; I(A.bk[f].col[2])[k] = s->b_hist[j] + s->b_new[j];
+        I(A.bk[f].mult)[k] = L;
       }
       {
-        int k = n_rows[1];
-        for (int32_t j = 0; j < n_seq; ++j, ++k) {
-          I(A.col[1][0])[k] = 1; I(A.col[1][1])[k] = s->b_new[j]; I(A.col[1][2])[k] = s->b_hist[j] + s->b_new[j];
-          I(A.mult[1])[k] = L;
-        }
-        n_rows[1] = k;
-      }
-      {
-        int k = n_rows[2];
+        int k = n_rows[B_ELEM];
         const int32_t width[6] = {m.hidden, m.hidden, (hq_p + hkv_p) * m.head_dim, 2 * hkv_p * m.head_dim, ffn_p, m.hidden};
         const int32_t sub[6] = {4, 0, 2, 3, 1, 0};   // embedding, RMSNorm, RoPE, KV write, SiLU*Mul, final RMSNorm
         const int32_t mu[6] = {1, L, L, L, L, 1};
         for (int j = 0; j < 6; ++j, ++k) {
-          I(A.col[2][0])[k] = T * width[j]; I(A.col[2][1])[k] = sub[j]; I(A.mult[2])[k] = mu[j];
+          I(A.bk[B_ELEM].col[0])[k] = T * width[j]; I(A.bk[B_ELEM].col[1])[k] = sub[j]; I(A.bk[B_ELEM].mult)[k] = mu[j];
         }
-        n_rows[2] = k;
+        n_rows[B_ELEM] = k;
       }
-      if (A.n_fam == 4) {
-        const int k = n_rows[3]++;
-        I(A.col[3][0])[k] = T * m.hidden * m.dtype_bytes; I(A.col[3][1])[k] = m.tp; I(A.mult[3])[k] = 2 * L;
+      if (B_AR >= 0) {
+        const int k = n_rows[B_AR]++;
+        I(A.bk[B_AR].col[0])[k] = T * m.hidden * m.dtype_bytes; I(A.bk[B_AR].col[1])[k] = m.tp; I(A.bk[B_AR].mult)[k] = 2 * L;
       }
-      for (int f = 0; f < A.n_fam; ++f) I(A.off[f])[ai + 1] = n_rows[f];
-      inst_total += (int64_t)L * (4 + n_seq + 4 + (A.n_fam == 4 ? 2 : 0)) + 3;
+      for (int f = 0; f < nb; ++f) I(A.bk[f].off)[ai + 1] = n_rows[f];
+      inst_total += (int64_t)L * (4 + n_seq + 4 + (B_AR >= 0 ? 2 : 0)) + 3;
     }
 
     const double tt1 = tnow();
     // one copy in, one pass of the hot path on device pointers, one copy out
     if (!in_place && cudaMemcpyAsync(A.dev, A.host, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = KS_ECUDA; break; }
-    ks_desc_batch b[4];
-    const int32_t* offs[4];
+    ks_desc_batch b[kSimBuckets];
+    const int32_t* offs[kSimBuckets];
     memset(b, 0, sizeof(b));
-    for (int f = 0; f < A.n_fam; ++f) {
-      b[f].family = fam_id[f];
-      b[f].model_slot = KS_SLOT_FAMILY;
+    for (int f = 0; f < nb; ++f) {
+      const SimBucket& k = A.bk[f];
+      b[f].family = k.family;
+      b[f].model_slot = k.slot;
       b[f].n = n_rows[f];
       b[f].col_dtype = KS_COL_I32;
       b[f].dtype_bytes = m.dtype_bytes;
-      b[f].n_cols = n_cols[f];
-      if (fam_id[f] == KS_FAM_ATTN) { b[f].attn_hq = hq_p; b[f].attn_hkv = hkv_p; b[f].attn_head_dim = m.head_dim; }
-      for (int c = 0; c < n_cols[f]; ++c) b[f].cols[c] = in_base + A.col[f][c];
-      b[f].mult = reinterpret_cast<const int32_t*>(in_base + A.mult[f]);
-      offs[f] = reinterpret_cast<const int32_t*>(in_base + A.off[f]);
+      b[f].n_cols = k.n_cols;
+      if (k.family == KS_FAM_ATTN) { b[f].attn_hq = hq_p; b[f].attn_hkv = hkv_p; b[f].attn_head_dim = m.head_dim; }
+      for (int c = 0; c < k.n_cols; ++c) b[f].cols[c] = in_base + k.col[c];
+      b[f].mult = reinterpret_cast<const int32_t*>(in_base + k.mult);
+      offs[f] = reinterpret_cast<const int32_t*>(in_base + k.off);
       rows_total += n_rows[f];
     }
-    rc = ks_run_steps(ctx, b, offs, A.n_fam, spec, 1, tier, n_act, params, nullptr, 0, KS_MEM_DEVICE, nullptr,
+    rc = ks_run_steps(ctx, b, offs, nb, spec, 1, tier, n_act, params, nullptr, 0, KS_MEM_DEVICE, nullptr,
                       reinterpret_cast<float*>(out_base + A.out), nullptr);
     if (rc != KS_OK) break;
     const double tt2 = tnow();

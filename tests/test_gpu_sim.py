@@ -70,9 +70,10 @@ def replay_and_check(B, reps, model, spec, tier, params, heads, scheds, clock, s
     return worst
 
 
-@pytest.mark.parametrize("tier,pressure,tp,prefix", [(W.TIER_NONE, False, 1, False), (W.TIER_NONE, True, 4, False),
-                                                     (W.TIER_A, False, 1, False), (W.TIER_NONE, True, 1, True)])
-def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp, prefix):
+@pytest.mark.parametrize("tier,pressure,tp,prefix,fine",
+                         [(W.TIER_NONE, False, 1, False, 0), (W.TIER_NONE, True, 4, False, 0), (W.TIER_A, False, 1, False, 0),
+                          (W.TIER_NONE, True, 1, True, 0), (W.TIER_A, False, 1, False, 1), (W.TIER_A, True, 2, False, 1)])
+def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp, prefix, fine):
     B = ks
     reps = W.sim_replicas(n_replicas=5, n_requests=40, seed=70 + tp, pressure=pressure)
     if prefix:          # shared system prompts + a two-tier prefix cache
@@ -86,7 +87,7 @@ def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp, prefix):
             r.num_blocks = 64
             if prefix:
                 r.prefix_len = np.minimum(r.prefix_len, r.prompt_len).astype(np.int32)
-    model = W.ServingModel(tp=tp)
+    model = W.ServingModel(tp=tp, fine_slots=fine)
     spec = W.spec_gb200()
     params = W.STEP_PARAMS_CFG4
     heads = {}
@@ -94,7 +95,11 @@ def test_closed_loop_matches_oracle_replay(ks, tier, pressure, tp, prefix):
     try:
         if tier == W.TIER_A:
             rng = np.random.Generator(np.random.PCG64(1))
-            heads = {f: W.make_head(rng, 12, 128) for f in (W.FAM_GEMM, W.FAM_ATTN, W.FAM_ELEMWISE)}
+            # fine: the paper's finer families — LM head, prefill and decode attention priced by their
+            # own slots, each with a different head; the plain attention slot stays empty on purpose
+            slots = ((W.FAM_GEMM, W.SLOT_ATTN_PREFILL, W.FAM_ELEMWISE, W.SLOT_LM_HEAD, W.SLOT_ATTN_DECODE) if fine
+                     else (W.FAM_GEMM, W.FAM_ATTN, W.FAM_ELEMWISE))
+            heads = {f: W.make_head(rng, 12, 128) for f in slots}
             for f, h in heads.items():
                 ctx.load_heads(f, h)
         scheds = make_scheds(B, reps)

@@ -335,3 +335,32 @@ def test_prefix_cache_invariants_on_random_traces(seed):
     assert sum(s.cached_tokens) > 0
     if sum(s.n_preempt) == 0:                            # every token is either computed once or served from the cache
         assert s.tokens_scheduled + sum(s.cached_tokens) == sum(p + o - 1 for p, o in zip(P, O))
+
+
+def test_fine_slots_regroup_the_same_rows():
+    """eta per family incl. "the LM head, attention prefill and decode".  With fine_slots the step's rows
+    are the same rows, grouped by model slot: 0 the four layer GEMMs, 5 the LM head, 6 prefill chunks, 7 decodes."""
+    import workloads as W
+    from oracle import oracle as O
+    m0, m1 = S.Model(n_layers=3), S.Model(n_layers=3, fine_slots=1)
+    batch = [(0, 1, 700), (1, 300, 0), (2, 1, 45), (3, 212, 512)]        # two decodes, two prefill chunks
+    r0, r1 = S.step_rows(batch, m0), S.step_rows(batch, m1)
+    assert sorted(r1) == [0, 3, 5, 6, 7]
+    assert r1[0][0] == r0[0][0][:4] and r1[5][0] == [r0[0][0][4]] == [[4, m0.vocab, m0.hidden]] and r1[5][1] == [1]
+    assert r1[6][0] == [[1, 300, 300], [1, 212, 724]] and r1[7][0] == [[1, 1, 701], [1, 1, 46]]
+    assert r1[6][1] == [3, 3] and r1[7][1] == [3, 3] and r1[3] == r0[3]
+    # priced with ONE head for GEMM + LM head and ONE for both attention slots, the regrouping changes nothing ...
+    rng = np.random.Generator(np.random.PCG64(3))
+    hg, ha, he, hl = (W.make_head(rng, 12, 64) for _ in range(4))
+    spec, par = W.spec_gb200(), W.STEP_PARAMS_CFG4
+    batches = [batch, [(0, 1, 9)], [(5, 64, 0)]]                          # a decode-only and a prefill-only step too
+    coarse = S.price_steps(batches, m0, spec, W.TIER_A, par, heads={0: hg, 2: ha, 3: he})
+    same = S.price_steps(batches, m1, spec, W.TIER_A, par, heads={0: hg, 5: hg, 6: ha, 7: ha, 3: he})
+    assert np.allclose(same, coarse, rtol=1e-12, atol=0)
+    # ... and a different LM head moves every step by exactly the LM-head kernel's change (multiplicity 1)
+    fine = S.price_steps(batches, m1, spec, W.TIER_A, par, heads={0: hg, 5: hl, 6: ha, 7: ha, 3: he})
+    for i, b in enumerate(batches):
+        row = W.Bucket(W.FAM_GEMM, W._i32([len(b)], [m0.vocab], [m0.hidden]))
+        d = (O.predict_bucket(row, [spec], W.TIER_A, head=O.Head(hl))["lat"][0, 0]
+             - O.predict_bucket(row, [spec], W.TIER_A, head=O.Head(hg))["lat"][0, 0])
+        assert abs((fine[i] - coarse[i]) - d) <= 1e-12 * coarse[i]

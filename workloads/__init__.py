@@ -568,6 +568,7 @@ class ServingModel:
     head_dim: int = HEAD_DIM
     dtype_bytes: int = 2
     tp: int = 1
+    fine_slots: int = 0    # 1: LM head, prefill and decode attention are priced by their own model slots
 
 
 @dataclass
