@@ -28,6 +28,7 @@ constexpr int kS = 32;                 // steps per chunk (one CTA); small probl
 constexpr int kSmallS = 8;
 constexpr int kSmallSteps = 16384;     // n_steps x n_specs up to which the small chunk is used
 constexpr int kCapFloats = 12032;      // staged floats per CTA (47 KiB + slack): four CTAs per SM
+constexpr int kCapFloatsBig = 18432;   // ... for workloads whose average chunk does not fit that: 72 KiB, three CTAs per SM
 constexpr int kSlackFloats = 192;      // readable floats behind the staged data (masked lanes of the last step)
 
 KS_DEV int mA_n(int n, int lane) { return n - lane; }   // elements 32 r < n - lane belong to this lane
@@ -85,7 +86,7 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
       used += len[b];
     }
   }
-  if (used > kCapFloats) staged = false;                          // very long steps: straight from global
+  if (used > p.cap_floats) staged = false;                        // very long steps: straight from global
   // Multiplicities (shared by all specs) ride in the same cp.async group behind the latencies when they fit:
   // a chunk then costs one trip to memory for all buckets instead of one per bucket inside the reduction —
   // which matters when the arrays live in pinned host memory (the simulation loop reads its arena in place).
@@ -108,7 +109,7 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
         mused += mlen[b];
       }
     }
-    if (((used + 3) & ~3) + mused > kCapFloats) mstaged = false;
+    if (((used + 3) & ~3) + mused > p.cap_floats) mstaged = false;
   }
   if (staged) {
     int base = 0;
@@ -335,8 +336,16 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
                                                                                      ks_compose_kernel<8, false, kS>;
       if (weighted) kern = p.n_batches <= 4 ? ks_compose_kernel<4, true, kS> : ks_compose_kernel<8, true, kS>;
     }
-    const size_t smem = (size_t)(kCapFloats + kSlackFloats) * 4;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the staging buffer: 47 KiB (four CTAs per SM) unless an average chunk would not fit it (cfg5: ~395 rows per
+    // step), then 72 KiB (three CTAs per SM) — a chunk that does not fit is summed from global memory, far slower
+    long long rows = 0;
+    for (int b = 0; b < p.n_batches; ++b) rows += p.spec_stride[b];
+    const bool big = (double)rows / (double)p.n_steps * ks > 0.85 * kCapFloats;
+    KsComposeParams q = p;
+    q.cap_floats = big ? kCapFloatsBig : kCapFloats;
+    const size_t smem = (size_t)(q.cap_floats + kSlackFloats) * 4;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)((kCapFloatsBig + kSlackFloats) * 4));
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)n_chunks);
@@ -348,7 +357,7 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    e = cudaLaunchKernelEx(&cfg, kern, p);
+    e = cudaLaunchKernelEx(&cfg, kern, q);
     if (e != cudaSuccess) return e;
     if (launches) *launches += 1;
   }

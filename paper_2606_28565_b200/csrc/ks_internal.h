@@ -98,6 +98,7 @@ struct KsComposeParams {
   const int32_t* mult[KS_MAX_BATCHES];    // optional per-row multiplicities (nullptr = ones)
   int64_t spec_stride[KS_MAX_BATCHES];
   int32_t n_batches, n_steps, n_specs, n_cfg;
+  int32_t cap_floats;                     // staging buffer of a CTA in floats (set by the launcher)
   ks_step_params sp;
   const int32_t* cfg_off;
   float* step_lat;   // [n_specs][n_steps]

@@ -156,6 +156,60 @@ def test_tier_b_nodes_exact_and_flat_axes(ks):
     check_bucket(g2[0], oracle_all(w2)[0], TOL_F32, what="elementwise grid")
 
 
+def _tierb_bucket(rng, fam, n, lo, hi, dtype=np.int32):
+    """n rows whose axis values straddle the span [lo, hi] (log2), with zeros, ones, exact span ends and huge values."""
+    lo, hi = np.asarray(lo, np.float64), np.asarray(hi, np.float64)
+    x = rng.uniform(lo[None, :] - 1.5, hi[None, :] + 1.5, size=(n, 3))
+    v = np.maximum(np.rint(np.exp2(x)), 0).astype(np.int64)
+    k = min(n, 12)
+    # (the CTA count B must stay below 2^31, DESIGN.md Q1: the huge values go to the third axis, K or kv, which B ignores)
+    special = np.array([0, 1, 2, 3, 2 ** 31 - 1, 2 ** 24 + 1, 2 ** 24 - 1, 255, 256, 257, 65535, 65537])[:k]
+    for a in range(3):
+        v[:k, a] = np.roll(np.minimum(special, 2 ** 31 - 1 if a == 2 else 65537), a)
+        if n > 20:   # the exact span ends (integers there are hull corners) and one beyond each
+            for j, e in enumerate((np.ceil(2.0 ** lo[a]), np.floor(2.0 ** hi[a]), np.floor(2.0 ** hi[a]) + 1)):
+                v[12 + 3 * a + j if 12 + 3 * a + j < n else 0, a] = int(e)
+    v = np.minimum(v, 2 ** 31 - 1)
+    if fam == W.FAM_ATTN:
+        kw = dict(hq=24, hkv=3, head_dim=96)
+    else:
+        kw = {}
+    if dtype == np.float32:          # F32 columns hold exact integers < 2^24
+        v = np.minimum(v, 2 ** 24 - 1)
+    return W.Bucket(fam, [np.ascontiguousarray(v[:, a], dtype=dtype) for a in range(3)], **kw)
+
+
+@pytest.mark.parametrize("dims,n_specs,dtype,n", [((7, 33, 5), 1, np.int32, 8191), ((2, 2, 300), 3, np.int32, 4097),
+                                                  ((32, 1, 31), 1, np.float32, 5), ((1, 64, 64), 2, np.float32, 12289),
+                                                  ((16, 16, 16), 1, np.int32, 1), ((2, 2, 8192), 1, np.int32, 3000)])
+def test_tier_b_kernel_edge_cases(ks, dims, n_specs, dtype, n):
+    # ks_tierb.cu away from the 32^3 / one-spec / int32 configuration: odd and flat dims (the zero tail behind the grid is
+    # what the corners one past an axis read), fractional and large lo, several specs (the 512-thread instance), fp32
+    # columns, ragged tails of 1..3 rows, values 0, 1, 2^31-1, span ends; five buckets = two launches of <= 4 buckets
+    B, D = ks
+    rng = np.random.Generator(np.random.PCG64(hash((dims, n_specs, n)) % 1000))
+    spans = {W.FAM_GEMM: ((0.5, 3.25, 9.0), (11.75, 14.0, 20.5)), W.FAM_ATTN: ((0.0, 0.0, 1.3), (7.0, 12.6, 17.0))}
+    specs = W.sweep_specs(rng, n_specs)
+    specs[0].update(tile_m=96, tile_n=1, ctas_per_sm=3)           # divisors that are not powers of two, and a divisor of one
+    buckets, grids = [], {}
+    for i, fam in enumerate((W.FAM_GEMM, W.FAM_ATTN, W.FAM_GEMM, W.FAM_ATTN, W.FAM_GEMM)):
+        lo, hi = spans[fam]
+        slot = 8 + i                                               # five slots, five different grids
+        b = _tierb_bucket(rng, fam, n if i != 3 else max(1, n // 3), lo, hi, dtype)
+        b.model_slot = slot
+        buckets.append(b)
+        # (fp32 interpolation holds 1e-5 RELATIVE only where e is not tiny next to large neighbours: config-like values;
+        # the last bucket's grid is a constant below the 2^-10 guard, so every row there comes out at t_roof * 2^10)
+        vals = W.make_grid(rng, lo, hi, dims=dims).values if i < 4 else np.full(dims, 2.0 ** -12, np.float32)
+        for a in range(3):          # an axis of hundreds of nodes asks more of an fp32 coordinate than 1e-5 leaves: flat there
+            if dims[a] > 64:
+                vals = np.ascontiguousarray(np.broadcast_to(np.take(vals, [0], axis=a), dims))
+        grids[slot] = W.Grid(np.asarray(dims, np.int32), np.asarray(lo, np.float32), np.asarray(hi, np.float32), vals)
+    w = W.Workload("tierb_edges", buckets, specs, W.TIER_B, grids=grids)
+    errs = run_and_check(ks, w, TOL_F32)
+    print(dims, n_specs, n, "tier-B edge max rel err", errs)
+
+
 # ------------------------------------------------------------------ Tier A (S3, S4a)
 @pytest.mark.parametrize("make", [lambda: W.config1(), lambda: W.config2(n=40013),
                                   lambda: W.config5(n_rows=12001, n_specs=3, n_layers=4),
