@@ -1,5 +1,5 @@
-// ks_mlp_common.cuh — pieces shared by the two Tier-A kernels (ks_mlp.cu: slot kernel, used for
-// H = 256; ks_mlp_ws.cu: warp-specialized pipeline, H <= 128).
+// ks_mlp_common.cuh — pieces shared by the two Tier-A kernels (ks_mlp_ws.cu: H <= 128; ks_mlp_ws256.cu:
+// H = 256; both warp-specialized tcgen05 pipelines; ks_mlp.cu picks one by head width).
 #pragma once
 #include "ks_internal.h"
 #include "ks_ptx.cuh"
