@@ -24,8 +24,9 @@
 //        read (the next row / plane, or the zero tail behind the grid) with weight zero, no second clamp;
 //  * the grid's hull test of density routing (Q16) appends out-of-hull rows with one atomic
 //    per warp and tile.
-// What bounds it (profiles/README.md): eight random 4-byte shared-memory gathers per query at 3.8
-// wavefronts each, next to ~120 instructions per query — 0.53 of the HBM copy rate at large sizes.
+// Where it stands (profiles/README.md): 0.53 of the HBM copy rate at large sizes, ~120 instructions and
+// eight random 4-byte shared-memory gathers (3.8 wavefronts each) per query; a control run against conflict-free
+// 2x2x2 grids gains 3 %: no single pipe bounds it, the warps' gather and arithmetic phases load the pipes in turn.
 #include "ks_internal.h"
 #include "ks_ptx.cuh"
 
@@ -39,7 +40,6 @@ KS_DEV F2 mul2(F2 a, F2 b) { F2 r; ks_mul2(r.x, r.y, a.x, a.y, b.x, b.y); return
 KS_DEV F2 fma2(F2 a, F2 b, F2 c) { F2 r; ks_fma2(r.x, r.y, a.x, a.y, b.x, b.y, c.x, c.y); return r; }
 KS_DEV F2 sub2(F2 a, F2 b) { return fma2(b, bc2(-1.0f), a); }    // a - b, exact like FADD (packed adds take no negation)
 KS_DEV F2 max2(F2 a, F2 b) { return mk2(fmaxf(a.x, b.x), fmaxf(a.y, b.y)); }
-KS_DEV F2 min2(F2 a, F2 b) { return mk2(fminf(a.x, b.x), fminf(a.y, b.y)); }
 // a + 2^23 rounded toward -inf: for 0 <= a < 2^22 the low mantissa bits of the result hold floor(a)
 KS_DEV F2 floor_magic2(F2 a) {
   F2 r;
