@@ -108,3 +108,22 @@ struct KsComposeParams {
 cudaStream_t ks_internal_stream(ks_ctx* c);
 cudaError_t ks_internal_set_device(ks_ctx* c);
 cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_t st, int* launches);
+
+// Every libks kernel is launched with programmatic stream serialization and opens with
+//   griddepcontrol.launch_dependents;  cudaGridDependencySynchronize();
+// so its launch latency and CTA scheduling overlap the tail of whatever kernel precedes it on the stream, while
+// nothing is read or written before that kernel has completed and flushed (the same ordering as a plain launch).
+template <typename Kern, typename Params>
+inline cudaError_t ks_launch_pdl(Kern kern, unsigned blocks, unsigned threads, size_t smem, cudaStream_t st, const Params& p) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks);
+  cfg.blockDim = dim3(threads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, p);
+}

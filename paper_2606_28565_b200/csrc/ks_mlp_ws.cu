@@ -408,7 +408,8 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
   const int tid = threadIdx.x;
   const int warp = tid >> 5;
 
-  ks_launch_dependents();     // the step kernel's launch overlaps this kernel (it waits for our completion itself)
+  ks_launch_dependents();     // the step kernel's launch overlaps this kernel (it waits for our completion itself) ...
+  cudaGridDependencySynchronize();   // ... as we wait for the kernel before us (ks_launch_pdl)
   if (tid == 32) tile_map_init(p, tmp);
   if (tid == 0) {
     ks_mbar_init(bars + BAR_W, 1);
@@ -485,8 +486,7 @@ cudaError_t launch_ws(const KsMlpParams& p, int num_sms, cudaStream_t st) {
   auto kern = ks_mlp_ws_kernel<NIN, H>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  kern<<<grid, kWsThreads, C::SMEM_BYTES, st>>>(p);
-  return cudaGetLastError();
+  return ks_launch_pdl(kern, grid, kWsThreads, C::SMEM_BYTES, st, p);
 }
 
 }  // namespace

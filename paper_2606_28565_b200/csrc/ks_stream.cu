@@ -141,7 +141,8 @@ KS_DEV float trilinear(const int* v, const KsGridDev& g, const float* __restrict
 template <int FAM, int TIER, bool F32, bool ONE>
 __global__ void __launch_bounds__(TIER == KS_TIER_B ? (FAM == KS_FAM_GROUPED_GEMM ? 512 : 1024) : 256)
 ks_stream_kernel(const __grid_constant__ KsStreamParams p) {
-  ks_launch_dependents();     // a step kernel launched behind this one may be scheduled now (it waits for us itself)
+  ks_launch_dependents();     // the next kernel of the stream may be scheduled now (it waits for us itself) ...
+  cudaGridDependencySynchronize();   // ... as we wait for the one before us (ks_launch_pdl)
   constexpr int NC = NCols<FAM>::v;
   extern __shared__ __align__(128) float sgrid[];
 
@@ -263,7 +264,7 @@ cudaError_t launch_ft(const KsStreamParams& p, int num_sms, cudaStream_t st) {
                     : (one ? ks_stream_kernel<FAM, TIER, false, true> : ks_stream_kernel<FAM, TIER, false, false>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<blocks, threads, smem, st>>>(p);
+    return ks_launch_pdl(kern, blocks, threads, smem, st, p);
   } else {
     const int threads = 256;
     int blocks = (n4 + threads - 1) / threads;
@@ -272,7 +273,9 @@ cudaError_t launch_ft(const KsStreamParams& p, int num_sms, cudaStream_t st) {
     const bool one = p.n_specs == 1;
     auto kern = f32 ? (one ? ks_stream_kernel<FAM, TIER, true, true> : ks_stream_kernel<FAM, TIER, true, false>)
                     : (one ? ks_stream_kernel<FAM, TIER, false, true> : ks_stream_kernel<FAM, TIER, false, false>);
-    kern<<<blocks, threads, 0, st>>>(p);
+    // launched programmatically dependent (ks_launch_pdl): measured on cfg4a, back to back: GEMM 37.0 -> 35.3 us,
+    // attention 16.5 -> 13.9 us, elementwise 31.1 -> 29.1 us
+    return ks_launch_pdl(kern, blocks, threads, 0, st, p);
   }
   return cudaGetLastError();
 }
@@ -316,6 +319,7 @@ KS_DEV void small_row(const KsStreamSmallParams& p, const KsBucketDev& bk, const
 
 __global__ void __launch_bounds__(256) ks_stream_small_kernel(const __grid_constant__ KsStreamSmallParams p) {
   ks_launch_dependents();
+  cudaGridDependencySynchronize();
   const int g = blockIdx.x * 256 + threadIdx.x;
   if (g >= p.row_begin[p.n_buckets]) return;
   int b = 0;
@@ -336,8 +340,7 @@ __global__ void __launch_bounds__(256) ks_stream_small_kernel(const __grid_const
 cudaError_t ks_launch_stream_small(const KsStreamSmallParams& p, cudaStream_t st) {
   const int n = p.row_begin[p.n_buckets];
   if (n <= 0) return cudaSuccess;
-  ks_stream_small_kernel<<<(n + 255) / 256, 256, 0, st>>>(p);
-  return cudaGetLastError();
+  return ks_launch_pdl(ks_stream_small_kernel, (n + 255) / 256, 256, 0, st, p);
 }
 
 cudaError_t ks_launch_stream(const KsStreamParams& p, int num_sms, cudaStream_t st) {

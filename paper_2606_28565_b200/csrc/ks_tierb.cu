@@ -313,7 +313,8 @@ KS_DEV void run_bucket(const KsTierBParams& p, const int b, const int tile0, con
 
 template <bool F32, bool ONE, int NT>
 __global__ void __launch_bounds__(NT, 1) ks_tierb_kernel(const __grid_constant__ KsTierBParams p) {
-  ks_launch_dependents();     // a step kernel launched behind this one may be scheduled now (it waits for us itself)
+  ks_launch_dependents();     // the next kernel of the stream may be scheduled now (it waits for us itself) ...
+  cudaGridDependencySynchronize();   // ... as we wait for the one before us (ks_launch_pdl)
   extern __shared__ __align__(128) float sgrid_f[];
   __shared__ __align__(8) uint64_t bar;
   const uint32_t sgrid = ks_smem_u32(sgrid_f);
@@ -382,6 +383,5 @@ cudaError_t ks_launch_tierb(const KsTierBParams& p, int num_sms, cudaStream_t st
           : (f32 ? ks_tierb_kernel<true, false, 512> : ks_tierb_kernel<false, false, 512>);
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  kern<<<blocks, nt, smem, st>>>(q);
-  return cudaGetLastError();
+  return ks_launch_pdl(kern, blocks, nt, smem, st, q);
 }
