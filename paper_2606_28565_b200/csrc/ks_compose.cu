@@ -287,7 +287,11 @@ ks_compose_kernel(const __grid_constant__ KsComposeParams p) {
   else reduce_all(std::false_type{});
 }
 
-__global__ void __launch_bounds__(256)
+constexpr int kTotThreads = 1024;
+
+// One CTA per (spec, configuration): 1024 threads, four independent loads in flight per thread (the launch is a
+// latency chain behind the step kernel: a 256-thread CTA walking its ~1,500 steps six dependent loads deep cost 5 us).
+__global__ void __launch_bounds__(kTotThreads)
 ks_cfg_total_kernel(const __grid_constant__ KsComposeParams p) {
   const int cfg = blockIdx.x % p.n_cfg;
   const int spec = blockIdx.x / p.n_cfg;
@@ -296,17 +300,24 @@ ks_cfg_total_kernel(const __grid_constant__ KsComposeParams p) {
   cudaGridDependencySynchronize();
   const int beg = __ldg(p.cfg_off + cfg), end = __ldg(p.cfg_off + cfg + 1);
   const float* sl = p.step_lat + (long long)spec * p.n_steps;
-  double acc = 0.0;
-  for (int s = beg + threadIdx.x; s < end; s += blockDim.x) acc += (double)sl[s];
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  int s = beg + (int)threadIdx.x;
+  for (; s + 3 * kTotThreads < end; s += 4 * kTotThreads) {
+    const float x0 = sl[s], x1 = sl[s + kTotThreads], x2 = sl[s + 2 * kTotThreads], x3 = sl[s + 3 * kTotThreads];
+    a0 += (double)x0; a1 += (double)x1; a2 += (double)x2; a3 += (double)x3;
+  }
+  for (; s < end; s += kTotThreads) a0 += (double)sl[s];
+  double acc = (a0 + a1) + (a2 + a3);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  __shared__ double part[8];
+  __shared__ double part[kTotThreads / 32];
   if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
   __syncthreads();
-  if (threadIdx.x == 0) {
-    double t = 0.0;
-    for (int w = 0; w < 8; ++w) t += part[w];
-    p.cfg_lat[(long long)spec * p.n_cfg + cfg] = (float)t;
+  if (threadIdx.x < 32) {
+    double t = part[threadIdx.x];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (threadIdx.x == 0) p.cfg_lat[(long long)spec * p.n_cfg + cfg] = (float)t;
   }
 }
 
@@ -364,7 +375,7 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
   if (p.n_cfg > 0 && p.n_specs > 0 && p.cfg_lat) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(p.n_cfg * p.n_specs));
-    cfg.blockDim = dim3(256);
+    cfg.blockDim = dim3(kTotThreads);
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // hide this launch under the step kernel's tail
