@@ -45,7 +45,8 @@ extern "C" {
 
 typedef struct ks_ctx ks_ctx;   /* opaque; owns device copies of heads and grids + workspace */
 
-typedef enum { KS_OK = 0, KS_EINVAL = 1, KS_ENOMEM = 2, KS_ECUDA = 3, KS_ESTATE = 4, KS_EUNSUPPORTED = 5 } ks_status;
+typedef enum { KS_OK = 0, KS_EINVAL = 1, KS_ENOMEM = 2, KS_ECUDA = 3, KS_ESTATE = 4, KS_EUNSUPPORTED = 5,
+               KS_ELIMIT = 6 /* a fixed capacity was exceeded (ks_predict_routed_static) */ } ks_status;
 typedef enum { KS_FAM_GEMM = 0, KS_FAM_GROUPED_GEMM = 1, KS_FAM_ATTN = 2, KS_FAM_ELEMWISE = 3, KS_FAM_ALLREDUCE = 4,
                KS_FAM_COUNT = 5 } ks_family;
 typedef enum { KS_TIER_NONE = 0, KS_TIER_A = 1, KS_TIER_B = 2, KS_TIER_B_ROUTED = 3 } ks_tier;
@@ -189,6 +190,25 @@ KS_API ks_status ks_predict_kernels(ks_ctx *ctx, const ks_desc_batch *batches, i
                              const ks_hw_spec *specs, int n_specs, ks_tier tier, ks_mem_space space,
                              float *const *latency, int32_t *const *tiles, int32_t *const *waves,
                              float *const *t_roof);
+
+/* Density-routed prediction that ALLOCATES NOTHING: ks_predict_kernels(..., KS_TIER_B_ROUTED, KS_MEM_DEVICE, ...)
+ * for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).
+ * The routing pass (Q16) needs scratch memory: per bucket, the list of the rows outside the
+ * grid's hull and its length.  ks_predict_kernels keeps them in the context's grow-only workspace; this entry point
+ * keeps them in ONE fixed array in the library's device image (4 MiB + 4 KiB, held by every GPU that loads libks
+ * until the process exits) and calls no cudaMalloc / cudaFree or allocating library routine.
+ *   Arguments, layouts, validation and results are those of ks_predict_kernels with tier = KS_TIER_B_ROUTED and
+ *   space = KS_MEM_DEVICE (columns and outputs are DEVICE pointers, 16-byte aligned); the same kernels run.
+ *   Limit: the rows of all buckets other than KS_FAM_ALLREDUCE (which is never routed) must total at most
+ *   KS_STATIC_ROUTE_MAX_ROWS; beyond it the call returns KS_ELIMIT and nothing is enqueued or written.
+ *   The array is shared by every context, stream and call on a device and keeps the last call's contents: each
+ *   call clears the list lengths it uses (stream-ordered) before its kernels run, so calls in sequence on one
+ *   stream are safe; calls that OVERLAP on the GPU (two streams, two contexts on one device) race on it and must be
+ *   ordered by the caller.  The first call on a device resolves the array's device address (no allocation). */
+#define KS_STATIC_ROUTE_MAX_ROWS (1 << 20)
+KS_API ks_status ks_predict_routed_static(ks_ctx *ctx, const ks_desc_batch *batches, int n_batches,
+                                          const ks_hw_spec *specs, int n_specs, float *const *latency,
+                                          int32_t *const *tiles, int32_t *const *waves, float *const *t_roof);
 
 /* Compose per-kernel latencies into per-step and per-configuration latencies (S6-S7).
  *   latency[b]      fp32 [n_specs][batch_n[b]] as written by ks_predict_kernels

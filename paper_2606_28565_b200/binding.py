@@ -15,7 +15,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libks.so")
 
-KS_OK, KS_EINVAL, KS_ENOMEM, KS_ECUDA, KS_ESTATE, KS_EUNSUPPORTED = range(6)
+KS_OK, KS_EINVAL, KS_ENOMEM, KS_ECUDA, KS_ESTATE, KS_EUNSUPPORTED, KS_ELIMIT = range(7)
+KS_STATIC_ROUTE_MAX_ROWS = 1 << 20
 KS_FAM_GEMM, KS_FAM_GROUPED_GEMM, KS_FAM_ATTN, KS_FAM_ELEMWISE = range(4)
 KS_TIER_NONE, KS_TIER_A, KS_TIER_B = range(3)
 KS_SLOT_FAMILY, KS_MAX_MODEL_SLOTS = -1, 16
@@ -24,7 +25,7 @@ KS_COL_I32, KS_COL_F32 = 0, 1
 KS_MEM_DEVICE, KS_MEM_HOST = 0, 1
 KS_MAX_COLS, KS_MAX_BATCHES = 10, 8
 EXPORTS = ["ks_create", "ks_load_heads", "ks_load_head_ensemble", "ks_load_bounded_head", "ks_load_grid", "ks_set_head_output",
-           "ks_predict_kernels", "ks_compose_steps",
+           "ks_predict_kernels", "ks_predict_routed_static", "ks_compose_steps",
            "ks_compose_steps_weighted",
            "ks_run_steps", "ks_sched_create", "ks_sched_add_requests", "ks_sched_add_prefixed_requests", "ks_sched_step", "ks_sched_commit",
            "ks_sched_results", "ks_sched_get_stats", "ks_sched_destroy", "ks_sim_run",
@@ -99,6 +100,8 @@ def load() -> C.CDLL:
     L.ks_set_head_output.argtypes = [vp, i32, i32]
     L.ks_predict_kernels.argtypes = [vp, C.POINTER(ks_desc_batch), i32, C.POINTER(ks_hw_spec), i32, i32, i32,
                                      C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    L.ks_predict_routed_static.argtypes = [vp, C.POINTER(ks_desc_batch), i32, C.POINTER(ks_hw_spec), i32,
+                                           C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.ks_compose_steps.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int32), i32, i32, i32,
                                    C.POINTER(ks_step_params), vp, i32, i32, vp, vp]
     L.ks_compose_steps_weighted.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int32), i32,
@@ -274,6 +277,18 @@ class Context:
         _check(self._lib.ks_predict_kernels(self._h, batches, nb, sp, len(specs), int(tier), int(space),
                                             _ptr_array(latency), opt(tiles), opt(waves), opt(t_roof)),
                "ks_predict_kernels")
+
+    def predict_routed_static(self, buckets: Sequence, specs: Sequence[dict], latency: Sequence,
+                              tiles: Optional[Sequence] = None, waves: Optional[Sequence] = None,
+                              t_roof: Optional[Sequence] = None) -> None:
+        """Density-routed prediction on device buffers with the row lists in the library's fixed device array:
+        no allocation; at most KS_STATIC_ROUTE_MAX_ROWS routed rows per call (KS_ELIMIT beyond)."""
+        nb = len(buckets)
+        batches = (ks_desc_batch * max(nb, 1))(*[make_batch(b) for b in buckets])
+        sp = (ks_hw_spec * max(len(specs), 1))(*[make_spec(s) for s in specs])
+        opt = lambda x: _ptr_array(x) if x is not None else None
+        _check(self._lib.ks_predict_routed_static(self._h, batches, nb, sp, len(specs), _ptr_array(latency),
+                                                  opt(tiles), opt(waves), opt(t_roof)), "ks_predict_routed_static")
 
     def compose_steps(self, latency: Sequence, step_off: Sequence, batch_n: Sequence[int], n_steps: int,
                       n_specs: int, params: dict, cfg_off, n_cfg: int, step_latency, cfg_latency,

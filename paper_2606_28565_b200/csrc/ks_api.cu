@@ -7,6 +7,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -407,6 +408,7 @@ const char* ks_status_string(ks_status s) {
     case KS_ECUDA: return "KS_ECUDA";
     case KS_ESTATE: return "KS_ESTATE";
     case KS_EUNSUPPORTED: return "KS_EUNSUPPORTED";
+    case KS_ELIMIT: return "KS_ELIMIT";
   }
   return "KS_?";
 }
@@ -817,6 +819,89 @@ ks_status ks_predict_kernels(ks_ctx* c, const ks_desc_batch* batches, int n_batc
   }
   KS_CUDA(c, cudaStreamSynchronize(c->stream));
   return KS_OK;
+}
+
+}  // extern "C"
+
+// ---- ks_predict_routed_static (include/ks.h): density routing with its row lists in a fixed device array.
+// Per routed bucket the lists take align_up(4 n, 256) + 256 bytes (route_need), at most 4 n + 511: the array holds
+// KS_STATIC_ROUTE_MAX_ROWS rows in up to KS_MAX_BATCHES buckets.  Every GPU that loads libks holds it until exit.
+// In host code `ks_static_route` is a host-side stand-in, not a device address: the kernels get the pointer that
+// cudaGetSymbolAddress returns, resolved once per device with that device current.
+namespace {
+
+constexpr size_t kStaticRouteBytes = (size_t)KS_STATIC_ROUTE_MAX_ROWS * 4 + (size_t)KS_MAX_BATCHES * 512;
+constexpr int kStaticMaxDevices = 64;
+
+}  // namespace
+
+static __device__ __align__(256) unsigned char ks_static_route[kStaticRouteBytes];
+
+namespace {
+
+std::mutex g_static_mu;
+unsigned char* g_static_ptr[kStaticMaxDevices] = {};
+
+// the array's address on the CURRENT device (the caller has made c->device current)
+ks_status static_route_ptr(ks_ctx* c, unsigned char** out) {
+  if (c->device < 0 || c->device >= kStaticMaxDevices) return KS_EUNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[c->device]) {
+    void* p = nullptr;
+    KS_CUDA(c, cudaGetSymbolAddress(&p, ks_static_route));
+    if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return cuda_fail(c);
+    g_static_ptr[c->device] = static_cast<unsigned char*>(p);
+  }
+  *out = g_static_ptr[c->device];
+  return KS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+ks_status ks_predict_routed_static(ks_ctx* c, const ks_desc_batch* batches, int n_batches, const ks_hw_spec* specs,
+                                   int n_specs, float* const* latency, int32_t* const* tiles, int32_t* const* waves,
+                                   float* const* t_roof) {
+  const int tier = KS_TIER_B_ROUTED;
+  ks_status st = validate_batches(c, batches, n_batches, specs, n_specs, tier, true);
+  if (st != KS_OK) return st;
+  if (n_batches > 0 && !latency) return KS_EINVAL;
+  long long rows = 0;
+  for (int b = 0; b < n_batches; ++b) {
+    if (batches[b].family != KS_FAM_ALLREDUCE) rows += batches[b].n;
+    if (batches[b].n == 0 || n_specs == 0) continue;
+    if (!latency[b]) return KS_EINVAL;
+    if (!aligned16(latency[b]) || (tiles && tiles[b] && !aligned16(tiles[b])) ||
+        (waves && waves[b] && !aligned16(waves[b])) || (t_roof && t_roof[b] && !aligned16(t_roof[b])))
+      return KS_EINVAL;
+  }
+  if (rows > (long long)KS_STATIC_ROUTE_MAX_ROWS) return KS_ELIMIT;        // the fixed array holds no more
+  if (route_need(batches, n_batches, tier) > kStaticRouteBytes) return KS_ELIMIT;
+  if (c->sticky) return KS_ECUDA;
+  if (n_batches == 0 || n_specs == 0) return KS_OK;
+  KS_CUDA(c, cudaSetDevice(c->device));
+  unsigned char* base = nullptr;
+  st = static_route_ptr(c, &base);
+  if (st != KS_OK) return st;
+
+  const void* cols[KS_MAX_BATCHES][KS_MAX_COLS] = {};
+  DevOut outs[KS_MAX_BATCHES];
+  RouteBuf rb[KS_MAX_BATCHES];
+  size_t used = 0;
+  for (int b = 0; b < n_batches; ++b) {
+    for (int k = 0; k < batches[b].n_cols; ++k) cols[b][k] = batches[b].cols[k];
+    outs[b].lat = latency[b];
+    outs[b].tiles = tiles ? tiles[b] : nullptr;
+    outs[b].waves = waves ? waves[b] : nullptr;
+    outs[b].troof = t_roof ? t_roof[b] : nullptr;
+    if (batches[b].family == KS_FAM_ALLREDUCE) continue;
+    rb[b].idx = reinterpret_cast<int32_t*>(base + used);
+    used += align_up((size_t)batches[b].n * 4, 256);
+    rb[b].count = reinterpret_cast<int32_t*>(base + used);   // cleared (stream-ordered) by predict_device before pass 1
+    used += 256;
+  }
+  return predict_device(c, batches, cols, n_batches, specs, n_specs, tier, outs, rb);
 }
 
 ks_status ks_compose_steps(ks_ctx* c, const float* const* latency, const int32_t* const* step_off,
