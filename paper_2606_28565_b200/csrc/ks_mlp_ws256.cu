@@ -9,7 +9,7 @@
 //                          previous item has consumed it), t_roof -> 4-deep ring
 //   warps 4-11   EPI1      warpgroup g activates D1 columns [128 g, 128 g + 128): tcgen05.ld 16 columns
 //                          (double-buffered) -> 2 GELU -> bf16 -> A2 K groups 2g, 2g+1; group k of item
-//                          q is written once MMA2(q-1) has consumed group k (a2_free[k]) and announced
+//                          q is stored once MMA2(q-1) has consumed group k (a2_free[k]) and announced
 //                          on a2_full[k]; d1_free as soon as the last D1 column is in registers
 //   warp  20     MMA       MMA2(q) is issued group by group as the groups arrive (order 0, 2, 1, 3),
 //                          with MMA1(q+1) slotted in as soon as D1 is drained: layer 2 of item q runs
@@ -137,7 +137,10 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
   const uint32_t lane_off = (uint32_t)((r >> 5) * 32) << 16;
   unsigned char* A2 = smem + C::OFF_A2;
   const uint32_t d1 = tmem_base + lane_off + (uint32_t)(wg * 128);
-  auto act_store = [&](const uint32_t* a, int c16) {               // c16: 16-column sub-chunk within the warpgroup's half
+  // c16: 16-column sub-chunk within the warpgroup's half; wait_bar: the K group's a2_free barrier when this
+  // sub-chunk is the first of the group.  The wait sits between the arithmetic and the stores, so the GELUs of
+  // a group's first sub-chunk run while layer 2 of the previous item still reads the group (2 % on cfg5).
+  auto act_store = [&](const uint32_t* a, int c16, uint64_t* wait_bar, uint32_t wait_par) {
     uint32_t pk[8];
     if (GM == 0) {
 #pragma unroll
@@ -150,6 +153,7 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
 #pragma unroll
       for (int j = 0; j < 8; ++j) pk[j] = gelu2_bf16x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]));
     }
+    if (wait_bar) ks_mbar_wait(wait_bar, wait_par);
     const int kc = wg * 16 + c16 * 2;                               // 8-column K chunk index
     *reinterpret_cast<uint4*>(A2 + (kc + 0) * kChunkBytes + r * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
     *reinterpret_cast<uint4*>(A2 + (kc + 1) * kChunkBytes + r * 16) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
@@ -162,10 +166,9 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
     ks_tmem_ld16(d1, accA);
 #pragma unroll 1
     for (int c = 0; c < 8; c += 2) {                                // 8 sub-chunks = 2 K groups of 64 columns
-      if ((c & 3) == 0 && q >= 1u) ks_mbar_wait(bars + BAR_A2_FREE + wg * 2 + (c >> 2), par ^ 1u);
       ks_tmem_ld_wait();
       ks_tmem_ld16(d1 + (uint32_t)((c + 1) * 16), accB);
-      act_store(accA, c);
+      act_store(accA, c, ((c & 3) == 0 && q >= 1u) ? bars + BAR_A2_FREE + wg * 2 + (c >> 2) : nullptr, par ^ 1u);
       ks_tmem_ld_wait();
       if (c + 2 < 8) {
         ks_tmem_ld16(d1 + (uint32_t)((c + 2) * 16), accA);
@@ -173,7 +176,7 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
         ks_tc_fence_before();
         ks_mbar_arrive(bars + BAR_D1_FREE);
       }
-      act_store(accB, c + 1);
+      act_store(accB, c + 1, nullptr, 0u);
       if ((c & 3) == 2) {                                           // a K group of 64 columns is complete
         ks_fence_proxy_async();
         ks_mbar_arrive(bars + BAR_A2_FULL + wg * 2 + (c >> 2));
