@@ -469,8 +469,8 @@ ks_mlp_ws_kernel(const __grid_constant__ KsMlpParams p) {
       if (p.gelu_mode == 0) epi2_all<NIN, H, 0, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
       else epi2_all<NIN, H, 1, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
     }
-  } else if (tid == kMmaWarp * 32) {
-    mma_all<NIN, H>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+  } else if (__shfl_sync(0xffffffffu, warp, 0) == kMmaWarp) {   // warp-uniform branch, then one elected lane
+    if (ks_elect_one()) mma_all<NIN, H>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   }
   ks_tc_fence_before();
   __syncthreads();

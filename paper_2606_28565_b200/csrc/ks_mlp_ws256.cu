@@ -307,7 +307,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
   }
 }
 
-// ------------------------------------------------------------------ MMA issuer (one thread of warp 20)
+// ------------------------------------------------------------------ MMA issuer (one elected lane of warp 20)
 template <int NIN>
 KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, const int t_hi, unsigned char* smem,
                     uint64_t* bars, const uint32_t tmem_base) {
@@ -453,8 +453,8 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
       if (p.gelu_mode == 0) epi2_all<NIN, 0, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
       else epi2_all<NIN, 1, false>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
     }
-  } else if (tid == kMmaWarp * 32) {
-    mma_all<NIN>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
+  } else if (__shfl_sync(0xffffffffu, warp, 0) == kMmaWarp) {   // warp-uniform branch, then one elected lane
+    if (ks_elect_one()) mma_all<NIN>(p, tm, t_lo, t_hi, smem, bars, tmem_base);
   }
   ks_tc_fence_before();
   __syncthreads();

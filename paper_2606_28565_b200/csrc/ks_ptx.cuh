@@ -128,6 +128,15 @@ KS_PTX void ks_tmem_relinquish() {
 KS_PTX void ks_tmem_dealloc(uint32_t taddr, uint32_t ncols) {     // same warp that allocated
   asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
 }
+// One lane of a CONVERGED warp (elect.sync).  The MMA-issuing role is entered through a warp-uniform branch
+// (__shfl_sync of the warp index) and this election, not through `tid == k`: ptxas then keeps the UMMA
+// descriptors in uniform registers and emits the tcgen05.mma instructions back to back, where the divergent form
+// cost 13 SASS instructions per UTCHMMA (descriptor arithmetic plus an ELECT / BRA.U.ANY loop around each).
+KS_PTX bool ks_elect_one() {
+  uint32_t leader;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(leader));
+  return leader != 0;
+}
 KS_PTX void ks_tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 KS_PTX void ks_tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
