@@ -236,7 +236,11 @@ KS_API ks_status ks_compose_steps_weighted(ks_ctx *ctx, const float *const *late
  * end-to-end call: descriptors and offsets go host->device, results device->host, then sync.  Buckets are
  * pipelined in the caller's order (bucket b is copied while bucket b-1 is predicted: largest first is best);
  * pinned host memory is what makes the copies asynchronous, and the columns of a bucket that lie back to
- * back in host memory (cols[k+1] == cols[k] + 4 n, n a multiple of 4) move with a single copy. */
+ * back in host memory (cols[k+1] == cols[k] + 4 n, n a multiple of 4) move with a single copy.
+ * KS_MEM_DEVICE with KS_TIER_NONE, one spec vector, int32 columns, no multiplicities, at most four buckets and no
+ * grouped-GEMM bucket (config 4a's shape) runs as ONE kernel plus the totals kernel: the latencies are computed in the
+ * step kernel's staging phase instead of being written to HBM and read back, and latency[b] is written only where the
+ * caller passed a buffer (none: a step moves the descriptor columns only).  Same bits as the two-call path. */
 KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const int32_t *const *step_off,
                        int n_batches, const ks_hw_spec *specs, int n_specs, ks_tier tier, int n_steps,
                        const ks_step_params *params, const int32_t *cfg_off, int n_cfg,

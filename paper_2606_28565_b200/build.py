@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libks.so")
-SOURCES = ["ks_api.cu", "ks_stream.cu", "ks_tierb.cu", "ks_mlp.cu", "ks_mlp_ws.cu", "ks_mlp_ws256.cu", "ks_compose.cu", "ks_sched.cu"]
+SOURCES = ["ks_api.cu", "ks_stream.cu", "ks_tierb.cu", "ks_mlp.cu", "ks_mlp_ws.cu", "ks_mlp_ws256.cu", "ks_compose.cu", "ks_fused.cu", "ks_sched.cu"]
 HEADERS = ["ks_common.cuh", "ks_ptx.cuh", "ks_mlp_common.cuh", "ks_internal.h", os.path.join("..", "..", "include", "ks.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math", "-Xptxas", "-v"]

@@ -982,6 +982,49 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
 
+  // Tier NONE with one spec vector and no multiplicities (config 4a's shape): ONE kernel computes the latencies in
+  // the step kernel's staging phase (ks_fused.cu) instead of writing them to HBM and reading them back; per-kernel
+  // latencies are written only where the caller passed a buffer.  Same bits as the two-call path.
+  if (dev && tier == KS_TIER_NONE && n_specs == 1 && n_steps > 0 && n_batches >= 1 && n_batches <= KS_FUSED_MAX_BUCKETS) {
+    bool fusable = true;
+    long long rows = 0;
+    for (int b = 0; b < n_batches; ++b) {
+      fusable = fusable && !batches[b].mult && ks_fused_none_supported(batches[b].family, batches[b].col_dtype == KS_COL_F32);
+      rows += batches[b].n;
+    }
+    // an average chunk of 32 steps must fit the 47 KiB staging buffer (a chunk that does not is summed from the columns)
+    fusable = fusable && (double)rows / (double)n_steps * 32.0 <= 0.85 * 12032.0;
+    if (fusable) {
+      KsFusedParams p;
+      memset(&p, 0, sizeof(p));
+      for (int b = 0; b < n_batches; ++b) {
+        DevOut o;
+        o.lat = latency ? latency[b] : nullptr;
+        p.bk[b] = make_bucket_dev(batches[b], batches[b].cols, o, 0);
+        p.step_off[b] = step_off[b];
+      }
+      p.n_batches = n_batches;
+      p.n_steps = n_steps;
+      p.sp = *params;
+      p.spec = make_spec_dev(specs[0]);
+      p.step_lat = step_latency;
+      KS_CUDA(c, ks_launch_fused_none(p, c->stream));
+      c->launches += 1;
+      KsComposeParams q;
+      memset(&q, 0, sizeof(q));
+      q.n_steps = n_steps;
+      q.n_specs = 1;
+      q.n_cfg = n_cfg;
+      q.cfg_off = cfg_off;
+      q.step_lat = step_latency;
+      q.cfg_lat = cfg_latency;
+      int launches = 0;
+      KS_CUDA(c, ks_launch_cfg_totals(q, c->stream, true, &launches));
+      c->launches += launches;
+      return KS_OK;
+    }
+  }
+
   size_t need = 0;
   for (int b = 0; b < n_batches; ++b) {
     const size_t n = batches[b].n;

@@ -372,6 +372,10 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
     if (e != cudaSuccess) return e;
     if (launches) *launches += 1;
   }
+  return ks_launch_cfg_totals(p, st, total > 0, launches);
+}
+
+cudaError_t ks_launch_cfg_totals(const KsComposeParams& p, cudaStream_t st, bool after_ours, int* launches) {
   if (p.n_cfg > 0 && p.n_specs > 0 && p.cfg_lat) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(p.n_cfg * p.n_specs));
@@ -381,7 +385,7 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // hide this launch under the step kernel's tail
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = total > 0 ? 1 : 0;               // (no preceding kernel of ours: plain launch)
+    cfg.numAttrs = after_ours ? 1 : 0;              // (no preceding kernel of ours: plain launch)
     cudaError_t e = cudaLaunchKernelEx(&cfg, ks_cfg_total_kernel, p);
     if (e != cudaSuccess) return e;
     if (launches) *launches += 1;

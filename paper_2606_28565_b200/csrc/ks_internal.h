@@ -108,6 +108,22 @@ struct KsComposeParams {
 cudaStream_t ks_internal_stream(ks_ctx* c);
 cudaError_t ks_internal_set_device(ks_ctx* c);
 cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_t st, int* launches);
+// S7's second half alone (per-configuration totals of p.step_lat); after_ours: the launch may overlap the tail of
+// the libks kernel that precedes it on the stream (it waits for that kernel's completion itself)
+cudaError_t ks_launch_cfg_totals(const KsComposeParams& p, cudaStream_t st, bool after_ours, int* launches);
+
+// ---- Tier NONE, one spec, unweighted: decode + roofline + floor + step sums + Eq. 4 in one kernel: ks_fused.cu
+#define KS_FUSED_MAX_BUCKETS 4
+struct KsFusedParams {
+  KsBucketDev bk[KS_FUSED_MAX_BUCKETS];      // lat may be nullptr: the per-kernel latencies are not written then
+  const int32_t* step_off[KS_FUSED_MAX_BUCKETS];
+  int32_t n_batches, n_steps, cap_floats, pad;
+  ks_step_params sp;
+  KsSpecDev spec;
+  float* step_lat;                           // [n_steps]
+};
+bool ks_fused_none_supported(int family, bool col_f32);
+cudaError_t ks_launch_fused_none(const KsFusedParams& p, cudaStream_t st);
 
 // Every libks kernel is launched with programmatic stream serialization and opens with
 //   griddepcontrol.launch_dependents;  cudaGridDependencySynchronize();
