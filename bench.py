@@ -396,6 +396,36 @@ def compose_roofline(h: Harness, st, peaks, iters=None, sets=None):
     return out
 
 
+def run_steps_roofline(h: Harness, st, peaks, iters=None, sets=None):
+    """ks_run_steps in device space (Tier NONE, one spec: the one-kernel path of ks_fused.cu) with and without the
+    per-kernel latency output; bytes = descriptor columns (+ 4 per kernel instance when the latencies are written)
+    + step offsets and step latencies."""
+    w = st["w"]
+    cols = sum((BYTES_PER_ROW[b.family] - 4) * b.n for b in st["db"])
+    steps = w.n_steps * (4 + 4 * len(st["db"]))
+    rows = sum(b.n for b in st["db"])
+
+    def run(db, lat):
+        h.ctx.run_steps(db, [b.step_off for b in st["db"]], w.specs, w.tier, w.n_steps, w.step_params, st["cfg"], st["n_cfg"],
+                        st["step"], st["tot"], latency=lat, space=h.B.KS_MEM_DEVICE)
+    out = {}
+    for name, with_lat in (("with_kernel_latencies", True), ("steps_only", False)):
+        byts = cols + steps + (4 * rows if with_lat else 0)
+        ms = h.timed([lambda: run(st["db"], st["lat"] if with_lat else None)], iters or EX_ITERS, EX_WARM)[:, 0]
+        o = dict(bytes=int(byts), ms=float(ms.mean()), ms_min=float(ms.min()), launches_per_call=2,
+                 frac_hbm=float(byts / (ms.mean() * 1e-3) / 1e9 / peaks["hbm"]),
+                 kernel_instances_per_s=float(rows / (ms.mean() * 1e-3)))
+        if sets is not None:
+            us = timed_b2b(h, lambda k: run(sets[k % len(sets)]["db"], sets[k % len(sets)]["lat"] if with_lat else None),
+                           len(sets), 4 * len(sets))
+            o.update(us_b2b=float(us), frac_hbm_b2b=float(byts / us / 1e3 / peaks["hbm"]),
+                     kernel_instances_per_s_b2b=float(rows / us * 1e6))
+        out[name] = o
+    out["note"] = ("one kernel computes the latencies in the step kernel's staging phase (no 2 x 4 B per kernel instance of "
+                   "write + re-read); outputs bit-identical to ks_predict_kernels + ks_compose_steps")
+    return out
+
+
 # ------------------------------------------------------------------------------- end to end + parity per config
 def e2e_measure(h: Harness, w, K: int, world: int = 1, dist=None, with_kernel_latencies: bool = False):
     """The metric through ks_run_steps with HOST (pinned) buffers: H2D + kernels + D2H inside the timed region.
@@ -552,6 +582,7 @@ def run_extras(h: Harness, peaks):
     sets = None if PROFILE else clone_sets(st, 4)
     ex["cfg4a"]["kernels"] = dict(stream=stream_roofline(h, st, peaks, sets=sets),
                                   compose=compose_roofline(h, st, peaks, sets=sets))
+    ex["cfg4a"]["run_steps_one_kernel"] = run_steps_roofline(h, st, peaks, sets=sets)
     del st, sets
     torch.cuda.empty_cache()
 
