@@ -21,6 +21,9 @@ KS_DEV uint32_t ks_ceil_div(uint32_t a, const KsFastDiv& f) {
   uint32_t q = ks_div(a, f);
   return q + (q * f.d != a ? 1u : 0u);
 }
+// ceil(a / d) for 1 <= a < 2^31 as floor((a - 1) / d) + 1: four instructions instead of seven (a = 0 gives garbage:
+// the caller selects 0 itself, usually together with a test it needs anyway)
+KS_DEV uint32_t ks_ceil_div_pos(uint32_t a, const KsFastDiv& f) { return (__umulhi(2u * a - 2u, f.mul) >> f.shr) + 1u; }
 
 // ------------------------------------------------------------------ per-spec constants (device form)
 struct KsSpecDev {
@@ -68,7 +71,10 @@ struct KsWork {
   uint32_t B;       // CTA / tile count (saturates at INT32_MAX)
 };
 
-KS_DEV uint32_t ks_sat31(unsigned long long x) { return x > 0x7fffffffull ? 0x7fffffffu : (uint32_t)x; }
+KS_DEV uint32_t ks_sat31(unsigned long long x) {
+  const uint32_t hi = (uint32_t)(x >> 32), lo = (uint32_t)x;      // two 32-bit tests instead of a 64-bit compare
+  return (hi != 0u || (int32_t)lo < 0) ? 0x7fffffffu : lo;
+}
 KS_DEV int ks_nonneg(int v) { return v > 0 ? v : 0; }
 
 // elementwise sub-op tables (words moved / FLOPs per element), Q1
@@ -85,7 +91,8 @@ KS_DEV KsWork ks_decode(const int* v, const KsBucketDev& bk, const KsSpecDev& sp
     const float Mf = (float)M, Nf = (float)N, Kf = (float)K;
     w.F = 2.0f * Mf * Nf * Kf;
     w.Y = s * fmaf(Mf, Kf, fmaf(Kf, Nf, Mf * Nf));
-    w.B = ks_sat31((unsigned long long)ks_ceil_div(M, sp.tile_m) * ks_ceil_div(N, sp.tile_n));
+    const uint32_t B = ks_sat31((unsigned long long)ks_ceil_div_pos(M, sp.tile_m) * ks_ceil_div_pos(N, sp.tile_n));
+    w.B = (M == 0 || N == 0) ? 0u : B;
   } else if (FAM == KS_FAM_GROUPED_GEMM) {
     const int N = ks_nonneg(v[0]), K = ks_nonneg(v[1]);
     const uint32_t cn = ks_ceil_div(N, sp.tile_n);
@@ -112,7 +119,8 @@ KS_DEV KsWork ks_decode(const int* v, const KsBucketDev& bk, const KsSpecDev& sp
     const float pairs = fmaf(qf, (float)(kv - q), 0.5f * qf * (qf + 1.0f));
     w.F = 4.0f * Bf * (float)bk.hq * hd * pairs;
     w.Y = s * 2.0f * Bf * hd * fmaf(qf, (float)bk.hq, (float)kv * (float)bk.hkv);
-    w.B = ks_sat31((unsigned long long)Bq * (unsigned long long)bk.hq * ks_ceil_div(q, sp.tile_m));
+    const uint32_t B = ks_sat31((unsigned long long)Bq * (unsigned long long)bk.hq * ks_ceil_div_pos(q, sp.tile_m));
+    w.B = q == 0 ? 0u : B;
   } else if (FAM == KS_FAM_ALLREDUCE) {
     w.F = 0.0f; w.Y = 0.0f; w.B = 0u;               // a communication row has no roofline (ks_allreduce)
   } else {
@@ -120,7 +128,7 @@ KS_DEV KsWork ks_decode(const int* v, const KsBucketDev& bk, const KsSpecDev& sp
     const int op = ks_ew_op(v[1]);
     w.Y = s * (float)n * ks_ew_rw(op);
     w.F = (float)n * ks_ew_fl(op);
-    w.B = ks_ceil_div(n, sp.ew);
+    w.B = n == 0 ? 0u : ks_ceil_div_pos(n, sp.ew);
   }
   if (w.B == 0u) { w.F = 0.0f; w.Y = 0.0f; }
   return w;
@@ -144,7 +152,7 @@ struct KsRoof {
 KS_DEV KsRoof ks_roofline(const KsWork& w, const KsSpecDev& sp) {
   KsRoof r;
   if (w.B == 0u) { r.W = 0u; r.u = 1.0f; r.t_comp = 0.0f; r.t_mem = 0.0f; r.t_roof = 0.0f; return r; }
-  r.W = ks_ceil_div(w.B, sp.slots);
+  r.W = ks_ceil_div_pos(w.B, sp.slots);             // B >= 1 here
   r.u = __fdividef((float)r.W * sp.slots_f, (float)w.B);
   r.t_comp = w.F * sp.inv_peak_flops;
   r.t_mem = w.Y * sp.inv_peak_bw;
