@@ -15,8 +15,12 @@
 //                          with MMA1(q+1) slotted in as soon as D1 is drained: layer 2 of item q runs
 //                          on the tensor core under the rest of layer 1's activation work, and layer 1
 //                          of item q+1 is ready when EPI1 finishes item q
-//   warps 12-19  EPI2      warpgroup g takes D2 columns [128 g, 128 g + 128): + b2 (fp32) -> 2 GELU ->
-//                          dot with w3/2; the two partial dots meet in shared memory; sigmoid, latency
+//   warps 12-19  EPI2      both warpgroups take 64 columns of D2 half 0, then 64 columns of half 1 (warpgroup g: columns
+//                          [64 g, 64 g + 64) and [128 + 64 g, 128 + 64 g + 64)): + b2 (fp32) -> 2 GELU -> dot with w3/2;
+//                          while they are on one half the tensor core refills the other with the next item (a clock64
+//                          trace showed the item period = activation of a half + its refill when a warpgroup owned a
+//                          whole half).  Ensembles keep a half per warpgroup (a member's columns stay in one warpgroup).
+//                          The two partial dots meet in shared memory; sigmoid, latency
 // so EPI1(q+1) and EPI2(q) share the MUFU pipe while the tensor core works on both items.
 // b2 is added in the fp32 epilogue here (in the H <= 128 kernels it rides through the tensor core
 // as one more K step): dropping the bias rows of W2 and the ones-block is what makes 225 KB fit.
@@ -206,8 +210,13 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
     const KsBucketDev& bk = p.bk[b];
     // this family's layer-3 weights and layer-2 bias: a warpgroup stages and reads only its own 128 columns
     ks_bar_sync(2 + wg, 128);
-    sw3[e] = __ldg(p.head[b].w3 + e);
-    sb2[e] = __ldg(p.head[b].b2 + e);
+    {
+      // ENS: the warpgroup owns columns [128 wg, 128 wg + 128); otherwise 64 columns of EACH half of D2:
+      // [64 wg, 64 wg + 64) and [128 + 64 wg, 128 + 64 wg + 64)
+      const int sc = ENS ? e : ((r >> 6) * 128 + wg * 64 + (r & 63));
+      sw3[sc] = __ldg(p.head[b].w3 + sc);
+      sb2[sc] = __ldg(p.head[b].b2 + sc);
+    }
     ks_bar_sync(2 + wg, 128);
     const KsHeadDev& hd = p.head[b];
     const float b3 = hd.b3, out_sgn = hd.out_sgn, out_lo = hd.out_lo, out_add = hd.out_add;
@@ -225,62 +234,119 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
       const bool valid = pos < ne;
       const int row = valid ? (idx ? __ldg(idx + pos) : pos) : 0;
       for (int s = 0; s < n_specs; ++s, ++q) {
-        ks_mbar_wait(bars + BAR_MMA2 + wg, q & 1u);                 // this half of D2 holds item q
-        ks_tc_fence_after();
-        uint32_t accA[16], accB[16];
-        ks_tmem_ld16(d2, accA);
-        const float t_roof = ring[(q & (kRing - 1)) * kRows + r];
-        float z0 = 0.0f, z1 = 0.0f, z2 = 0.0f, z3 = 0.0f;
-        auto act_dot = [&](const uint32_t* a, int c16) {
-          const int col = wg * 128 + c16 * 16;
-#pragma unroll
-          for (int j = 0; j < 16; j += 4) {
-            const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col + j);
-            const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
-            float x0, x1, x2, x3;
-            ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
-            ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
-            if (GM == 0) {
-              float g0, g1, g2, g3;
-              gelu2_f32x2(x0, x1, g0, g1);
-              gelu2_f32x2(x2, x3, g2, g3);
-              ks_fma2(z0, z1, g0, g1, w4.x, w4.y, z0, z1);
-              ks_fma2(z2, z3, g2, g3, w4.z, w4.w, z2, z3);
-            } else {
-              const uint32_t g0 = gelu2_bf16x2(x0, x1), g1 = gelu2_bf16x2(x2, x3);
-              z0 = fmaf(__uint_as_float(g0 << 16), w4.x, z0);
-              z1 = fmaf(__uint_as_float(g0 & 0xffff0000u), w4.y, z1);
-              z2 = fmaf(__uint_as_float(g1 << 16), w4.z, z2);
-              z3 = fmaf(__uint_as_float(g1 & 0xffff0000u), w4.w, z3);
+        float z;
+        if (ENS) {
+          ks_mbar_wait(bars + BAR_MMA2 + wg, q & 1u);                 // this half of D2 holds item q
+          ks_tc_fence_after();
+          uint32_t accA[16], accB[16];
+          ks_tmem_ld16(d2, accA);
+          float z0 = 0.0f, z1 = 0.0f, z2 = 0.0f, z3 = 0.0f;
+          auto act_dot = [&](const uint32_t* a, int c16) {
+            const int col = wg * 128 + c16 * 16;
+  #pragma unroll
+            for (int j = 0; j < 16; j += 4) {
+              const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col + j);
+              const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
+              float x0, x1, x2, x3;
+              ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
+              ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
+              if (GM == 0) {
+                float g0, g1, g2, g3;
+                gelu2_f32x2(x0, x1, g0, g1);
+                gelu2_f32x2(x2, x3, g2, g3);
+                ks_fma2(z0, z1, g0, g1, w4.x, w4.y, z0, z1);
+                ks_fma2(z2, z3, g2, g3, w4.z, w4.w, z2, z3);
+              } else {
+                const uint32_t g0 = gelu2_bf16x2(x0, x1), g1 = gelu2_bf16x2(x2, x3);
+                z0 = fmaf(__uint_as_float(g0 << 16), w4.x, z0);
+                z1 = fmaf(__uint_as_float(g0 & 0xffff0000u), w4.y, z1);
+                z2 = fmaf(__uint_as_float(g1 << 16), w4.z, z2);
+                z3 = fmaf(__uint_as_float(g1 & 0xffff0000u), w4.w, z3);
+              }
             }
-          }
-        };
-        float esum = 0.0f;                         // ensemble: sum of this half's members' efficiencies
-        auto sweep = [&](auto ens) {
-          int m = wg * (members >> 1);             // first member of this warpgroup's 128 columns
+          };
+          float esum = 0.0f;                         // ensemble: sum of this half's members' efficiencies
+          auto sweep = [&](auto ens) {
+            int m = wg * (members >> 1);             // first member of this warpgroup's 128 columns
+  #pragma unroll 1
+            for (int c = 0; c < 8; c += 2) {
+              ks_tmem_ld_wait();
+              ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
+              act_dot(accA, c);
+              ks_tmem_ld_wait();
+              if (c + 2 < 8) {
+                ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
+              } else {                                                  // D2 is drained: MMA2(q+1) may overwrite it
+                ks_tc_fence_before();
+                ks_mbar_arrive(bars + BAR_D2_FREE + wg);
+              }
+              act_dot(accB, c + 1);
+              if (decltype(ens)::value && ((c + 2) & ens_mask) == 0) {  // last column of member m (Q17)
+                const float zm = ((z0 + z1) + (z2 + z3)) + hd.b3m[m++];
+                esum += __fdividef(1.0f, 1.0f + __expf(-zm));
+                z0 = z1 = z2 = z3 = 0.0f;
+              }
+            }
+          };
+          if (members > 1) sweep(std::true_type{}); else sweep(std::false_type{});
+          // single head: partial logit of this half; ensemble: partial sum of efficiencies
+          z = members > 1 ? esum : (z0 + z1) + (z2 + z3);
+        } else {
+          // Both warpgroups activate 64 columns of half 0, then 64 columns of half 1: while they are on half 1 the tensor
+          // core refills half 0 with the next item and vice versa, so the 1,000-1,300 cycles of a refill no longer sit
+          // between two activations of the same half (clock64 trace: the item period was activation + refill).
+          float z0 = 0.0f, z1 = 0.0f, z2 = 0.0f, z3 = 0.0f;
 #pragma unroll 1
-          for (int c = 0; c < 8; c += 2) {
-            ks_tmem_ld_wait();
-            ks_tmem_ld16(d2 + (uint32_t)((c + 1) * 16), accB);
-            act_dot(accA, c);
-            ks_tmem_ld_wait();
-            if (c + 2 < 8) {
-              ks_tmem_ld16(d2 + (uint32_t)((c + 2) * 16), accA);
-            } else {                                                  // D2 is drained: MMA2(q+1) may overwrite it
-              ks_tc_fence_before();
-              ks_mbar_arrive(bars + BAR_D2_FREE + wg);
-            }
-            act_dot(accB, c + 1);
-            if (decltype(ens)::value && ((c + 2) & ens_mask) == 0) {  // last column of member m (Q17)
-              const float zm = ((z0 + z1) + (z2 + z3)) + hd.b3m[m++];
-              esum += __fdividef(1.0f, 1.0f + __expf(-zm));
-              z0 = z1 = z2 = z3 = 0.0f;
+          for (int h = 0; h < 2; ++h) {
+            ks_mbar_wait(bars + BAR_MMA2 + h, q & 1u);               // half h of D2 holds item q
+            ks_tc_fence_after();
+            const uint32_t d2h = tmem_base + (uint32_t)H + lane_off + (uint32_t)(h * 128 + wg * 64);
+            const int col0 = h * 128 + wg * 64;
+            uint32_t accA[16], accB[16];
+            ks_tmem_ld16(d2h, accA);
+            auto act_dot = [&](const uint32_t* a, int c16) {
+              const int col = col0 + c16 * 16;
+#pragma unroll
+              for (int j = 0; j < 16; j += 4) {
+                const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col + j);
+                const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
+                float x0, x1, x2, x3;
+                ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
+                ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
+                if (GM == 0) {
+                  float g0, g1, g2, g3;
+                  gelu2_f32x2(x0, x1, g0, g1);
+                  gelu2_f32x2(x2, x3, g2, g3);
+                  ks_fma2(z0, z1, g0, g1, w4.x, w4.y, z0, z1);
+                  ks_fma2(z2, z3, g2, g3, w4.z, w4.w, z2, z3);
+                } else {
+                  const uint32_t g0 = gelu2_bf16x2(x0, x1), g1 = gelu2_bf16x2(x2, x3);
+                  z0 = fmaf(__uint_as_float(g0 << 16), w4.x, z0);
+                  z1 = fmaf(__uint_as_float(g0 & 0xffff0000u), w4.y, z1);
+                  z2 = fmaf(__uint_as_float(g1 << 16), w4.z, z2);
+                  z3 = fmaf(__uint_as_float(g1 & 0xffff0000u), w4.w, z3);
+                }
+              }
+            };
+#pragma unroll 1
+            for (int c = 0; c < 4; c += 2) {
+              ks_tmem_ld_wait();
+              ks_tmem_ld16(d2h + (uint32_t)((c + 1) * 16), accB);
+              act_dot(accA, c);
+              ks_tmem_ld_wait();
+              if (c + 2 < 4) {
+                ks_tmem_ld16(d2h + (uint32_t)((c + 2) * 16), accA);
+              } else {                                               // this warpgroup's part of half h is in registers
+                ks_tc_fence_before();
+                ks_mbar_arrive(bars + BAR_D2_FREE + h);
+              }
+              act_dot(accB, c + 1);
             }
           }
-        };
-        if (members > 1) sweep(std::true_type{}); else sweep(std::false_type{});
-        // single head: partial logit of this half; ensemble: partial sum of efficiencies
-        float z = members > 1 ? esum : (z0 + z1) + (z2 + z3);
+          z = (z0 + z1) + (z2 + z3);
+        }
+        // (read after the MMA2 waits: layer 2 of item q is complete, so the producer's t_roof(q) has long been written)
+        const float t_roof = ring[(q & (kRing - 1)) * kRows + r];
         // The two column halves meet in shared memory.  Warpgroup 0 (first half of D2, ready one MMA pass
         // earlier) leaves its partial in zpart[q & 1] and moves on; warpgroup 1 picks it up and writes
         // the result.  z_full / z_free hand the two slots back and forth.
@@ -408,7 +474,7 @@ ks_mlp_ws256_kernel(const __grid_constant__ KsMlpParams p) {
     ks_mbar_init(bars + BAR_D1_FREE, 256);
     for (int h = 0; h < 2; ++h) {
       ks_mbar_init(bars + BAR_MMA2 + h, 1);
-      ks_mbar_init(bars + BAR_D2_FREE + h, 128);
+      ks_mbar_init(bars + BAR_D2_FREE + h, p.any_ens ? 128 : 256);   // drained by one warpgroup (ensembles) or by both
       ks_mbar_init(bars + BAR_Z_FULL + h, 128);
       ks_mbar_init(bars + BAR_Z_FREE + h, 128);
     }
