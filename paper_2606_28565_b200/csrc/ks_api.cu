@@ -486,7 +486,9 @@ ks_status install_head(ks_ctx* c, int slot, int n_in, int H, const float* W1, co
   const int n_real = n_in == 32 ? 22 : n_in;          // features 22..31 are identically zero (Q2)
   const int bias_row = n_real;
   // UMMA operand images, K-major no-swizzle: element (n, k) at ((k/8) * H + n) * 8 + k % 8
-  std::vector<uint16_t> i1((size_t)K1 * H, 0), i2((size_t)(H + 16) * H, 0);
+  // (rows H + 16 .. H + 23 of the layer-2 image: one more K chunk with b2 hi / lo at the chunk positions of layer 1's
+  // constant-1 feature columns -- the H = 256 kernel adds b2 with one K = 16 MMA against the A1 operand, ks_mlp_ws256.cu)
+  std::vector<uint16_t> i1((size_t)K1 * H, 0), i2((size_t)(H + 24) * H, 0);
   auto at = [H](int n, int k) { return ((size_t)(k / 8) * H + n) * 8 + (k % 8); };
   for (int j = 0; j < H; ++j) {
     for (int k = 0; k < n_real; ++k) i1[at(j, k)] = f32_to_bf16_bits(W1[(size_t)k * H + j]);
@@ -499,6 +501,8 @@ ks_status install_head(ks_ctx* c, int slot, int n_in, int H, const float* W1, co
     const uint16_t hi2 = f32_to_bf16_bits(b2[j]);
     i2[at(j, H)] = hi2;
     i2[at(j, H + 1)] = f32_to_bf16_bits(b2[j] - bf16_bits_to_f32(hi2));
+    i2[at(j, H + 16 + bias_row % 8)] = hi2;
+    i2[at(j, H + 16 + bias_row % 8 + 1)] = i2[at(j, H + 1)];
   }
   // layer 3 runs in fp32 on the CUDA cores; its weights are still bf16-rounded like the others
   std::vector<float> w3r(H);

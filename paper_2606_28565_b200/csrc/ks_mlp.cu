@@ -9,7 +9,7 @@
 
 int ks_mlp_k1(int n_in) { return n_in == 32 ? 32 : 16; }
 size_t ks_mlp_w1_img_bytes(int n_in, int h) { return (size_t)ks_mlp_k1(n_in) * h * 2; }
-size_t ks_mlp_w2_img_bytes(int h) { return (size_t)(h + 16) * h * 2; }
+size_t ks_mlp_w2_img_bytes(int h) { return (size_t)(h + 24) * h * 2; }
 
 cudaError_t ks_launch_mlp(const KsMlpParams& p, int n_in, int h, int num_sms, cudaStream_t st) {
   if (h == 64 || h == 128) return ks_launch_mlp_ws(p, n_in, h, num_sms, st);

@@ -49,15 +49,23 @@ struct Cfg256 {
   static constexpr int A1_BYTES = (K1 / 8) * kChunkBytes;
   static constexpr int A2_BYTES = (H / 8) * kChunkBytes;
   static constexpr int OFF_W1 = 0;
-  static constexpr int OFF_W2 = OFF_W1 + W1_BYTES;
+  static constexpr int OFF_B2IMG = OFF_W1 + W1_BYTES;         // directly in front of the W2 image (see BIAS_MMA below)
+  static constexpr int OFF_W2 = OFF_B2IMG + (NIN == 32 ? H * 16 : 0);
   static constexpr int OFF_A1 = OFF_W2 + W2_BYTES;
   static constexpr int OFF_A2 = OFF_A1 + A1_BYTES;
   static constexpr int OFF_W3 = OFF_A2 + A2_BYTES;            // [H] fp32 w3/2 of the current family
   static constexpr int OFF_B2 = OFF_W3 + H * 4;               // [H] fp32 b2
   static constexpr int OFF_RING = OFF_B2 + H * 4;             // [kRing][128] fp32 t_roof
   static constexpr int OFF_ZP = OFF_RING + kRing * kRows * 4; // [2][128] fp32 partial dots of warpgroup 1
+  // b2 through the tensor core (NIN = 32 only): one K chunk [H][8] bf16 with b2 hi / lo at positions 6, 7 -- where A1
+  // carries layer 1's constant-1 columns 22, 23 -- as the FIRST K chunk of a K = 16 MMA against A1 chunks 2, 3 (columns
+  // 16..31: six features that meet zero rows, the two ones, then eight zero columns); the second K chunk the MMA reads
+  // is whatever follows in shared memory, the first chunk of the W2 image: finite values that meet A1's zero columns
+  static constexpr bool BIAS_MMA = NIN == 32;
+  static constexpr int B2IMG_BYTES = BIAS_MMA ? H * 16 : 0;
   static constexpr int OFF_BAR = OFF_ZP + 2 * kRows * 4;
   static constexpr int SMEM_BYTES = OFF_BAR + 256;   // 21 barriers + TMEM slot (192) + TileMap
+  static_assert(SMEM_BYTES <= 232448, "shared memory");
 };
 
 // MMA2, D2_FREE, Z_FULL, Z_FREE come in pairs (column half of D2 / parity of the item)
@@ -246,10 +254,15 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
   #pragma unroll
             for (int j = 0; j < 16; j += 4) {
               const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col + j);
-              const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
               float x0, x1, x2, x3;
-              ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
-              ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
+              if (C::BIAS_MMA) {
+                x0 = __uint_as_float(a[j + 0]); x1 = __uint_as_float(a[j + 1]);
+                x2 = __uint_as_float(a[j + 2]); x3 = __uint_as_float(a[j + 3]);
+              } else {
+                const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
+                ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
+                ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
+              }
               if (GM == 0) {
                 float g0, g1, g2, g3;
                 gelu2_f32x2(x0, x1, g0, g1);
@@ -309,10 +322,15 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
 #pragma unroll
               for (int j = 0; j < 16; j += 4) {
                 const float4 w4 = *reinterpret_cast<const float4*>(sw3 + col + j);
-                const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
                 float x0, x1, x2, x3;
-                ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
-                ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
+                if (C::BIAS_MMA) {
+                  x0 = __uint_as_float(a[j + 0]); x1 = __uint_as_float(a[j + 1]);
+                  x2 = __uint_as_float(a[j + 2]); x3 = __uint_as_float(a[j + 3]);
+                } else {
+                  const float4 b4 = *reinterpret_cast<const float4*>(sb2 + col + j);
+                  ks_add2(x0, x1, __uint_as_float(a[j + 0]), __uint_as_float(a[j + 1]), b4.x, b4.y);
+                  ks_add2(x2, x3, __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]), b4.z, b4.w);
+                }
                 if (GM == 0) {
                   float g0, g1, g2, g3;
                   gelu2_f32x2(x0, x1, g0, g1);
@@ -416,7 +434,16 @@ KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, con
       ks_umma_bf16(d2 + (uint32_t)(h * (H / 2)), ad, bd, idesc_half, (first && kk == 0) ? 0u : 1u);
     }
     if (h == 1) ks_umma_commit(bars + BAR_A2_FREE + g);   // both passes have read this K group: EPI1 may rewrite it
-    if (last) ks_umma_commit(bars + BAR_MMA2 + h);
+    if (last) {
+      if (C::BIAS_MMA) {
+        // + b2: whatever item A1 holds by now, its columns 22, 23 are 1 and 24..31 are 0; the features beside them
+        // meet zero rows of the bias chunk (finite values: the producers may be rewriting them meanwhile)
+        const uint64_t ad = ks_umma_desc(a1_addr + 2 * kChunkBytes, kChunkBytes, 128);   // A1 chunks 2, 3
+        const uint64_t bd = ks_umma_desc(ks_smem_u32(smem + C::OFF_B2IMG) + h * (H / 2) * 16, B_LBO, 128);
+        ks_umma_bf16(d2 + (uint32_t)(h * (H / 2)), ad, bd, idesc_half, 1u);
+      }
+      ks_umma_commit(bars + BAR_MMA2 + h);
+    }
   };
 
   for (int b = 0; b < p.n_buckets; ++b) {
@@ -427,7 +454,10 @@ KS_DEV void mma_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, con
       ks_mbar_wait_backoff(bars + BAR_DRAIN, dphase);
       dphase ^= 1u;
     }
-    ks_mbar_expect_tx(bars + BAR_W, (uint32_t)(C::W1_BYTES + C::W2_BYTES));
+    ks_mbar_expect_tx(bars + BAR_W, (uint32_t)(C::W1_BYTES + C::W2_BYTES + C::B2IMG_BYTES));
+    if (C::BIAS_MMA)
+      ks_bulk_g2s(smem + C::OFF_B2IMG, reinterpret_cast<const char*>(p.head[b].w2_img) + (H + 16) * H * 2, C::B2IMG_BYTES,
+                  bars + BAR_W);
     ks_bulk_g2s(smem + C::OFF_W1, p.head[b].w1_img, C::W1_BYTES, bars + BAR_W);
     for (int off = 0; off < C::W2_BYTES; off += 32768)
       ks_bulk_g2s(smem + C::OFF_W2 + off, reinterpret_cast<const char*>(p.head[b].w2_img) + off, 32768, bars + BAR_W);
