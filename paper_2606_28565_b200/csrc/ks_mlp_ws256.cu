@@ -159,7 +159,7 @@ KS_DEV void epi1_items(const KsMlpParams& p, const uint32_t n_items, unsigned ch
       for (int j = 0; j < 8; ++j) {
         float g0, g1;
         gelu2_f32x2(__uint_as_float(a[2 * j]), __uint_as_float(a[2 * j + 1]), g0, g1);
-        pk[j] = ks_pack_bf16x2_alu(g0, g1);
+        pk[j] = ks_pack_bf16x2(g0, g1);
       }
     } else {
 #pragma unroll

@@ -217,8 +217,10 @@ KS_PTX uint32_t ks_pack_bf16x2(float lo, float hi) {
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
-// Same packing on the ALU pipe (IADD + PRMT) instead of F2FP, which shares the 16-lane XU pipe
-// with MUFU.TANH: round-to-nearest with ties away from zero (differs from RNE only on exact ties).
+// Same packing on the ALU pipe (IADD + PRMT) instead of F2FP: round-to-nearest with ties away from zero (differs from
+// RNE only on exact ties).  Not used by the kernels any more: the belief that F2FP costs MUFU.TANH throughput was
+// wrong -- a loop of one F2FP.BF16.F32.PACK_AB per MUFU.TANH runs at the MUFU rate alone (profiles/README.md) -- and the
+// two extra instructions per pair cost the H = 256 kernel 8 %.
 KS_PTX uint32_t ks_pack_bf16x2_alu(float lo, float hi) {
   return __byte_perm(__float_as_uint(lo) + 0x8000u, __float_as_uint(hi) + 0x8000u, 0x7632);
 }
