@@ -2,7 +2,7 @@
 // tcgen05 pipeline of ks_mlp_ws.cu re-laid-out for a head whose W2 image alone is 128 KiB.
 // S1-S3, S4a, S5 of DESIGN.md §1 (PAPER.md:191 Eq. 2, :199-201 per-family heads), fused.
 //
-// Shared memory holds W1, W2 (without bias rows), ONE A1 and ONE A2 buffer (225 KB in all) and TMEM
+// Shared memory holds W1, W2 (without bias rows), ONE A1 and ONE A2 buffer (225-229 KB in all) and TMEM
 // holds one D1 and one D2 (256 + 256 columns), so nothing is double-buffered by item; instead the
 // hand-over between layer 1 and layer 2 is pipelined at the granularity of 64-column K groups:
 //   warps 0-3    PRODUCER  thread = row: decode + roofline + features -> bf16 A1 (after MMA1 of the
@@ -16,14 +16,16 @@
 //                          on the tensor core under the rest of layer 1's activation work, and layer 1
 //                          of item q+1 is ready when EPI1 finishes item q
 //   warps 12-19  EPI2      both warpgroups take 64 columns of D2 half 0, then 64 columns of half 1 (warpgroup g: columns
-//                          [64 g, 64 g + 64) and [128 + 64 g, 128 + 64 g + 64)): + b2 (fp32) -> 2 GELU -> dot with w3/2;
+//                          [64 g, 64 g + 64) and [128 + 64 g, 128 + 64 g + 64)): (+ b2 in fp32 unless n_in = 32) -> 2 GELU -> dot with w3/2;
 //                          while they are on one half the tensor core refills the other with the next item (a clock64
 //                          trace showed the item period = activation of a half + its refill when a warpgroup owned a
 //                          whole half).  Ensembles keep a half per warpgroup (a member's columns stay in one warpgroup).
 //                          The two partial dots meet in shared memory; sigmoid, latency
 // so EPI1(q+1) and EPI2(q) share the MUFU pipe while the tensor core works on both items.
-// b2 is added in the fp32 epilogue here (in the H <= 128 kernels it rides through the tensor core
-// as one more K step): dropping the bias rows of W2 and the ones-block is what makes 225 KB fit.
+// b2: in the H <= 128 kernels it rides through the tensor core as one more K step against a ones-block; there is no
+// room for that here (12 KiB).  n_in = 32 (cfg5) gets it through the tensor core all the same: a 4 KiB bias chunk in
+// front of the W2 image and A1's own constant-1 columns as the A operand (Cfg256::BIAS_MMA); other widths add it in
+// the fp32 epilogue.
 // Every mbarrier completes exactly once per item, so its phase parity is q & 1; a waiter for item q
 // always runs before the completion for item q+1 can happen (that one depends on the waiter).
 #include <type_traits>
