@@ -324,12 +324,13 @@ ks_cfg_total_kernel(const __grid_constant__ KsComposeParams p) {
 }  // namespace
 
 cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_t st, int* launches) {
-  (void)num_sms;
   const long long total = (long long)p.n_specs * p.n_steps;
   if (total > 0) {
     // a cfg2-sized problem (thousands of steps) is a latency chain per CTA: 8-step chunks give four times
     // as many, lighter CTAs (measured 2.3 us off a 99.6 us cfg2 step); 100k-step problems keep 32-step chunks
-    const bool small = total <= kSmallSteps;
+    // ... unless 32-step chunks already give every SM two CTAs (cfg3: 16,384 steps of 256 rows = 512 chunks): then the
+    // eight-lanes-per-step reduction of the large chunks wins (cfg3 step kernel 13.4 us with 8-step chunks)
+    const bool small = total <= kSmallSteps && total / kS < 2ll * (num_sms > 0 ? num_sms : 148);
     const int ks = small ? kSmallS : kS;
     const long long n_chunks = (long long)((p.n_steps + ks - 1) / ks) * p.n_specs;
     if (n_chunks > 0x7fffffffll) return cudaErrorInvalidValue;
