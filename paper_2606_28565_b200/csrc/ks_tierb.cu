@@ -314,7 +314,6 @@ KS_DEV void run_bucket(const KsTierBParams& p, const int b, const int tile0, con
 template <bool F32, bool ONE, int NT>
 __global__ void __launch_bounds__(NT, 1) ks_tierb_kernel(const __grid_constant__ KsTierBParams p) {
   ks_launch_dependents();     // the next kernel of the stream may be scheduled now (it waits for us itself) ...
-  cudaGridDependencySynchronize();   // ... as we wait for the one before us (ks_launch_pdl)
   extern __shared__ __align__(128) float sgrid_f[];
   __shared__ __align__(8) uint64_t bar;
   const uint32_t sgrid = ks_smem_u32(sgrid_f);
@@ -335,6 +334,10 @@ __global__ void __launch_bounds__(NT, 1) ks_tierb_kernel(const __grid_constant__
       ks_bulk_g2s(reinterpret_cast<char*>(sgrid_f) + o, reinterpret_cast<const char*>(p.grid[b].values) + o,
                   min(32768u, bytes - o), &bar);
   }
+  // ... as we wait for the one before us (ks_launch_pdl) -- AFTER the grid's bulk copies have been issued: the grid is
+  // model data that ks_load_grid copied in synchronously, nothing on the stream writes it, so its staging (128 KiB per
+  // CTA) may overlap the tail of the preceding kernel; descriptor columns and outputs are touched only below
+  cudaGridDependencySynchronize();
   if (p.bk[b].family == KS_FAM_GEMM) run_bucket<KS_FAM_GEMM, F32, ONE, NT>(p, b, t0, t1, sgrid, &bar, 0u);
   else run_bucket<KS_FAM_ATTN, F32, ONE, NT>(p, b, t0, t1, sgrid, &bar, 0u);
 }
