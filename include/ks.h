@@ -240,7 +240,9 @@ KS_API ks_status ks_compose_steps_weighted(ks_ctx *ctx, const float *const *late
  * KS_MEM_DEVICE with KS_TIER_NONE, one spec vector, int32 columns, no multiplicities, at most four buckets and no
  * grouped-GEMM bucket (config 4a's shape) runs as ONE kernel plus the totals kernel: the latencies are computed in the
  * step kernel's staging phase instead of being written to HBM and read back, and latency[b] is written only where the
- * caller passed a buffer (none: a step moves the descriptor columns only).  Same bits as the two-call path. */
+ * caller passed a buffer (none: a step moves the descriptor columns only).  Per-kernel latencies are bit-identical to
+ * ks_predict_kernels'; step and configuration latencies are summed in the same fixed order as ks_compose_steps'
+ * (bit-identical wherever that call stages a chunk in shared memory, within 2e-6 relative otherwise). */
 KS_API ks_status ks_run_steps(ks_ctx *ctx, const ks_desc_batch *batches, const int32_t *const *step_off,
                        int n_batches, const ks_hw_spec *specs, int n_specs, ks_tier tier, int n_steps,
                        const ks_step_params *params, const int32_t *cfg_off, int n_cfg,
