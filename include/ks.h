@@ -237,8 +237,9 @@ KS_API ks_status ks_compose_steps_weighted(ks_ctx *ctx, const float *const *late
  * pipelined in the caller's order (bucket b is copied while bucket b-1 is predicted: largest first is best);
  * pinned host memory is what makes the copies asynchronous, and the columns of a bucket that lie back to
  * back in host memory (cols[k+1] == cols[k] + 4 n, n a multiple of 4) move with a single copy.
- * KS_MEM_DEVICE with KS_TIER_NONE, one spec vector, int32 columns, no multiplicities, at most four buckets and no
- * grouped-GEMM bucket (config 4a's shape) runs as ONE kernel plus the totals kernel: the latencies are computed in the
+ * KS_MEM_DEVICE with KS_TIER_NONE, one spec vector, int32 columns, at most eight buckets and no grouped-GEMM bucket
+ * (config 4a's shape, with or without multiplicities: also what ks_sim_run prices at Tier NONE) runs as ONE kernel plus
+ * the totals kernel: the latencies are computed in the
  * step kernel's staging phase instead of being written to HBM and read back, and latency[b] is written only where the
  * caller passed a buffer (none: a step moves the descriptor columns only).  Per-kernel latencies are bit-identical to
  * ks_predict_kernels'; step and configuration latencies are summed in the same fixed order as ks_compose_steps'

@@ -986,18 +986,19 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
   if (c->sticky) return KS_ECUDA;
   KS_CUDA(c, cudaSetDevice(c->device));
 
-  // Tier NONE with one spec vector and no multiplicities (config 4a's shape): ONE kernel computes the latencies in
+  // Tier NONE with one spec vector (config 4a's shape; also the closed loop's weighted rows): ONE kernel computes the latencies in
   // the step kernel's staging phase (ks_fused.cu) instead of writing them to HBM and reading them back; per-kernel
   // latencies are written only where the caller passed a buffer.  Same bits as the two-call path.
   if (dev && tier == KS_TIER_NONE && n_specs == 1 && n_steps > 0 && n_batches >= 1 && n_batches <= KS_FUSED_MAX_BUCKETS) {
-    bool fusable = true;
+    bool fusable = true, weighted = false;
     long long rows = 0;
     for (int b = 0; b < n_batches; ++b) {
-      fusable = fusable && !batches[b].mult && ks_fused_none_supported(batches[b].family, batches[b].col_dtype == KS_COL_F32);
+      fusable = fusable && ks_fused_none_supported(batches[b].family, batches[b].col_dtype == KS_COL_F32);
+      weighted = weighted || batches[b].mult != nullptr;
       rows += batches[b].n;
     }
-    // an average chunk of 32 steps must fit the 47 KiB staging buffer (a chunk that does not is summed from the columns)
-    fusable = fusable && (double)rows / (double)n_steps * 32.0 <= 0.85 * 12032.0;
+    // an average chunk of 32 steps must fit the staging buffer (a chunk that does not is summed from the columns)
+    fusable = fusable && (double)rows / (double)n_steps * 32.0 <= 0.85 * (double)ks_fused_none_cap_floats(weighted);
     if (fusable) {
       KsFusedParams p;
       memset(&p, 0, sizeof(p));
@@ -1006,6 +1007,7 @@ ks_status ks_run_steps(ks_ctx* c, const ks_desc_batch* batches, const int32_t* c
         o.lat = latency ? latency[b] : nullptr;
         p.bk[b] = make_bucket_dev(batches[b], batches[b].cols, o, 0);
         p.step_off[b] = step_off[b];
+        p.mult[b] = batches[b].mult;
       }
       p.n_batches = n_batches;
       p.n_steps = n_steps;

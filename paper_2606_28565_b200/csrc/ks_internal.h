@@ -113,10 +113,11 @@ cudaError_t ks_launch_compose(const KsComposeParams& p, int num_sms, cudaStream_
 cudaError_t ks_launch_cfg_totals(const KsComposeParams& p, cudaStream_t st, bool after_ours, int* launches);
 
 // ---- Tier NONE, one spec, unweighted: decode + roofline + floor + step sums + Eq. 4 in one kernel: ks_fused.cu
-#define KS_FUSED_MAX_BUCKETS 4
+#define KS_FUSED_MAX_BUCKETS 8
 struct KsFusedParams {
   KsBucketDev bk[KS_FUSED_MAX_BUCKETS];      // lat may be nullptr: the per-kernel latencies are not written then
   const int32_t* step_off[KS_FUSED_MAX_BUCKETS];
+  const int32_t* mult[KS_FUSED_MAX_BUCKETS];  // optional per-row multiplicities (nullptr = ones)
   int32_t n_batches, n_steps, cap_floats, pad;
   ks_step_params sp;
   KsSpecDev spec;
@@ -124,6 +125,7 @@ struct KsFusedParams {
 };
 bool ks_fused_none_supported(int family, bool col_f32);
 cudaError_t ks_launch_fused_none(const KsFusedParams& p, cudaStream_t st);
+int ks_fused_none_cap_floats(bool weighted);   // staging capacity of a chunk (floats)
 
 // Every libks kernel is launched with programmatic stream serialization and opens with
 //   griddepcontrol.launch_dependents;  cudaGridDependencySynchronize();

@@ -133,18 +133,78 @@ def test_fused_ragged_steps_empty_steps_and_a_chunk_that_does_not_fit(ks):
         assert np.all(a[0, used:] == -1.0)                     # rows behind the last step belong to no step: untouched
 
 
-def test_fused_is_not_taken_with_multiplicities_or_several_specs(ks):
-    """Weighted rows and spec sweeps keep the two-kernel path (same results as before: three or more launches)."""
+@pytest.mark.parametrize("tp", [1, 2])
+def test_fused_weighted_rows_match_two_calls_and_oracle(ks, tp):
+    """Layer-homogeneous rows (a row stands for m_k identical kernels): the one-kernel path stages
+    m_k t_k and the multiplicities; per-kernel latencies stay unweighted and bit-identical, step latencies agree with
+    ks_predict_kernels + ks_compose_steps_weighted to fp32 rounding (a product and a sum instead of one FMA) and with
+    the oracle to 1e-5; Eq. 4's launch count is the sum of the multiplicities (c_disp = 4 us makes it visible)."""
+    B, D = ks
+    w = W.config4(n_steps=1203, n_layers=6, dedupe=True, tp=tp)
+    assert any(b.mult is not None for b in w.buckets)
+    ctx = B.Context(0)
+    try:
+        db = D.to_device(w)
+        g = D.predict(ctx, w, dbuckets=db)
+        step2, tot2 = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+        step1, tot1, lat1, launches = run_fused(B, D, ctx, w, db, True)
+        assert launches == 2
+        step0, tot0, _, _ = run_fused(B, D, ctx, w, db, False)
+    finally:
+        ctx.close()
+    lats = [O.predict_bucket(b, w.specs, W.TIER_NONE)["lat"][0] for b in w.buckets]
+    so, to = O.compose(lats, [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off,
+                       mults=[b.mult for b in w.buckets])
+    assert all(np.array_equal(a, b_["lat"]) for a, b_ in zip(lat1, g))
+    assert rel_err(step1[0], so).max() <= TOL_F32 and rel_err(tot1[0], to).max() <= TOL_F32
+    assert rel_err(step1[0], step2[0]).max() <= 2e-6 and rel_err(tot1[0], tot2[0]).max() <= 2e-6
+    assert np.array_equal(step0, step1) and np.array_equal(tot0, tot1)
+
+
+def test_fused_six_buckets(ks):
+    """More than four buckets (the closed loop's fine model slots make six): the eight-bucket instance."""
+    B, D = ks
+    rng = np.random.Generator(np.random.PCG64(5))
+    w = W.config2(n=60_000)
+    w.tier = W.TIER_NONE
+    import copy
+    w.buckets = w.buckets + [copy.deepcopy(b) for b in w.buckets]
+    n_steps = 700
+    for b in w.buckets:
+        cnt = rng.multinomial(b.n - 7, np.full(n_steps, 1.0 / n_steps))
+        b.step_off = np.concatenate([[0], np.cumsum(cnt)]).astype(np.int32)
+    w.n_steps = n_steps
+    w.cfg_off = np.array([0, 100, 700], np.int32)
+    ctx = B.Context(0)
+    try:
+        db = D.to_device(w)
+        g = D.predict(ctx, w, dbuckets=db)
+        step2, tot2 = D.compose(ctx, w, [x["lat_dev"] for x in g], db)
+        step1, tot1, lat1, launches = run_fused(B, D, ctx, w, db, True)
+        assert launches == 2
+    finally:
+        ctx.close()
+    lats, so, to = oracle_steps(w)
+    assert rel_err(step1[0], so).max() <= TOL_F32 and rel_err(tot1[0], to).max() <= TOL_F32
+    assert rel_err(step1[0], step2[0]).max() <= 2e-6
+    for a, b_, bk in zip(lat1, g, w.buckets):
+        used = int(bk.step_off[-1])
+        assert np.array_equal(a[0, :used], b_["lat"][0, :used])
+
+
+def test_fused_is_not_taken_with_several_specs(ks):
+    """A spec sweep keeps the two-kernel path (three or more launches), with the same results as before."""
     B, D = ks
     import torch
-    w = W.config4(n_steps=61, n_layers=6, dedupe=True)
+    w = W.config4(n_steps=61, n_layers=6)
+    w.specs = [W.spec_gb200(), W.spec_gb200(n_sm=132, peak_flops=1.0e15)]
     ctx = B.Context(0)
     try:
         db = D.to_device(w)
         n_cfg = len(w.cfg_off) - 1
         cfg = torch.from_numpy(np.ascontiguousarray(w.cfg_off, dtype=np.int32)).cuda()
-        step = torch.empty((1, w.n_steps), dtype=torch.float32, device="cuda")
-        tot = torch.empty((1, n_cfg), dtype=torch.float32, device="cuda")
+        step = torch.empty((2, w.n_steps), dtype=torch.float32, device="cuda")
+        tot = torch.empty((2, n_cfg), dtype=torch.float32, device="cuda")
         n0 = ctx.launch_count()
         ctx.run_steps(db, [b.step_off for b in db], w.specs, W.TIER_NONE, w.n_steps, w.step_params, cfg, n_cfg, step, tot)
         torch.cuda.synchronize()
@@ -152,7 +212,7 @@ def test_fused_is_not_taken_with_multiplicities_or_several_specs(ks):
         step = step.cpu().numpy()
     finally:
         ctx.close()
-    lats = [O.predict_bucket(b, w.specs, W.TIER_NONE)["lat"][0] for b in w.buckets]
-    so, _ = O.compose(lats, [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off,
-                      mults=[b.mult for b in w.buckets])
-    assert rel_err(step[0], so).max() <= TOL_F32
+    for s in range(2):
+        lats = [O.predict_bucket(b, w.specs, W.TIER_NONE)["lat"][s] for b in w.buckets]
+        so, _ = O.compose(lats, [b.step_off for b in w.buckets], w.n_steps, w.step_params, w.cfg_off)
+        assert rel_err(step[s], so).max() <= TOL_F32
