@@ -243,6 +243,8 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
         uint32_t accA[16], accB[16];
         ks_tmem_ld16(d2, accA);
         const float t_roof = ring[(qi & (kRing - 1)) * kRows + r];
+        float t0 = p.specs.s[s].t0;                 // (an indexed constant load: issued here, used after the sweep)
+        asm volatile("" : "+f"(t0));
         float z0 = 0.0f, z1 = 0.0f, z2 = 0.0f, z3 = 0.0f;
         auto act_dot = [&](const uint32_t* a, int c16) {
           if (GM == 0) {
@@ -306,7 +308,7 @@ KS_DEV void epi2_all(const KsMlpParams& p, const TileMap& tm, const int t_lo, co
             // guarded at e >= 2^-10 (Q3); Eq. 2 floor after eta
             eta = fminf(out_add + __expf(fmaxf(out_sgn * z, out_lo)), 1024.0f);
           }
-          lat[(long long)s * bn + row] = fmaxf(t_roof * eta, p.specs.s[s].t0);
+          lat[(long long)s * bn + row] = fmaxf(t_roof * eta, t0);
         }
       }
       s += 2;
