@@ -64,7 +64,8 @@ cudaError_t ks_launch_stream_small(const KsStreamSmallParams& p, cudaStream_t st
 #define KS_MLP_MAX_BUCKETS 4
 struct KsHeadDev {
   const void* w1_img;      // bf16 UMMA image [K1/8][H][8]  (rows n_in, n_in+1 hold b1 hi/lo)
-  const void* w2_img;      // bf16 UMMA image [(H+16)/8][H][8] (K rows H, H+1 hold b2 hi/lo)
+  const void* w2_img;      // bf16 UMMA image [(H+24)/8][H][8] (K rows H, H+1 hold b2 hi/lo; the last K chunk holds them again at
+                           // the chunk positions of layer 1's constant-1 columns: the H = 256 kernel's bias MMA, ks_mlp_ws256.cu)
   const float* w3;         // fp32 [H], holds w3 / 2
   const float* b2;         // fp32 [H] (the H = 256 kernel adds b2 in its fp32 epilogue)
   float b3;
